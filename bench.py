@@ -1,0 +1,400 @@
+#!/usr/bin/env python
+"""bench.py — response samples/s of the LISA response hot path (lr_project + lr_tdi) on B200.
+
+Contract: `python bench.py --gpus N --steps K --warmup W` prints ONE JSON line.
+  * a step = one pass of the whole hot path (six-link projection + TDI-2) over one batch of synthetic input;
+  * N = 1 workload = BASELINE.json configs[1]: one Galactic binary, 1 year at dt = 10 s (3,153,600 samples),
+    Keplerian orbits, Lagrange order 25, nested second-generation TDI, X,Y,Z + A,E,T;  `--workload batch`
+    times configs[2] (MCMC batch, templates/s) in chunks instead;
+  * N > 1: every rank runs the same-sized workload on its own seeded template(s) (the path shards over
+    templates with no collective: "scaling": "weak"); time = max over ranks, value = all ranks' samples / time;
+  * `value` has the inputs resident in HBM; `e2e` goes through lr_response_host with pinned HOST buffers;
+  * `roofline`: the dominant kernel (TDI) against the FP64 issue rate measured live by lr_measure_fp64_peak;
+  * `cpu_baseline` / `--impl reference`: the oracle (fp64 arithmetic, all host cores) on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+# algorithmic FP64 instruction slots per time sample (SURVEY.md §8(d), T = order + 1 taps; DFMA = 1)
+def ops_project(T):
+    return 63 * T + 300
+
+
+def ops_tdi(T, gen):
+    return (252 * T + 336 if gen == 2 else 108 * T + 170) + 10
+
+
+# algorithmic HBM bytes per time sample
+BYTES_PROJECT = 16 + 48
+
+
+def bytes_tdi(nout):
+    return 48 + 8 * nout
+
+
+# ------------------------------------------------------------------------------------------ distributed
+def _dist():
+    import torch.distributed as dist
+    return dist if dist.is_available() and dist.is_initialized() else None
+
+
+def _reduce(x, op):
+    import torch
+    dist = _dist()
+    if dist is None:
+        return float(x)
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([float(x)], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=op)
+    return float(t.item())
+
+
+def max_over_ranks(x):
+    import torch.distributed as dist
+    return _reduce(x, dist.ReduceOp.MAX)
+
+
+def sum_over_ranks(x):
+    import torch.distributed as dist
+    return _reduce(x, dist.ReduceOp.SUM)
+
+
+def barrier():
+    dist = _dist()
+    if dist is not None:
+        dist.barrier()
+
+
+# ----------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self._stop, self._thr = [], set(), threading.Event(), None
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self._nv = None
+
+    def _run(self):
+        nv = self._nv
+        names = {"hw_slowdown": nv.nvmlClocksThrottleReasonHwSlowdown,
+                 "hw_thermal_slowdown": nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksThrottleReasonSwThermalSlowdown,
+                 "sw_power_cap": nv.nvmlClocksThrottleReasonSwPowerCap}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h)
+                self.reasons.update(k for k, bit in names.items() if r & bit)
+            except Exception:
+                pass
+            self._stop.wait(0.02)
+
+    def __enter__(self):
+        if self._nv:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+
+    def summary(self):
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# -------------------------------------------------------------------------------------------- workloads
+def make_workload(kind, rank):
+    """The benchmarked workload of this rank: (Workload descriptor, number of templates per step)."""
+    from paper_2204_06633_b200 import inputs
+    if kind == "year":
+        w = inputs.config(2)
+        if rank:  # other ranks: same shape, their own seeded source
+            w.sources = [inputs.draw_gb(np.random.default_rng(2204 + rank))]
+        return w, 1
+    if kind == "batch":
+        w = inputs.config(3)
+        lo, hi = 0, len(w.sources)
+        return w, hi - lo
+    if kind == "tiny":
+        return inputs.config(1), 1
+    raise ValueError(kind)
+
+
+def gb_waveform_device(srcs, n, dt, t0, device):
+    """The configs' GB waveform family evaluated on the device (input generation only; not timed)."""
+    import torch
+    t = t0 + dt * torch.arange(n, dtype=torch.float64, device=device)
+    hp = torch.empty((len(srcs), n), dtype=torch.float64, device=device)
+    hc = torch.empty_like(hp)
+    for b, s in enumerate(srcs):
+        ph = s.phi0 + 2.0 * np.pi * (s.f0 * t + 0.5 * s.fdot * t * t)
+        ci = np.cos(s.iota)
+        hp[b] = s.A * (1.0 + ci * ci) * torch.cos(ph)
+        hc[b] = -2.0 * s.A * ci * torch.sin(ph)
+    return hp, hc
+
+
+# ------------------------------------------------------------------------------------------ CPU oracle
+def time_oracle(w, target_s=12.0):
+    """The oracle as it stands (oracle/lr_oracle.cpp, fp64 arithmetic, OpenMP over samples) on a window of
+    the workload's first template, sized for about target_s of host time.  Returns (samples/s, info)."""
+    from oracle import oracle as orc
+    tab = w.table()
+    O = orc.Oracle(tab, w.dt, w.t0, w.order)
+    hp, hc = w.waveform(0)
+    s = w.sources[0]
+    mp, mf, mb = O.margins(w.tdi_gen)
+    ch = {"XYZ": 0, "AET": 1, "XYZ_AET": 2}[w.channels]
+    cores = os.cpu_count() or 1
+    mid = w.n // 2
+
+    def run(m):
+        lo, hi = mid, min(mid + m, w.n - mb)
+        t0 = time.perf_counter()
+        y = O.project(hp, hc, s.beta, s.lam, s.psi, lo=max(mp, lo - (mf - mp)), hi=hi, precision="d")
+        O.tdi(y, w.tdi_gen, nested=True, channels=ch, lo=lo, hi=hi, precision="d")
+        return time.perf_counter() - t0, hi - lo
+
+    t_probe, m_probe = run(2000)
+    m = int(max(2000, min(w.n - mb - mid, m_probe * target_s / max(t_probe, 1e-6))))
+    t, m = run(m)
+    return m / t, {"cores": cores, "kind": "oracle",
+                   "sample": f"{m} consecutive samples from the middle of template 0 (projection + TDI-{w.tdi_gen}, "
+                             f"fp64 build of the oracle, OpenMP over samples), {t:.1f} s wall"}
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle on the host cores, same metric/config; rank 0 only."""
+    if rank != 0:
+        return
+    w, _ = make_workload(args.workload, 0)
+    vals, info = [], None
+    per_step = max(1.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    for i in range(args.warmup + args.steps):
+        v, info = time_oracle(w, target_s=per_step)
+        if i >= args.warmup:
+            vals.append(v)
+    v = float(np.mean(vals))
+    line = {"impl": "reference", "metric": "response samples/s (6-link proj + TDI-2, fp64)", "value": v,
+            "unit": "samples/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * w.n / v, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_config(w, 1, args),
+            "cpu_baseline": dict(info, value=v, unit="samples/s"),
+            "e2e": {"value": v, "unit": "samples/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(w, batch, args):
+    return {"workload": f"BASELINE.json configs[{ {'tiny': 0, 'year': 1, 'batch': 2}[args.workload] }] ({w.name})",
+            "batch": batch, "n": w.n, "dt": w.dt, "lagrange_order": w.order, "tdi_gen": w.tdi_gen,
+            "chain": "nested", "channels": w.channels, "orbits": w.orbit_kind,
+            "l2": "flushed between steps (256 MiB memset outside the per-step event pairs)"}
+
+
+# --------------------------------------------------------------------------------------------- GPU arm
+def run_gpu(args, rank, world, local_rank):
+    import torch
+    import paper_2204_06633_b200 as lr
+    lr.binding.lib()  # no CUDA extension -> fail loudly, there is no fallback
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    w, batch = make_workload(args.workload, rank)
+    chunk = min(batch, args.chunk)
+    n, T = w.n, w.order + 1
+    nout = 6 if w.channels == "XYZ_AET" else 3
+    R = lr.Response(w.table(), w.dt, w.order, w.tdi_gen, t0=w.t0, chain="nested", channels=w.channels)
+    stream = torch.cuda.current_stream()
+
+    y = torch.empty((chunk, 6, n), dtype=torch.float64, device=dev)
+    out = torch.empty((chunk, nout, n), dtype=torch.float64, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    chunks = [(lo, min(lo + chunk, batch)) for lo in range(0, batch, chunk)]
+
+    def angles(lo, hi):
+        src = w.sources[lo:hi]
+        return [s.beta for s in src], [s.lam for s in src], [s.psi for s in src]
+
+    if batch == 1:
+        hp_np, hc_np = w.waveform(0)
+        h_cache = {0: (torch.from_numpy(hp_np).to(dev)[None], torch.from_numpy(hc_np).to(dev)[None])}
+    else:
+        h_cache = {}
+
+    def chunk_inputs(lo, hi):
+        if lo not in h_cache:
+            h_cache.clear()
+            h_cache[lo] = gb_waveform_device(w.sources[lo:hi], n, w.dt, w.t0, dev)
+        return h_cache[lo]
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def step(timed):
+        """One pass over the whole batch; returns (ms project, ms tdi) from CUDA events on the launch stream."""
+        tp = tt = 0.0
+        for lo, hi in chunks:
+            hp, hc = chunk_inputs(lo, hi)
+            be, la, ps = angles(lo, hi)
+            flush.zero_()
+            e0, e1, e2 = ev(), ev(), ev()
+            e0.record(stream)
+            R.project(hp, hc, be, la, ps, y_out=y[:hi - lo])
+            e1.record(stream)
+            R.tdi(y[:hi - lo], out=out[:hi - lo])
+            e2.record(stream)
+            if timed:
+                e2.synchronize()
+                tp += e0.elapsed_time(e1)
+                tt += e1.elapsed_time(e2)
+        return tp, tt
+
+    for _ in range(args.warmup):
+        step(False)
+    torch.cuda.synchronize()
+    peak = lr.lr_measure_fp64_peak(args.peak_seconds)   # FP64 thread-instructions / s, this device, now
+    barrier()
+    torch.cuda.synchronize()
+    launches0 = lr.lr_launch_count()
+    tps, tts = [], []
+    wall0 = time.perf_counter()
+    with ClockSampler(local_rank) as clk:
+        for _ in range(args.steps):
+            a, b = step(True)
+            tps.append(a)
+            tts.append(b)
+        torch.cuda.synchronize()
+    barrier()
+    wall = time.perf_counter() - wall0
+    launches = lr.lr_launch_count() - launches0
+    ms_proj, ms_tdi = float(np.mean(tps)), float(np.mean(tts))
+    ms_step = max_over_ranks(ms_proj + ms_tdi)
+    units = sum_over_ranks(float(batch) * n)
+    value = units / (ms_step * 1e-3)
+    templates = sum_over_ranks(float(batch))
+
+    # end to end through the C ABI with pinned HOST buffers (H2D + project + TDI + D2H inside the timed region)
+    eb = min(batch, args.e2e_templates)
+    hp_h = torch.empty((eb, n), dtype=torch.float64).pin_memory()
+    hc_h = torch.empty((eb, n), dtype=torch.float64).pin_memory()
+    out_h = torch.empty((eb, nout, n), dtype=torch.float64).pin_memory()
+    hp_d, hc_d = chunk_inputs(0, min(chunk, batch))
+    hp_h.copy_(hp_d[:eb].cpu())
+    hc_h.copy_(hc_d[:eb].cpu())
+    be, la, ps = angles(0, eb)
+    for _ in range(max(1, min(args.warmup, 3))):
+        R.response_host(hp_h, hc_h, be, la, ps, out_h)
+    torch.cuda.synchronize()
+    barrier()
+    e2e_ms = []
+    for _ in range(max(3, min(args.steps, 10))):
+        flush.zero_()
+        torch.cuda.synchronize()
+        e0, e1 = ev(), ev()
+        e0.record(stream)
+        R.response_host(hp_h, hc_h, be, la, ps, out_h)
+        e1.record(stream)
+        e1.synchronize()
+        e2e_ms.append(e0.elapsed_time(e1))
+    e2e_ms = max_over_ranks(float(np.mean(e2e_ms)))
+    e2e_units = sum_over_ranks(float(eb) * n)
+
+    if rank != 0:
+        return
+    ops_t, ops_p = ops_tdi(T, w.tdi_gen), ops_project(T)
+    ach_tdi = ops_t * batch * n / (ms_tdi * 1e-3)
+    ach_proj = ops_p * batch * n / (ms_proj * 1e-3)
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(args.workload, {}).get("tdi_kernel_bytes_per_launch")
+        except Exception:
+            traffic = None
+    line = {
+        "metric": "response samples/s (6-link proj + TDI-2, fp64)" if args.workload != "batch"
+                  else "response samples/s (6-link proj + TDI-2 AET, fp64), batched",
+        "value": value, "unit": "samples/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": dict(workload_config(w, batch, args), chunk_templates=chunk,
+                       parallelism=f"{world} rank(s), templates sharded, no collective"),
+        "templates_per_s": templates / (ms_step * 1e-3),
+        "e2e": {"value": e2e_units / (e2e_ms * 1e-3), "unit": "samples/s", "ms_per_step": e2e_ms,
+                "templates": eb, "h2d_bytes_per_step": 2 * eb * n * 8, "d2h_bytes_per_step": nout * eb * n * 8,
+                "api": "lr_response_host (pinned host buffers)"},
+        "gpu_launches": launches,
+        "kernels": {"lr_project": {"ms": ms_proj, "alg_ops_per_sample": ops_p, "gops": ach_proj / 1e9,
+                                   "frac_fp64": ach_proj / peak, "alg_GBps": BYTES_PROJECT * batch * n / (ms_proj * 1e6)},
+                    "lr_tdi": {"ms": ms_tdi, "alg_ops_per_sample": ops_t, "gops": ach_tdi / 1e9,
+                               "frac_fp64": ach_tdi / peak, "alg_GBps": bytes_tdi(nout) * batch * n / (ms_tdi * 1e6)}},
+        "roofline": {"bound": "alu", "kernel": "tdi_kernel (lr_tdi)", "achieved": ach_tdi / 1e9, "peak": peak / 1e9,
+                     "unit": "Gop/s (FP64 thread-instruction slots, DFMA = 1)", "frac": ach_tdi / peak,
+                     "traffic": traffic,
+                     "peak_source": f"lr_measure_fp64_peak({args.peak_seconds} s DFMA kernel) on this device, this run",
+                     "path_frac": (ops_t + ops_p) * batch * n / ((ms_proj + ms_tdi) * 1e-3) / peak},
+        "clocks": clk.summary(), "wall_s_timed_region": wall,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        v, info = time_oracle(w, target_s=args.cpu_seconds)
+        line["cpu_baseline"] = dict(info, value=v, unit="samples/s")
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="year", choices=["year", "batch", "tiny"])
+    ap.add_argument("--chunk", type=int, default=64, help="templates per launch (batch workload)")
+    ap.add_argument("--e2e-templates", type=int, default=4)
+    ap.add_argument("--peak-seconds", type=float, default=1.0)
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    try:
+        run_gpu(args, rank, world, local_rank)
+    finally:
+        if world > 1:
+            import torch.distributed as dist
+            dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

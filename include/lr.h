@@ -1,0 +1,142 @@
+/* lr.h — C ABI of liblr: the generic time-domain LISA response on one B200 (sm_100a).
+ *
+ * The library computes the data-parallel hot path of arXiv:2204.06633:
+ *   stage 1  lr_project : the six single-link responses y_ij(t)          (eqs. 10-16)
+ *   stage 2  lr_tdi     : first/second-generation TDI X,Y,Z and A,E,T     (eqs. 17-21)
+ * over arbitrary orbits given as a table that lr_create turns into device-resident cubic splines
+ * ("interpolated and then evaluated at each evenly-spaced time step"), with centred
+ * Lagrange fractional-delay interpolation of user-defined order, batched over templates
+ * (one response per walker per MCMC step).
+ *
+ * Conventions (DESIGN.md §3 lists the readings A1..A16 behind them)
+ *   - every array is fp64, C-contiguous; "DEVICE" = CUDA device memory of the current device,
+ *     "HOST" = ordinary host memory.  The caller owns every buffer it passes.
+ *   - link slots are ordered [12, 23, 31, 13, 32, 21]; link ij is received on spacecraft i and was
+ *     emitted by spacecraft j.
+ *   - sample n of every series (h, y, out) is at time t0 + n*dt (LR_OPT_T0, default orbits->t_start).
+ *   - "order" is the polynomial degree of the Lagrange interpolant: order+1 taps, order odd (1..65).
+ *   - L_ij are light travel TIMES in seconds ("the delay time").
+ *   - outputs are fully written; samples inside the fixed margins (lr_get_margins) are exactly 0.0.
+ *   - lr_project / lr_tdi enqueue work on `cuda_stream` (a cudaStream_t, NULL = legacy default stream)
+ *     and return without synchronising.  lr_response_host is synchronous.
+ *   - all entry points return 0 on success or a negative LR_E* code; they never abort, throw or print.
+ *     Inputs are not scanned for NaN (NaN propagates).
+ *   - there is no CPU fallback: every call that computes needs a CUDA device and fails with LR_ECUDA
+ *     otherwise.
+ */
+#ifndef LR_H_
+#define LR_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lr_handle lr_handle; /* opaque; owns the device spline coefficients and small staging buffers */
+
+/* Orbit table on uniform knots (§IV.D: positions and light travel times as
+ * delivered by an orbit product).  lr_create copies it; the caller may free it on return. */
+typedef struct {
+  int64_t n_knots;   /* >= 4 */
+  double t_start;    /* time of knot 0 [s] */
+  double knot_dt;    /* uniform knot spacing [s] (> 0), e.g. 86400 */
+  const double* x;   /* HOST [3 spacecraft][3 xyz][n_knots], metres, SSB frame */
+  const double* ltt; /* HOST [6 links: 12,23,31,13,32,21][n_knots], seconds */
+} lr_orbits;
+
+/* error codes */
+#define LR_OK 0
+#define LR_EINVAL (-1)  /* null pointer, bad order / generation / dt / sizes */
+#define LR_ERANGE (-2)  /* the sample span (with the backward reach of the delays) leaves the knot table */
+#define LR_ECUDA (-3)   /* a CUDA call failed; lr_last_cuda_error gives the CUDA code */
+#define LR_ENOMEM (-4)  /* host allocation failed */
+
+/* option keys for lr_set_option */
+#define LR_OPT_T0 1       /* time of sample 0 [s]; default orbits->t_start */
+#define LR_OPT_CHAIN 2    /* LR_CHAIN_NESTED (default) | LR_CHAIN_SUM */
+#define LR_OPT_CHANNELS 3 /* LR_XYZ (default) | LR_AET | LR_XYZ_AET */
+#define LR_OPT_TDI_GEN 4  /* 1 | 2: changes the generation given to lr_create */
+
+/* Chained delays D_{i1 i2 ... in} (eqs. 19-20).
+ *   LR_CHAIN_SUM    : eq. 20 verbatim, the sum of the L's all taken at t.
+ *   LR_CHAIN_NESTED : d_0 = 0, d_k = d_{k-1} + L_{i_k i_{k+1}}(t - d_{k-1}) (leftmost pair at t); the whole
+ *                     chain is applied as ONE interpolation at t - d_n. */
+#define LR_CHAIN_NESTED 0
+#define LR_CHAIN_SUM 1
+
+/* Output channels of lr_tdi (eq. 21). LR_XYZ_AET writes [X,Y,Z,A,E,T]. */
+#define LR_XYZ 0
+#define LR_AET 1
+#define LR_XYZ_AET 2
+
+#define LR_MAX_ORDER 65
+
+/* Build a response object: fit a not-a-knot cubic spline to each of the 15 orbit channels on the host,
+ * upload the per-interval coefficients, fix the margins.  dt = sample spacing of h, y and out [s];
+ * lagrange_order odd in [1, LR_MAX_ORDER]; tdi_gen in {1, 2}.  *out receives the handle.
+ * Errors: LR_EINVAL, LR_ENOMEM, LR_ECUDA. */
+int lr_create(const lr_orbits* orbits, double dt, int lagrange_order, int tdi_gen, lr_handle** out);
+
+/* Free the handle and its device memory (NULL is allowed).  Work enqueued earlier must have finished. */
+void lr_destroy(lr_handle* h);
+
+/* Set an option (see LR_OPT_*).  Errors: LR_EINVAL for an unknown key or value. */
+int lr_set_option(lr_handle* h, int key, double value);
+
+/* Fixed margins in samples (reading A8), computed once from the table maxima R_max = max|x_i|
+ * and L_max = max L_ij over the knots, p = (order+1)/2:
+ *   m_proj      = ceil((1.001 R_max/c + 1.001 L_max)/dt) + p + 2          y is 0 outside [m_proj, n - m_proj)
+ *   m_tdi_front = m_proj + ceil(G 1.001 L_max/dt) + p + 2, G = 4 (gen 1) | 8 (gen 2)
+ *   m_tdi_back  = m_proj + p + 2                              out is 0 outside [m_tdi_front, n - m_tdi_back)
+ * Any of the three pointers may be NULL. */
+int lr_get_margins(const lr_handle* h, int64_t* m_proj, int64_t* m_tdi_front, int64_t* m_tdi_back);
+
+/* Stage 1 (eqs. 10-16).  For every template b and sample n in [m_proj, n - m_proj), t = t0 + n dt:
+ *   k,u,v from (beta, lambda) per eq. 10, (u,v) rotated by psi (equivalent to eq. 9's rotation of h by 2 psi);
+ *   n_ij = (x_i(t) - x_j(t))/|.|, xi+ = (u.n)^2 - (v.n)^2, xix = 2 (u.n)(v.n)                    (eq. 12)
+ *   y_ij = [xi+ (h+(t_e) - h+(t_r)) + xix (hx(t_e) - hx(t_r))] / (2 (1 - k.n_ij))               (eq. 16)
+ *   t_e = t - L_ij(t) - k.x_j(t)/c,  t_r = t - k.x_i(t)/c, h evaluated by Lagrange interpolation.
+ * h_plus, h_cross : DEVICE [batch][n];  beta (ecliptic latitude), lambda (ecliptic longitude), psi : HOST [batch]
+ * y_out : DEVICE [batch][6][n].  Requires n > 2 m_proj and n < 2^31 - 2^20.
+ * Errors: LR_EINVAL, LR_ERANGE, LR_ECUDA. */
+int lr_project(lr_handle* h, const double* h_plus, const double* h_cross, const double* beta,
+               const double* lambda, const double* psi, int64_t batch, int64_t n, double* y_out,
+               void* cuda_stream);
+
+/* Stage 2 (eqs. 17-21).  y : DEVICE [batch][6][n] (any handle's lr_project output — a handle with
+ * other orbits gives the paper's hybrid templates).  out : DEVICE [batch][3][n] (LR_XYZ,
+ * LR_AET) or [batch][6][n] (LR_XYZ_AET).  Requires n > m_tdi_front + m_tdi_back.
+ * Errors: LR_EINVAL, LR_ERANGE, LR_ECUDA. */
+int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out, void* cuda_stream);
+
+/* Both stages with HOST buffers: copies h_plus/h_cross [batch][n] to the device, runs lr_project on
+ * `h_proj` and lr_tdi on `h_tdi` (may be the same handle), copies out [batch][3|6][n] back and waits.
+ * Device scratch is owned by h_proj and grown on demand (kept until lr_destroy).
+ * `cuda_stream` as above.  Errors: as lr_project / lr_tdi, LR_ECUDA for a failed allocation or copy. */
+int lr_response_host(lr_handle* h_proj, lr_handle* h_tdi, const double* h_plus, const double* h_cross,
+                     const double* beta, const double* lambda, const double* psi, int64_t batch, int64_t n,
+                     double* out, void* cuda_stream);
+
+/* Evaluate the device spline of one orbit channel (0..8 = x[i][a] as i*3+a, 9..14 = L link slots) at
+ * `m` times t (DEVICE [m]) into out (DEVICE [m]); used by the tests to pin the orbit ingestion. */
+int lr_eval_orbit(lr_handle* h, int channel, const double* t, int64_t m, double* out, void* cuda_stream);
+
+/* Measure this device's FP64 issue rate with a DFMA-only kernel that runs for about `seconds`:
+ * *inst_per_s = FP64 thread-instructions per second (one DFMA = 1).  The roofline denominator of bench.py.
+ * Synchronous.  Errors: LR_EINVAL, LR_ECUDA. */
+int lr_measure_fp64_peak(double seconds, double* inst_per_s);
+
+/* Number of kernels liblr has launched in this process (all handles); bench.py's gpu_launches. */
+int64_t lr_launch_count(void);
+
+/* CUDA error code (cudaError_t as int) of the last failed CUDA call on this handle, 0 if none. */
+int lr_last_cuda_error(const lr_handle* h);
+
+/* Static description of an LR_* code. */
+const char* lr_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LR_H_ */

@@ -1,0 +1,206 @@
+"""ctypes binding of liblr (include/lr.h).  Argument marshalling only.
+
+Every function below has the name and the meaning of the C entry point it calls; all arithmetic of the
+response runs in the CUDA kernels of csrc/.  There is no CPU fallback: if liblr.so is missing or cannot
+be loaded the import of the library fails loudly (`LrUnavailable`), and every computing call needs a CUDA
+device.  PyTorch is used only for device memory and streams.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblr.so")
+
+LR_OK, LR_EINVAL, LR_ERANGE, LR_ECUDA, LR_ENOMEM = 0, -1, -2, -3, -4
+LR_OPT_T0, LR_OPT_CHAIN, LR_OPT_CHANNELS, LR_OPT_TDI_GEN = 1, 2, 3, 4
+LR_CHAIN_NESTED, LR_CHAIN_SUM = 0, 1
+LR_XYZ, LR_AET, LR_XYZ_AET = 0, 1, 2
+LR_MAX_ORDER = 65
+
+# every symbol include/lr.h declares
+SYMBOLS = ("lr_create", "lr_destroy", "lr_set_option", "lr_get_margins", "lr_project", "lr_tdi",
+           "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count",
+           "lr_last_cuda_error", "lr_strerror")
+
+
+class LrUnavailable(RuntimeError):
+    """liblr.so is not built / not loadable.  The library has no CPU path."""
+
+
+class LrError(RuntimeError):
+    def __init__(self, code, where, cuda=0):
+        self.code = code
+        self.cuda = cuda
+        msg = lib().lr_strerror(code).decode()
+        super().__init__(f"{where}: {msg} (code {code}" + (f", cudaError {cuda})" if cuda else ")"))
+
+
+class lr_orbits(ctypes.Structure):
+    _fields_ = [("n_knots", ctypes.c_int64), ("t_start", ctypes.c_double), ("knot_dt", ctypes.c_double),
+                ("x", ctypes.c_void_p), ("ltt", ctypes.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    """The loaded liblr (ctypes.CDLL) with argument types set."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise LrUnavailable(f"{LIB_PATH} not found: build it with `python -m paper_2204_06633_b200.build` "
+                            "(nvcc, sm_100a).  There is no CPU fallback.")
+    try:
+        L = ctypes.CDLL(LIB_PATH)
+    except OSError as e:  # pragma: no cover
+        raise LrUnavailable(f"cannot load {LIB_PATH}: {e}") from e
+    i64, dbl, vp, ci = ctypes.c_int64, ctypes.c_double, ctypes.c_void_p, ctypes.c_int
+    pi64 = ctypes.POINTER(i64)
+    L.lr_create.argtypes = [ctypes.POINTER(lr_orbits), dbl, ci, ci, ctypes.POINTER(vp)]
+    L.lr_create.restype = ci
+    L.lr_destroy.argtypes = [vp]
+    L.lr_destroy.restype = None
+    L.lr_set_option.argtypes = [vp, ci, dbl]
+    L.lr_get_margins.argtypes = [vp, pi64, pi64, pi64]
+    L.lr_project.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
+    L.lr_tdi.argtypes = [vp, vp, i64, i64, vp, vp]
+    L.lr_response_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
+    L.lr_eval_orbit.argtypes = [vp, ci, vp, i64, vp, vp]
+    L.lr_measure_fp64_peak.argtypes = [dbl, ctypes.POINTER(dbl)]
+    L.lr_launch_count.argtypes = []
+    L.lr_launch_count.restype = i64
+    L.lr_last_cuda_error.argtypes = [vp]
+    L.lr_strerror.argtypes = [ci]
+    L.lr_strerror.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+def _host(a):
+    return np.ascontiguousarray(np.atleast_1d(a), dtype=np.float64)
+
+
+def _check(rc, where, handle=None):
+    if rc != LR_OK:
+        cuda = lib().lr_last_cuda_error(handle) if handle else 0
+        raise LrError(rc, where, cuda)
+
+
+def _dev_ptr(t, name, numel=None):
+    """data_ptr of a contiguous fp64 CUDA tensor."""
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+        raise TypeError(f"{name} must be a contiguous float64 CUDA tensor")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{name} has {t.numel()} elements, expected {numel}")
+    return t.data_ptr()
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+# ------------------------------------------------------------------------------------------------ C calls
+def lr_create(table, dt, lagrange_order, tdi_gen):
+    """lr_create: `table` has .n_knots .t_start .knot_dt .x[3,3,K] .ltt[6,K] (host numpy).  Returns a handle."""
+    x, ltt = _host(table.x), _host(table.ltt)
+    if x.size != 9 * table.n_knots or ltt.size != 6 * table.n_knots:
+        raise ValueError("orbit table: x must be [3,3,n_knots] and ltt [6,n_knots]")
+    orb = lr_orbits(int(table.n_knots), float(table.t_start), float(table.knot_dt),
+                    x.ctypes.data_as(ctypes.c_void_p), ltt.ctypes.data_as(ctypes.c_void_p))
+    h = ctypes.c_void_p()
+    _check(lib().lr_create(ctypes.byref(orb), float(dt), int(lagrange_order), int(tdi_gen), ctypes.byref(h)),
+           "lr_create")
+    return h
+
+
+def lr_destroy(h):
+    lib().lr_destroy(h)
+
+
+def lr_set_option(h, key, value):
+    _check(lib().lr_set_option(h, int(key), float(value)), "lr_set_option", h)
+
+
+def lr_get_margins(h):
+    a, b, c = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
+    _check(lib().lr_get_margins(h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)), "lr_get_margins", h)
+    return a.value, b.value, c.value
+
+
+def lr_project(h, h_plus, h_cross, beta, lam, psi, y_out, stream=None):
+    """lr_project: h_plus, h_cross CUDA [B,N]; beta, lam, psi host [B]; y_out CUDA [B,6,N] (written)."""
+    beta, lam, psi = _host(beta), _host(lam), _host(psi)
+    B = beta.size
+    if lam.size != B or psi.size != B:
+        raise ValueError("beta, lambda, psi must have one entry per template")
+    if h_plus.numel() % B:
+        raise ValueError("h_plus size is not a multiple of the batch")
+    n = h_plus.numel() // B
+    _check(lib().lr_project(h, _dev_ptr(h_plus, "h_plus"), _dev_ptr(h_cross, "h_cross", B * n),
+                            beta.ctypes.data, lam.ctypes.data, psi.ctypes.data, B, n,
+                            _dev_ptr(y_out, "y_out", B * 6 * n), _stream(stream)), "lr_project", h)
+    return y_out
+
+
+def lr_tdi(h, y, out, batch, stream=None):
+    """lr_tdi: y CUDA [B,6,N]; out CUDA [B,3|6,N] (written)."""
+    if y.numel() % (6 * batch):
+        raise ValueError("y must be [batch,6,n]")
+    n = y.numel() // (6 * batch)
+    if out.numel() not in (3 * batch * n, 6 * batch * n):
+        raise ValueError("out must be [batch,3,n] or [batch,6,n]")
+    _check(lib().lr_tdi(h, _dev_ptr(y, "y"), batch, n, _dev_ptr(out, "out"), _stream(stream)), "lr_tdi", h)
+    return out
+
+
+def lr_response_host(h_proj, h_tdi, h_plus, h_cross, beta, lam, psi, out, stream=None):
+    """lr_response_host: host numpy (or pinned CPU tensors viewed as numpy) in, host out; synchronous."""
+    beta, lam, psi = _host(beta), _host(lam), _host(psi)
+    B = beta.size
+    hp, hc = _as_host_f64(h_plus), _as_host_f64(h_cross)
+    o = _as_host_f64(out)
+    n = hp.size // B
+    if hp.size != B * n or hc.size != B * n or o.size not in (3 * B * n, 6 * B * n):
+        raise ValueError("lr_response_host: inconsistent sizes")
+    _check(lib().lr_response_host(h_proj, h_tdi, hp.ctypes.data, hc.ctypes.data, beta.ctypes.data,
+                                  lam.ctypes.data, psi.ctypes.data, B, n, o.ctypes.data,
+                                  _stream(stream) if stream is not None else _stream(None)),
+           "lr_response_host", h_proj)
+    return out
+
+
+def _as_host_f64(a):
+    if hasattr(a, "numpy") and not isinstance(a, np.ndarray):
+        a = a.numpy()  # CPU (possibly pinned) torch tensor: shares memory
+    if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]):
+        raise TypeError("host buffers must be C-contiguous float64")
+    return a
+
+
+def lr_eval_orbit(h, channel, t, out, stream=None):
+    _check(lib().lr_eval_orbit(h, int(channel), _dev_ptr(t, "t"), t.numel(), _dev_ptr(out, "out", t.numel()),
+                               _stream(stream)), "lr_eval_orbit", h)
+    return out
+
+
+def lr_measure_fp64_peak(seconds=0.5):
+    v = ctypes.c_double()
+    _check(lib().lr_measure_fp64_peak(float(seconds), ctypes.byref(v)), "lr_measure_fp64_peak")
+    return v.value
+
+
+def lr_launch_count():
+    return int(lib().lr_launch_count())
+
+
+def lr_strerror(code):
+    return lib().lr_strerror(int(code)).decode()

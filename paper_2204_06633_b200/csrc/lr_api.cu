@@ -1,0 +1,314 @@
+// lr_api.cu — host side of liblr: the C ABI of include/lr.h.
+//
+// lr_create fits the orbit splines on the host (long double) and uploads per-interval cubic coefficients;
+// lr_project / lr_tdi marshal arguments and launch the kernels of lr_kernels.cuh on the caller's stream.
+// There is no CPU compute path: without a CUDA device every computing call returns LR_ECUDA.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <string.h>
+
+#include <atomic>
+#include <new>
+#include <vector>
+
+#include "../../include/lr.h"
+#include "lr_host.hpp"
+#include "lr_kernels.cuh"
+
+namespace lr {
+extern std::atomic<int64_t> g_launches;
+}
+
+namespace {
+
+constexpr int kSlots = 4;  // ring of staging buffers for the per-template source basis
+
+struct Stage {
+  double* host = nullptr;  // pinned
+  double* dev = nullptr;
+  int64_t cap = 0;         // templates
+  cudaEvent_t done = nullptr;
+  bool pending = false;
+};
+
+}  // namespace
+
+struct lr_handle {
+  // configuration
+  double dt = 0, t_start = 0, knot_dt = 0, t0 = 0;
+  int64_t n_knots = 0;
+  int order = 0, p = 0, gen = 2, chain = LR_CHAIN_NESTED, channels = LR_XYZ;
+  double r_max = 0, l_max = 0;
+  double bk[lr::kPMax + 1];
+  // device state
+  lr::D4* coef = nullptr;
+  Stage stage[kSlots];
+  int next_slot = 0;
+  // scratch of lr_response_host
+  double* scratch = nullptr;
+  size_t scratch_bytes = 0;
+  int last_cuda = 0;
+
+  int64_t m_proj() const {
+    return (int64_t)ceil((1.001 * r_max / lr::kC + 1.001 * l_max) / dt) + p + 2;
+  }
+  int64_t tdi_reach(int g) const { return (int64_t)ceil((double)(g == 1 ? 4 : 8) * 1.001 * l_max / dt); }
+  int64_t m_front(int g) const { return m_proj() + tdi_reach(g) + p + 2; }
+  int64_t m_back() const { return m_proj() + p + 2; }
+};
+
+namespace {
+
+#define LR_CUDA(h, call)                      \
+  do {                                        \
+    cudaError_t e__ = (call);                 \
+    if (e__ != cudaSuccess) {                 \
+      (h)->last_cuda = (int)e__;              \
+      return LR_ECUDA;                        \
+    }                                         \
+  } while (0)
+
+lr::Params make_params(const lr_handle* h, int64_t n) {
+  lr::Params P;
+  memset(&P, 0, sizeof(P));
+  P.coef = h->coef;
+  P.nint = (int)(h->n_knots - 1);
+  P.p = h->p;
+  P.trel0 = (double)((long double)h->t0 - (long double)h->t_start);
+  P.dt = h->dt;
+  P.inv_h = 1.0 / h->knot_dt;
+  P.inv_dt = 1.0 / h->dt;
+  P.inv_cdt = 1.0 / (lr::kC * h->dt);
+  P.n = (int)n;
+  P.m_proj = (int)h->m_proj();
+  P.m_front = (int)h->m_front(h->gen);
+  P.m_back = (int)h->m_back();
+  memcpy(P.bk, h->bk, sizeof(P.bk));
+  return P;
+}
+
+bool size_ok(int64_t batch, int64_t n) {
+  return batch >= 1 && n >= 1 && n < ((int64_t)1 << 31) - ((int64_t)1 << 20) &&
+         batch <= (((int64_t)1 << 31) - 1) / ((n + 255) / 256);
+}
+
+// the times the kernels evaluate the splines at must lie inside the knot table (no extrapolation)
+bool in_table(const lr_handle* h, int64_t n_first, int64_t n_last, double back_reach) {
+  const long double span = (long double)(h->n_knots - 1) * h->knot_dt;
+  const long double rel0 = (long double)h->t0 - (long double)h->t_start;
+  const long double lo = rel0 + (long double)n_first * h->dt - back_reach;
+  const long double hi = rel0 + (long double)n_last * h->dt;
+  return lo >= 0 && hi <= span;
+}
+
+int stage_basis(lr_handle* h, const double* beta, const double* lam, const double* psi, int64_t batch,
+                cudaStream_t st, Stage** used) {
+  Stage& S = h->stage[h->next_slot];
+  h->next_slot = (h->next_slot + 1) % kSlots;
+  if (!S.done) LR_CUDA(h, cudaEventCreateWithFlags(&S.done, cudaEventDisableTiming));
+  if (S.pending) { LR_CUDA(h, cudaEventSynchronize(S.done)); S.pending = false; }
+  if (S.cap < batch) {
+    if (S.host) cudaFreeHost(S.host);
+    if (S.dev) cudaFree(S.dev);
+    S.host = nullptr; S.dev = nullptr; S.cap = 0;
+    LR_CUDA(h, cudaMallocHost(&S.host, (size_t)batch * 9 * sizeof(double)));
+    LR_CUDA(h, cudaMalloc(&S.dev, (size_t)batch * 9 * sizeof(double)));
+    S.cap = batch;
+  }
+  for (int64_t b = 0; b < batch; ++b) lr::source_basis(beta[b], lam[b], psi[b], S.host + 9 * b);
+  LR_CUDA(h, cudaMemcpyAsync(S.dev, S.host, (size_t)batch * 9 * sizeof(double), cudaMemcpyHostToDevice, st));
+  *used = &S;
+  return LR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lr_create(const lr_orbits* orb, double dt, int order, int tdi_gen, lr_handle** out) {
+  if (!orb || !out || !orb->x || !orb->ltt) return LR_EINVAL;
+  if (!(dt > 0) || !(orb->knot_dt > 0) || orb->n_knots < 4 || orb->n_knots > ((int64_t)1 << 30)) return LR_EINVAL;
+  if (order < 1 || order > LR_MAX_ORDER || order % 2 == 0) return LR_EINVAL;
+  if (tdi_gen != 1 && tdi_gen != 2) return LR_EINVAL;
+  const int64_t nk = orb->n_knots;
+  for (int64_t i = 0; i < 9 * nk; ++i)
+    if (!isfinite(orb->x[i])) return LR_EINVAL;
+  for (int64_t i = 0; i < 6 * nk; ++i)
+    if (!isfinite(orb->ltt[i]) || orb->ltt[i] < 0) return LR_EINVAL;
+
+  lr_handle* h = new (std::nothrow) lr_handle();
+  if (!h) return LR_ENOMEM;
+  h->dt = dt; h->t_start = orb->t_start; h->knot_dt = orb->knot_dt; h->t0 = orb->t_start;
+  h->n_knots = nk; h->order = order; h->p = (order + 1) / 2; h->gen = tdi_gen;
+
+  // table maxima for the margins (reading A8)
+  for (int64_t k = 0; k < nk; ++k)
+    for (int i = 0; i < 3; ++i) {
+      double r = 0;
+      for (int a = 0; a < 3; ++a) { const double v = orb->x[((int64_t)i * 3 + a) * nk + k]; r += v * v; }
+      r = sqrt(r);
+      if (r > h->r_max) h->r_max = r;
+    }
+  for (int64_t k = 0; k < 6 * nk; ++k)
+    if (orb->ltt[k] > h->l_max) h->l_max = orb->ltt[k];
+
+  lr::pair_constants(h->p, h->bk);
+
+  std::vector<lr::D4> coef;
+  try { coef.resize((size_t)15 * (nk - 1)); } catch (...) { delete h; return LR_ENOMEM; }
+  try {
+    for (int ch = 0; ch < 9; ++ch) lr::fit_channel(orb->x + (int64_t)ch * nk, nk, orb->knot_dt, coef.data() + (size_t)ch * (nk - 1));
+    for (int s = 0; s < 6; ++s) lr::fit_channel(orb->ltt + (int64_t)s * nk, nk, orb->knot_dt, coef.data() + (size_t)(9 + s) * (nk - 1));
+  } catch (...) { delete h; return LR_ENOMEM; }
+
+  cudaError_t e = cudaMalloc(&h->coef, coef.size() * sizeof(lr::D4));
+  if (e == cudaSuccess) e = cudaMemcpy(h->coef, coef.data(), coef.size() * sizeof(lr::D4), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    if (h->coef) cudaFree(h->coef);
+    delete h;
+    *out = nullptr;
+    return LR_ECUDA;
+  }
+  *out = h;
+  return LR_OK;
+}
+
+void lr_destroy(lr_handle* h) {
+  if (!h) return;
+  for (int s = 0; s < kSlots; ++s) {
+    Stage& S = h->stage[s];
+    if (S.pending) cudaEventSynchronize(S.done);
+    if (S.done) cudaEventDestroy(S.done);
+    if (S.host) cudaFreeHost(S.host);
+    if (S.dev) cudaFree(S.dev);
+  }
+  if (h->scratch) cudaFree(h->scratch);
+  if (h->coef) cudaFree(h->coef);
+  delete h;
+}
+
+int lr_set_option(lr_handle* h, int key, double value) {
+  if (!h || !isfinite(value)) return LR_EINVAL;
+  switch (key) {
+    case LR_OPT_T0: h->t0 = value; return LR_OK;
+    case LR_OPT_CHAIN:
+      if (value != LR_CHAIN_NESTED && value != LR_CHAIN_SUM) return LR_EINVAL;
+      h->chain = (int)value; return LR_OK;
+    case LR_OPT_CHANNELS:
+      if (value != LR_XYZ && value != LR_AET && value != LR_XYZ_AET) return LR_EINVAL;
+      h->channels = (int)value; return LR_OK;
+    case LR_OPT_TDI_GEN:
+      if (value != 1 && value != 2) return LR_EINVAL;
+      h->gen = (int)value; return LR_OK;
+    default: return LR_EINVAL;
+  }
+}
+
+int lr_get_margins(const lr_handle* h, int64_t* m_proj, int64_t* m_front, int64_t* m_back) {
+  if (!h) return LR_EINVAL;
+  if (m_proj) *m_proj = h->m_proj();
+  if (m_front) *m_front = h->m_front(h->gen);
+  if (m_back) *m_back = h->m_back();
+  return LR_OK;
+}
+
+int lr_project(lr_handle* h, const double* hp, const double* hc, const double* beta, const double* lam,
+               const double* psi, int64_t batch, int64_t n, double* y, void* stream) {
+  if (!h || !hp || !hc || !beta || !lam || !psi || !y) return LR_EINVAL;
+  if (!size_ok(batch, n) || n <= 2 * h->m_proj()) return LR_EINVAL;
+  const int64_t mp = h->m_proj();
+  if (!in_table(h, mp, n - mp - 1, 0.0)) return LR_ERANGE;
+  cudaStream_t st = (cudaStream_t)stream;
+  Stage* S = nullptr;
+  int rc = stage_basis(h, beta, lam, psi, batch, st, &S);
+  if (rc != LR_OK) return rc;
+  lr::Params P = make_params(h, n);
+  P.halo_lo = (int)mp; P.halo_hi = (int)mp;
+  P.ntiles = (int)((n + lr::kProjThreads - 1) / lr::kProjThreads);
+  const int e = lr::launch_project(P, h->order, hp, hc, S->dev, y, batch, stream);
+  if (e != 0) { h->last_cuda = e; return LR_ECUDA; }
+  LR_CUDA(h, cudaEventRecord(S->done, st));
+  S->pending = true;
+  return LR_OK;
+}
+
+int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out, void* stream) {
+  if (!h || !y || !out) return LR_EINVAL;
+  const int64_t mf = h->m_front(h->gen), mb = h->m_back();
+  if (!size_ok(batch, n) || n <= mf + mb) return LR_EINVAL;
+  const double reach = (double)(h->gen == 1 ? 4 : 8) * 1.001 * h->l_max;
+  if (!in_table(h, mf, n - mb - 1, reach)) return LR_ERANGE;
+  lr::Params P = make_params(h, n);
+  P.halo_lo = (int)(mf - h->m_proj()); P.halo_hi = h->p + 2;
+  P.ntiles = (int)((n + lr::kTdiThreads - 1) / lr::kTdiThreads);
+  const int e = lr::launch_tdi(P, h->order, h->gen, h->chain, h->channels, y, out, batch, stream);
+  if (e != 0) { h->last_cuda = e; return LR_ECUDA; }
+  return LR_OK;
+}
+
+int lr_response_host(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const double* h_cross, const double* beta,
+                     const double* lam, const double* psi, int64_t batch, int64_t n, double* out, void* stream) {
+  lr_handle* h = hp_;
+  if (!h || !ht_ || !h_plus || !h_cross || !beta || !lam || !psi || !out) return LR_EINVAL;
+  if (!size_ok(batch, n)) return LR_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int nout = ht_->channels == LR_XYZ_AET ? 6 : 3;
+  const size_t per = (size_t)n * sizeof(double) * (size_t)(2 + 6 + nout);  // device bytes per template
+  const size_t limit = (size_t)8 << 30;
+  int64_t chunk = (int64_t)(limit / per);
+  if (chunk < 1) chunk = 1;
+  if (chunk > batch) chunk = batch;
+  const size_t need = per * (size_t)chunk;
+  if (h->scratch_bytes < need) {
+    if (h->scratch) { cudaFree(h->scratch); h->scratch = nullptr; h->scratch_bytes = 0; }
+    LR_CUDA(h, cudaMalloc(&h->scratch, need));
+    h->scratch_bytes = need;
+  }
+  for (int64_t b0 = 0; b0 < batch; b0 += chunk) {
+    const int64_t nb = (batch - b0 < chunk) ? batch - b0 : chunk;
+    double* d_hp = h->scratch;
+    double* d_hc = d_hp + (size_t)nb * n;
+    double* d_y = d_hc + (size_t)nb * n;
+    double* d_out = d_y + (size_t)nb * 6 * n;
+    LR_CUDA(h, cudaMemcpyAsync(d_hp, h_plus + (size_t)b0 * n, (size_t)nb * n * sizeof(double), cudaMemcpyHostToDevice, st));
+    LR_CUDA(h, cudaMemcpyAsync(d_hc, h_cross + (size_t)b0 * n, (size_t)nb * n * sizeof(double), cudaMemcpyHostToDevice, st));
+    int rc = lr_project(h, d_hp, d_hc, beta + b0, lam + b0, psi + b0, nb, n, d_y, stream);
+    if (rc != LR_OK) return rc;
+    rc = lr_tdi(ht_, d_y, nb, n, d_out, stream);
+    if (rc != LR_OK) { h->last_cuda = ht_->last_cuda; return rc; }
+    LR_CUDA(h, cudaMemcpyAsync(out + (size_t)b0 * nout * n, d_out, (size_t)nb * nout * n * sizeof(double),
+                               cudaMemcpyDeviceToHost, st));
+  }
+  LR_CUDA(h, cudaStreamSynchronize(st));
+  return LR_OK;
+}
+
+int lr_eval_orbit(lr_handle* h, int channel, const double* t, int64_t m, double* out, void* stream) {
+  if (!h || !t || !out || channel < 0 || channel > 14 || m < 1) return LR_EINVAL;
+  lr::Params P = make_params(h, 1);
+  const int threads = 256;
+  const int64_t blocks = (m + threads - 1) / threads;
+  if (blocks > 0x7fffffff) return LR_EINVAL;
+  lr::eval_orbit_kernel<<<(unsigned)blocks, threads, 0, (cudaStream_t)stream>>>(P, channel, h->t_start, t, m, out);
+  lr::g_launches.fetch_add(1);
+  LR_CUDA(h, cudaGetLastError());
+  return LR_OK;
+}
+
+int64_t lr_launch_count(void) { return lr::g_launches.load(); }
+
+int lr_last_cuda_error(const lr_handle* h) { return h ? h->last_cuda : 0; }
+
+const char* lr_strerror(int code) {
+  switch (code) {
+    case LR_OK: return "success";
+    case LR_EINVAL: return "invalid argument";
+    case LR_ERANGE: return "sample span (with the delays' backward reach) is not covered by the orbit table";
+    case LR_ECUDA: return "CUDA error (see lr_last_cuda_error)";
+    case LR_ENOMEM: return "host allocation failed";
+    default: return "unknown error code";
+  }
+}
+
+}  // extern "C"

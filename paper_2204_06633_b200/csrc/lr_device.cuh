@@ -1,0 +1,288 @@
+// lr_device.cuh — per-sample arithmetic of the LISA response (device functions).
+//
+// Everything here is the product's own restatement of arXiv:2204.06633 (eqs. 10-21); it shares
+// nothing with oracle/.  The functions are LR_HD (__host__ __device__) so that a host harness can single-
+// step them while debugging; the library itself only ever calls them from kernels.
+//
+// Numerical design:
+//   * the sample index stays an integer; a delay D (in samples) is split as I = ceil(D), eps = I - D in
+//     [0,1), and the stencil is addressed with integers only;
+//   * Lagrange weights come from the pair factorisation (eps-k)(eps-1+k) = z - k(k-1), z = eps^2 - eps,
+//     with prefix/suffix products over the P = (order+1)/2 pairs: no division, regular at eps = 0;
+//   * an interpolated value is returned as  x[a] - S  with a = the sample just above the target and S a
+//     weighted sum of exact first differences (summation by parts, the constant mode removed
+//     structurally), so that differences of interpolations of one series (Delta h in eq. 16, the +/- pairs
+//     of eqs. 17-18) lose no digits to cancellation.
+#pragma once
+#include <math.h>
+#include <stdint.h>
+
+#ifdef __CUDACC__
+#define LR_HD __host__ __device__ __forceinline__
+#else
+#define LR_HD inline
+#define __host__
+#define __device__
+#endif
+
+namespace lr {
+
+constexpr int kPMax = 33;        // order <= 65
+constexpr double kC = 299792458.0;  // m/s
+
+struct alignas(16) D2 { double x, y; };
+struct alignas(32) D4 { double x, y, z, w; };
+
+// link slots [12,23,31,13,32,21] -> receiver / emitter (0-based spacecraft)
+__host__ __device__ constexpr int link_rx(int s) { return s == 0 ? 0 : s == 1 ? 1 : s == 2 ? 2 : s == 3 ? 0 : s == 4 ? 2 : 1; }
+__host__ __device__ constexpr int link_tx(int s) { return s == 0 ? 1 : s == 1 ? 2 : s == 2 ? 0 : s == 3 ? 2 : s == 4 ? 1 : 0; }
+// slot of link (rx i, tx j), 0-based
+__host__ __device__ constexpr int link_slot(int i, int j) {
+  return (i == 0 && j == 1) ? 0 : (i == 1 && j == 2) ? 1 : (i == 2 && j == 0) ? 2
+       : (i == 0 && j == 2) ? 3 : (i == 2 && j == 1) ? 4 : 5;
+}
+// the circular permutation 1->2->3->1 applied r times to a slot
+__host__ __device__ constexpr int rot_slot(int s, int r) {
+  return link_slot((link_rx(s) + r) % 3, (link_tx(s) + r) % 3);
+}
+
+// Kernel parameters shared by both stages (passed by value).
+struct Params {
+  const D4* coef;      // DEVICE [15][nint] cubic coefficients (c0,c1,c2,c3) in u = (t - t_i)/h in [0,1)
+  int nint;            // spline intervals = n_knots - 1
+  int p;               // P = (order+1)/2
+  double trel0;        // t0 - t_start  [s]
+  double dt;           // sample spacing [s]
+  double inv_h;        // 1 / knot_dt
+  double inv_dt;       // 1 / dt
+  double inv_cdt;      // 1 / (c dt)
+  int n;               // samples per template
+  int m_proj, m_front, m_back;
+  int halo_lo, halo_hi;  // staged window = [n0 - halo_lo, n0 + B + halo_hi)
+  int ntiles;
+  double bk[kPMax + 1];  // bk[k] = 1 / prod_{m != k} (k - m), m = -P+1..P, for k = 1..P
+};
+
+LR_HD D4 load4(const D4* p) {
+#ifdef __CUDA_ARCH__
+  const double2 lo = __ldg(reinterpret_cast<const double2*>(p));
+  const double2 hi = __ldg(reinterpret_cast<const double2*>(p) + 1);
+  return D4{lo.x, lo.y, hi.x, hi.y};
+#else
+  return *p;
+#endif
+}
+
+// time of sample n relative to knot 0
+LR_HD double sample_trel(const Params& P, int n) { return fma((double)n, P.dt, P.trel0); }
+
+// cubic spline channel `ch` at relative time trel (reading A9)
+LR_HD double spline_eval(const Params& P, int ch, double trel) {
+  const double s = trel * P.inv_h;
+  int i = (int)floor(s);
+  i = i < 0 ? 0 : (i > P.nint - 1 ? P.nint - 1 : i);
+  const double u = s - (double)i;
+  const D4 c = load4(P.coef + (int64_t)ch * P.nint + i);
+  return fma(fma(fma(c.w, u, c.z), u, c.y), u, c.x);
+}
+
+// Split a delay of D samples: anchor index a = n - ceil(D) + 1 (the sample just above the target
+// n - D), eps = ceil(D) - D in [0,1).  Stencil taps are a-P .. a+P-1.
+LR_HD void split_delay(double D, int n, int& a, double& eps) {
+  const double I = ceil(D);
+  eps = I - D;
+  a = n - (int)I + 1;
+}
+
+// Centred Lagrange interpolation of NS series that share one target, in summation-by-parts form.
+//   value_s = raw_s[a] - S[s],   S[s] = sum_{j=1-P}^{0} C_j dif_s[a-1+j] - sum_{j=1}^{P-1} E_j dif_s[a-1+j]
+// with C_j = sum_{j'<=j} w_j', E_j = sum_{j'>j} w_j' and dif_s[m] = raw_s[m+1] - raw_s[m].
+// `dif(m, out)` fetches the NS first differences at staged index m.  PT > 0 fixes P at compile time.
+template <int PT, int NS, class Dif>
+LR_HD void interp_sbp(const Params& prm, double eps, int a, Dif dif, double (&S)[NS]) {
+  const int P = PT > 0 ? PT : prm.p;
+  double R[PT > 0 ? PT : kPMax];
+  const double z = fma(eps, eps, -eps);
+  // ascending pass: R[k-1] = b_k * prod_{k'<k} G_k',  G_k = (eps-k)(eps-1+k) = z - k(k-1)
+  double pre = 1.0;
+#pragma unroll
+  for (int k = 1; k <= P; ++k) {
+    R[k - 1] = pre * prm.bk[k];
+    pre *= z - (double)(k * (k - 1));
+  }
+  // descending pass: complete the pair products, build running sums C (taps below the target, outside
+  // in) and E (taps above, outside in), and accumulate against the first differences.
+  double suf = 1.0, C = 0.0, E = 0.0;
+  double lo[NS], hi[NS];
+#pragma unroll
+  for (int s = 0; s < NS; ++s) { lo[s] = 0.0; hi[s] = 0.0; }
+  const int q = a - 1;
+#pragma unroll
+  for (int k = P; k >= 1; --k) {
+    const double Rk = R[k - 1] * suf;            // b_k prod_{k' != k} G_k'
+    suf *= z - (double)(k * (k - 1));
+    C = fma(Rk, (double)k - eps, C);             // += w_{1-k}
+    double d[NS];
+    dif(q + 1 - k, d);
+#pragma unroll
+    for (int s = 0; s < NS; ++s) lo[s] = fma(C, d[s], lo[s]);
+    if (k >= 2) {
+      E = fma(Rk, eps + (double)(k - 1), E);     // += w_k
+      dif(q + k - 1, d);
+#pragma unroll
+      for (int s = 0; s < NS; ++s) hi[s] = fma(E, d[s], hi[s]);
+    }
+  }
+#pragma unroll
+  for (int s = 0; s < NS; ++s) S[s] = lo[s] - hi[s];
+}
+
+// ---------------------------------------------------------------------------------------------- stage 1
+// One time sample of eqs. 10-16 for all six links.  raw/dif: staged (h+, hx) pairs and their first
+// differences, W entries; nl = this sample's staged index; bs = k(3), u(3), v(3).  y6[slot] receives y_ij.
+template <int PT>
+LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W, int nl, double trel,
+                          const double* bs, double (&y6)[6]) {
+  const double k0 = bs[0], k1 = bs[1], k2 = bs[2];
+  const double u0 = bs[3], u1 = bs[4], u2 = bs[5];
+  const double v0 = bs[6], v1 = bs[7], v2 = bs[8];
+  double x[3][3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int a = 0; a < 3; ++a) x[i][a] = spline_eval(prm, i * 3 + a, trel);
+
+  auto fetch = [&](int m, double (&d)[2]) {
+    const D2 v = dif[m];
+    d[0] = v.x; d[1] = v.y;
+  };
+  const int a_min = PT > 0 ? PT : prm.p, a_max = W - (PT > 0 ? PT : prm.p);
+  auto clampi = [](int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); };
+
+  // reception: h at t - k.x_i/c for the three receivers (each shared by the two links it receives)
+  double Dr[3], Sr[3][2];
+  int ar[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    Dr[i] = (k0 * x[i][0] + k1 * x[i][1] + k2 * x[i][2]) * prm.inv_cdt;
+    double eps;
+    split_delay(Dr[i], nl, ar[i], eps);
+    ar[i] = clampi(ar[i], a_min, a_max);
+    interp_sbp<PT, 2>(prm, eps, ar[i], fetch, Sr[i]);
+  }
+
+  // three arms: arm a joins receiver i = a and emitter j = (a+1)%3 (links 12, 23, 31); the reverse links
+  // 21, 32, 13 share xi+ and xix and flip the sign of k.n
+#pragma unroll
+  for (int arm = 0; arm < 3; ++arm) {
+    const int i = arm, j = (arm + 1) % 3;
+    const double d0 = x[i][0] - x[j][0], d1 = x[i][1] - x[j][1], d2 = x[i][2] - x[j][2];
+    const double inv = 1.0 / sqrt(d0 * d0 + d1 * d1 + d2 * d2);
+    const double n0v = d0 * inv, n1v = d1 * inv, n2v = d2 * inv;  // emitter j -> receiver i
+    const double un = u0 * n0v + u1 * n1v + u2 * n2v;
+    const double vn = v0 * n0v + v1 * n1v + v2 * n2v;
+    const double kn = k0 * n0v + k1 * n1v + k2 * n2v;
+    const double xip = un * un - vn * vn, xic = 2.0 * un * vn;  // eq. 12
+#pragma unroll
+    for (int dir = 0; dir < 2; ++dir) {
+      const int rx = dir == 0 ? i : j, tx = dir == 0 ? j : i;
+      const int slot = link_slot(rx, tx);
+      const double kappa = dir == 0 ? kn : -kn;
+      // emission: t - L_rx,tx(t) - k.x_tx(t)/c
+      const double De = fma(spline_eval(prm, 9 + slot, trel), prm.inv_dt, Dr[tx]);
+      int ae;
+      double eps, Se[2];
+      split_delay(De, nl, ae, eps);
+      ae = clampi(ae, a_min, a_max);
+      interp_sbp<PT, 2>(prm, eps, ae, fetch, Se);
+      const D2 re = raw[ae], rr = raw[ar[rx]];
+      const double dhp = (re.x - rr.x) - Se[0] + Sr[rx][0];
+      const double dhc = (re.y - rr.y) - Se[1] + Sr[rx][1];
+      y6[slot] = (xip * dhp + xic * dhc) / (2.0 * (1.0 - kappa));  // eq. 16
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- stage 2
+// X's two delay chains (eqs. 17-18): term k of chain A is + y_{A[k]} delayed by the
+// first k links of A, term k of chain B is - y_{B[k]} delayed by the first k links of B; k = 0..3 is the
+// first generation, k = 0..7 the second.  Term k^2 of A and term k of B carry the same series.
+// slots: chain A = 13 31 12 21 12 21 13 31, chain B = 12 21 13 31 13 31 12 21
+__host__ __device__ constexpr int chain_a(int k) { return k == 0 ? 3 : k == 1 ? 2 : k == 2 ? 0 : k == 3 ? 5 : k == 4 ? 0 : k == 5 ? 5 : k == 6 ? 3 : 2; }
+__host__ __device__ constexpr int chain_b(int k) { return k == 0 ? 0 : k == 1 ? 5 : k == 2 ? 3 : k == 3 ? 2 : k == 4 ? 3 : k == 5 ? 2 : k == 6 ? 0 : 5; }
+
+// One time sample of eqs. 17-18 for X, Y, Z.  raw/dif: six staged series [6][W] and first differences.
+// MODE 0: nested delays, 1: eq. 20 sums.
+template <int PT, int GEN, int MODE>
+LR_HD void tdi_sample(const Params& prm, const double* raw, const double* dif, int W, int nl, double trel,
+                      double (&xyz)[3]) {
+  constexpr int NK = GEN == 1 ? 4 : 8;
+  const int a_min = PT > 0 ? PT : prm.p, a_max = W - (PT > 0 ? PT : prm.p);
+  auto clampi = [](int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); };
+
+  double Lt[6];
+  if (MODE == 1) {  // eq. 20: every L at t
+#pragma unroll
+    for (int s = 0; s < 6; ++s) Lt[s] = spline_eval(prm, 9 + s, trel);
+  }
+#pragma unroll
+  for (int ch = 0; ch < 3; ++ch) {  // Y, Z: every index of X rotated 1->2->3->1
+    int aA[NK];
+    double acc = 0.0;
+    {
+      double d = 0.0;
+#pragma unroll
+      for (int k = 0; k < NK; ++k) {
+        const int s = rot_slot(chain_a(k), ch);
+        if (k == 0) {
+          aA[k] = nl;
+        } else {
+          double eps, S[1];
+          split_delay(d * prm.inv_dt, nl, aA[k], eps);
+          aA[k] = clampi(aA[k], a_min, a_max);
+          const double* ds = dif + s * W;
+          interp_sbp<PT, 1>(prm, eps, aA[k], [&](int m, double (&o)[1]) { o[0] = ds[m]; }, S);
+          acc -= S[0];
+        }
+        if (k + 1 < NK) d += MODE == 1 ? Lt[s] : spline_eval(prm, 9 + s, trel - d);
+      }
+    }
+    {
+      double d = 0.0;
+#pragma unroll
+      for (int k = 0; k < NK; ++k) {
+        const int s = rot_slot(chain_b(k), ch);
+        int aB = nl;
+        if (k > 0) {
+          double eps, S[1];
+          split_delay(d * prm.inv_dt, nl, aB, eps);
+          aB = clampi(aB, a_min, a_max);
+          const double* ds = dif + s * W;
+          interp_sbp<PT, 1>(prm, eps, aB, [&](int m, double (&o)[1]) { o[0] = ds[m]; }, S);
+          acc += S[0];
+        }
+        // same series: + y_s at the anchor of A's term k^2, - y_s at this term's anchor
+        acc += raw[s * W + aA[k ^ 2]] - raw[s * W + aB];
+        if (k + 1 < NK) d += MODE == 1 ? Lt[s] : spline_eval(prm, 9 + s, trel - d);
+      }
+    }
+    xyz[ch] = acc;
+  }
+}
+
+// Source basis (eq. 10) with the polarisation angle applied to (u, v) (reading A4):
+// out[0..2] = k, out[3..5] = u, out[6..8] = v.  Host-side helper of lr_project.
+inline void source_basis(double beta, double lam, double psi, double* out) {
+  const double cb = cos(beta), sb = sin(beta), cl = cos(lam), sl = sin(lam);
+  const double k[3] = {-cb * cl, -cb * sl, -sb};
+  const double u0[3] = {sl, -cl, 0.0};                 // -e_phi
+  const double v0[3] = {-sb * cl, -sb * sl, cb};       // -e_theta
+  const double cp = cos(psi), sp = sin(psi);
+  for (int a = 0; a < 3; ++a) {
+    out[a] = k[a];
+    out[3 + a] = u0[a] * cp + v0[a] * sp;
+    out[6 + a] = -u0[a] * sp + v0[a] * cp;
+  }
+}
+
+}  // namespace lr

@@ -1,0 +1,128 @@
+// lr_kernels.cuh — the two CUDA kernels of liblr (sm_100a) and their launchers' declarations.
+//
+//   project_kernel<PT>       : PAPER.md eqs. 10-16, one thread per time sample, all six links
+//   tdi_kernel<PT,GEN,MODE>  : PAPER.md eqs. 17-21, one thread per time sample, X, Y, Z (+ A, E, T)
+//
+// Both stage the window a tile of samples needs (raw samples and their exact first differences) in
+// shared memory with coalesced loads, keep the Lagrange pair products in registers, and write coalesced
+// fp64 along the time axis.  The path is bound by the FP64 pipe, so there is no tensor-core
+// or TMA use: the staged windows are small (tens of KB) and each is read ~T times from shared memory.
+#pragma once
+#include "lr_device.cuh"
+
+namespace lr {
+
+constexpr int kProjThreads = 256;
+constexpr int kTdiThreads = 256;
+
+// ---------------------------------------------------------------------------------------------- stage 1
+// grid.x = ntiles * batch; tile = blockIdx.x % ntiles, template = blockIdx.x / ntiles.
+// dynamic smem: D2 raw[W], D2 dif[W] with W = kProjThreads + halo_lo + halo_hi  (x = h+, y = hx)
+template <int PT>
+__global__ void __launch_bounds__(kProjThreads)
+project_kernel(const Params prm, const double* __restrict__ hp, const double* __restrict__ hc,
+               const double* __restrict__ basis /* [batch][9] */, double* __restrict__ y) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int W = kProjThreads + prm.halo_lo + prm.halo_hi;
+  D2* raw = reinterpret_cast<D2*>(smem_raw);
+  D2* dif = raw + W;
+
+  const int tile = blockIdx.x % prm.ntiles;
+  const int64_t b = blockIdx.x / prm.ntiles;
+  const int n0 = tile * kProjThreads;
+  const int g0 = n0 - prm.halo_lo;  // global sample index of staged index 0
+  const double* hpb = hp + b * (int64_t)prm.n;
+  const double* hcb = hc + b * (int64_t)prm.n;
+
+  for (int m = threadIdx.x; m < W; m += kProjThreads) {
+    const int g = g0 + m;
+    D2 v{0.0, 0.0};
+    if (g >= 0 && g < prm.n) { v.x = __ldg(hpb + g); v.y = __ldg(hcb + g); }
+    raw[m] = v;
+  }
+  __syncthreads();
+  for (int m = threadIdx.x; m < W - 1; m += kProjThreads) {
+    dif[m] = D2{raw[m + 1].x - raw[m].x, raw[m + 1].y - raw[m].y};
+  }
+  __syncthreads();
+
+  const int n = n0 + (int)threadIdx.x;
+  if (n >= prm.n) return;
+  double* yb = y + b * 6 * (int64_t)prm.n + n;
+  if (n < prm.m_proj || n >= prm.n - prm.m_proj) {
+#pragma unroll
+    for (int s = 0; s < 6; ++s) yb[(int64_t)s * prm.n] = 0.0;
+    return;
+  }
+
+  double bs[9];
+#pragma unroll
+  for (int a = 0; a < 9; ++a) bs[a] = __ldg(basis + b * 9 + a);
+  double y6[6];
+  project_sample<PT>(prm, raw, dif, W, n - g0, sample_trel(prm, n), bs, y6);
+#pragma unroll
+  for (int s = 0; s < 6; ++s) yb[(int64_t)s * prm.n] = y6[s];
+}
+
+// ---------------------------------------------------------------------------------------------- stage 2
+// dynamic smem: double raw[6][W], dif[6][W], W = kTdiThreads + halo_lo + halo_hi
+// CH: LR_XYZ 0 | LR_AET 1 | LR_XYZ_AET 2 ; MODE: 0 nested, 1 sum
+template <int PT, int GEN, int MODE>
+__global__ void __launch_bounds__(kTdiThreads)
+tdi_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ out, int channels) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int W = kTdiThreads + prm.halo_lo + prm.halo_hi;
+  double* raw = reinterpret_cast<double*>(smem_raw);
+  double* dif = raw + 6 * W;
+
+  const int tile = blockIdx.x % prm.ntiles;
+  const int64_t b = blockIdx.x / prm.ntiles;
+  const int n0 = tile * kTdiThreads;
+  const int g0 = n0 - prm.halo_lo;
+  const double* yb = y + b * 6 * (int64_t)prm.n;
+
+  for (int m = threadIdx.x; m < 6 * W; m += kTdiThreads) {
+    const int s = m / W, g = g0 + (m - s * W);
+    raw[m] = (g >= 0 && g < prm.n) ? __ldg(yb + (int64_t)s * prm.n + g) : 0.0;
+  }
+  __syncthreads();
+  for (int m = threadIdx.x; m < 6 * W; m += kTdiThreads) {
+    const int w = m % W;
+    dif[m] = (w < W - 1) ? raw[m + 1] - raw[m] : 0.0;
+  }
+  __syncthreads();
+
+  const int n = n0 + (int)threadIdx.x;
+  if (n >= prm.n) return;
+  const int nout = channels == 2 ? 6 : 3;
+  double* ob = out + b * nout * (int64_t)prm.n + n;
+  if (n < prm.m_front || n >= prm.n - prm.m_back) {
+    for (int c = 0; c < nout; ++c) ob[(int64_t)c * prm.n] = 0.0;
+    return;
+  }
+
+  double xyz[3];
+  tdi_sample<PT, GEN, MODE>(prm, raw, dif, W, n - g0, sample_trel(prm, n), xyz);
+
+  const int64_t N = prm.n;
+  if (channels != 1) { ob[0] = xyz[0]; ob[N] = xyz[1]; ob[2 * N] = xyz[2]; }
+  if (channels != 0) {  // eq. 21
+    const double A = (xyz[2] - xyz[0]) * 0.70710678118654752440;
+    const double E = (xyz[0] - 2.0 * xyz[1] + xyz[2]) * 0.40824829046386301637;
+    const double T = (xyz[0] + xyz[1] + xyz[2]) * 0.57735026918962576451;
+    double* oa = channels == 2 ? ob + 3 * N : ob;
+    oa[0] = A; oa[N] = E; oa[2 * N] = T;
+  }
+}
+
+// small helper kernel: spline channel at arbitrary absolute times (lr_eval_orbit)
+__global__ void eval_orbit_kernel(const Params prm, int ch, double t_start, const double* __restrict__ t,
+                                  int64_t m, double* __restrict__ out);
+
+// launchers (lr_kernels_*.cu); return cudaError_t as int
+int launch_project(const Params& prm, int order, const double* hp, const double* hc, const double* basis,
+                   double* y, int64_t batch, void* stream);
+int launch_tdi(const Params& prm, int order, int gen, int mode, int channels, const double* y, double* out,
+               int64_t batch, void* stream);
+
+}  // namespace lr

@@ -1,0 +1,79 @@
+"""Convenience wrapper around the lr_* calls (allocation of outputs, option handling, batch sharding).
+
+No arithmetic of the method lives here.
+"""
+from __future__ import annotations
+
+from . import binding as B
+
+_CHANNELS = {"XYZ": B.LR_XYZ, "AET": B.LR_AET, "XYZ_AET": B.LR_XYZ_AET}
+
+
+def shard_templates(batch, rank, world):
+    """Contiguous slice [lo, hi) of `batch` templates owned by `rank` of `world` (no collective is needed:
+    templates are independent).  The first batch % world ranks get one template more."""
+    if world < 1 or not 0 <= rank < world or batch < 0:
+        raise ValueError("bad shard arguments")
+    base, extra = divmod(batch, world)
+    lo = rank * base + min(rank, extra)
+    return lo, lo + base + (1 if rank < extra else 0)
+
+
+class Response:
+    """One orbit table + (dt, order, TDI generation): owns an lr_handle."""
+
+    def __init__(self, table, dt, order=25, tdi_gen=2, t0=None, chain="nested", channels="XYZ"):
+        self._h = None
+        self._h = B.lr_create(table, dt, order, tdi_gen)
+        self.dt, self.order, self.tdi_gen = dt, order, tdi_gen
+        if t0 is not None:
+            B.lr_set_option(self._h, B.LR_OPT_T0, t0)
+        self.set_chain(chain)
+        self.set_channels(channels)
+
+    @property
+    def handle(self):
+        return self._h
+
+    def set_chain(self, chain):
+        B.lr_set_option(self._h, B.LR_OPT_CHAIN, {"nested": B.LR_CHAIN_NESTED, "sum": B.LR_CHAIN_SUM}[chain])
+
+    def set_channels(self, channels):
+        B.lr_set_option(self._h, B.LR_OPT_CHANNELS, _CHANNELS[channels])
+        self.n_out = 6 if channels == "XYZ_AET" else 3
+
+    def set_tdi_gen(self, gen):
+        B.lr_set_option(self._h, B.LR_OPT_TDI_GEN, gen)
+        self.tdi_gen = gen
+
+    def margins(self):
+        return B.lr_get_margins(self._h)
+
+    def project(self, h_plus, h_cross, beta, lam, psi, y_out=None, stream=None):
+        import torch
+        h_plus = h_plus.reshape(-1, h_plus.shape[-1])
+        b, n = h_plus.shape
+        if y_out is None:
+            y_out = torch.empty((b, 6, n), dtype=torch.float64, device=h_plus.device)
+        return B.lr_project(self._h, h_plus, h_cross, beta, lam, psi, y_out, stream)
+
+    def tdi(self, y, out=None, stream=None):
+        import torch
+        b, _, n = y.shape
+        if out is None:
+            out = torch.empty((b, self.n_out, n), dtype=torch.float64, device=y.device)
+        return B.lr_tdi(self._h, y, out, b, stream)
+
+    def response_host(self, h_plus, h_cross, beta, lam, psi, out, tdi=None, stream=None):
+        return B.lr_response_host(self._h, (tdi or self)._h, h_plus, h_cross, beta, lam, psi, out, stream)
+
+    def close(self):
+        if self._h is not None:
+            B.lr_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,149 @@
+"""CPU-side checks (no GPU): the C-ABI library builds, loads and exports every symbol include/lr.h
+declares; host-only entry points behave; the batch sharding used for N > 1 GPUs is a partition."""
+import ctypes
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2204_06633_b200 import binding, build
+    build.build()
+    return binding.lib()
+
+
+def _declared_symbols():
+    src = open(os.path.join(ROOT, "include", "lr.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(lr_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_header_symbols_exported(lib):
+    from paper_2204_06633_b200 import binding
+    decl = _declared_symbols()
+    assert sorted(binding.SYMBOLS) == decl
+    for name in decl:
+        assert hasattr(lib, name), f"liblr.so does not export {name}"
+
+
+def test_header_compiles_as_c():
+    """include/lr.h is plain C: no torch or C++ types in the signatures."""
+    code = '#include "lr.h"\nint main(void){ lr_orbits o; (void)o; return LR_MAX_ORDER == 65 ? 0 : 1; }\n'
+    r = subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-fsyntax-only", "-I", os.path.join(ROOT, "include"),
+                        "-x", "c", "-"], input=code, text=True, capture_output=True)
+    assert r.returncode == 0, r.stderr
+
+
+def test_host_only_entry_points(lib):
+    from paper_2204_06633_b200 import binding
+    assert binding.lr_strerror(0) == "success"
+    for code in (-1, -2, -3, -4, -99):
+        assert binding.lr_strerror(code)
+    assert binding.lr_launch_count() >= 0
+    # argument validation happens before any CUDA call
+    h = ctypes.c_void_p()
+    assert lib.lr_create(None, 10.0, 25, 2, ctypes.byref(h)) == binding.LR_EINVAL
+    assert lib.lr_set_option(None, 1, 0.0) == binding.LR_EINVAL
+    assert lib.lr_get_margins(None, None, None, None) == binding.LR_EINVAL
+    assert lib.lr_project(None, None, None, None, None, None, 1, 1, None, None) == binding.LR_EINVAL
+    assert lib.lr_tdi(None, None, 1, 1, None, None) == binding.LR_EINVAL
+    lib.lr_destroy(None)
+
+
+def test_create_rejects_bad_arguments_without_gpu(lib):
+    from paper_2204_06633_b200 import binding, inputs
+    tab = inputs.orbit_table("eq", 0.0, 86400.0)
+    for order, gen, dt in ((24, 2, 10.0), (0, 2, 10.0), (67, 2, 10.0), (25, 3, 10.0), (25, 2, 0.0)):
+        with pytest.raises(binding.LrError) as e:
+            binding.lr_create(tab, dt, order, gen)
+        assert e.value.code == binding.LR_EINVAL
+    bad = inputs.OrbitTable(tab.t_start, tab.knot_dt, tab.x.copy(), tab.ltt.copy())
+    bad.x[0, 0, 1] = np.nan
+    with pytest.raises(binding.LrError):
+        binding.lr_create(bad, 10.0, 25, 2)
+
+
+def test_no_cpu_fallback_without_device(lib):
+    """Without a CUDA device a valid lr_create fails with LR_ECUDA: there is no CPU compute path."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    from paper_2204_06633_b200 import binding, inputs
+    tab = inputs.orbit_table("eq", 0.0, 86400.0)
+    with pytest.raises(binding.LrError) as e:
+        binding.lr_create(tab, 10.0, 25, 2)
+    assert e.value.code == binding.LR_ECUDA
+
+
+def test_product_never_imports_oracle():
+    """The product path shares nothing with oracle/ (and does not read _work/)."""
+    pkg = os.path.join(ROOT, "paper_2204_06633_b200")
+    for dirpath, _, files in os.walk(pkg):
+        if os.path.basename(dirpath) == "build":
+            continue
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".hpp", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle", text, flags=re.M), f
+                assert "lr_oracle" not in text and "_work/" not in text, f
+    text = open(os.path.join(ROOT, "oracle", "lr_oracle.cpp")).read()
+    assert "paper_2204_06633_b200/csrc/" not in re.sub(r"//.*", "", text)
+
+
+def test_shard_templates_is_a_partition():
+    from paper_2204_06633_b200 import shard_templates
+    for batch in (0, 1, 7, 128, 1024, 1025):
+        for world in (1, 2, 3, 8):
+            spans = [shard_templates(batch, r, world) for r in range(world)]
+            assert spans[0][0] == 0 and spans[-1][1] == batch
+            for a, b in zip(spans, spans[1:]):
+                assert a[1] == b[0]
+            sizes = [hi - lo for lo, hi in spans]
+            assert max(sizes) - min(sizes) <= 1
+    with pytest.raises(ValueError):
+        shard_templates(4, 2, 2)
+
+
+_GLOO_WORKER = r'''
+import os, sys
+sys.path.insert(0, sys.argv[1])
+import torch, torch.distributed as dist
+from paper_2204_06633_b200 import shard_templates
+import bench
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+batch = 11
+lo, hi = shard_templates(batch, rank, world)
+# every rank claims its templates; the union must be a partition (no data-path collective is involved)
+own = torch.zeros(batch, dtype=torch.int64); own[lo:hi] = 1
+dist.all_reduce(own)
+assert bool((own == 1).all()), own
+# max-over-ranks timing + whole-job aggregation used by bench.py
+ms = bench.max_over_ranks(10.0 * (rank + 1))
+assert ms == 10.0 * world, ms
+tot = bench.sum_over_ranks(float(hi - lo))
+assert tot == batch, tot
+dist.barrier()
+dist.destroy_process_group()
+print("ok", rank)
+'''
+
+
+def test_multi_rank_host_logic_gloo(tmp_path):
+    """world_size-2 run of the N > 1 host logic on CPU (gloo): template sharding partitions the batch,
+    timing is the max over ranks, units are summed over ranks."""
+    script = tmp_path / "worker.py"
+    script.write_text(_GLOO_WORKER)
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1")
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
+                        "--master-addr", "127.0.0.1", "--master-port", "29517", str(script), ROOT],
+                       capture_output=True, text=True, timeout=300, env=env)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert r.stdout.count("ok") == 2

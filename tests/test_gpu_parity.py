@@ -1,0 +1,305 @@
+"""GPU parity: liblr (CUDA, through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Run on the B200 box with `pytest -m gpu`.
+
+Per-call parity: lr_project against the oracle's projection of the same h;
+lr_tdi against the oracle's TDI of the *same fp64 y* (the GPU's own).  Bar: parity_util.REL_L2_TOL /
+MAX_ABS_TOL = 1e-10 (north_star).  Reduced sizes still span several 256-sample tiles and end in a ragged
+tail; the full BASELINE.json sizes are checked on sampled windows in the launch configuration bench.py
+times (test_full_size_*).
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_2204_06633_b200 import inputs
+from parity_util import (CH_NAMES, LINK_NAMES, ORC_CH, assert_parity, to_dev, windows)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lr():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    import paper_2204_06633_b200 as pkg
+    pkg.binding.lib()  # fail loudly if liblr.so is missing
+    return pkg
+
+
+def _stack(w, idx):
+    hp, hc = zip(*(w.waveform(b) for b in idx))
+    return np.stack(hp), np.stack(hc)
+
+
+def check_workload(lr, w, *, chain="nested", channels=None, gen=None, idx=(0,), wins=None, tab=None,
+                   tdi_tab=None, tdi_gen=None, proj=True):
+    """Run w's templates `idx` through lr_project and lr_tdi and compare with the oracle.
+    wins: list of (lo, hi) sample windows to compare on (None = the whole valid region)."""
+    import torch
+    channels = channels or w.channels
+    gen = gen or w.tdi_gen
+    tab = tab or w.table()
+    n = w.n
+    R = lr.Response(tab, w.dt, w.order, gen, t0=w.t0, chain=chain, channels=channels)
+    O = orc.Oracle(tab, w.dt, w.t0, w.order)
+    mp, mf, mb = R.margins()
+    assert (mp, mf, mb) == O.margins(gen)
+    hp, hc = _stack(w, idx)
+    src = [w.sources[b] for b in idx]
+    beta, lam, psi = ([getattr(s, k) for s in src] for k in ("beta", "lam", "psi"))
+    y = R.project(to_dev(hp), to_dev(hc), beta, lam, psi)
+    torch.cuda.synchronize()
+    yh = y.cpu().numpy()
+    assert np.all(yh[:, :, :mp] == 0) and np.all(yh[:, :, n - mp:] == 0)
+    errs = {}
+    if proj:
+        for k, b in enumerate(idx):
+            for lo, hi in (wins or [(mp, n - mp)]):
+                lo, hi = max(lo, mp), min(hi, n - mp)
+                yo = O.project(hp[k], hc[k], beta[k], lam[k], psi[k], lo=lo, hi=hi)
+                errs[("proj", b, lo)] = assert_parity(yh[k][:, lo:hi], yo[:, lo:hi], f"{w.name} project b={b} [{lo},{hi})",
+                                                      LINK_NAMES)
+    # stage 2 on the GPU's own fp64 y; optionally with another handle (hybrid)
+    Rt, Ot, g2 = R, O, gen
+    if tdi_tab is not None:
+        g2 = tdi_gen or gen
+        Rt = lr.Response(tdi_tab, w.dt, w.order, g2, t0=w.t0, chain=chain, channels=channels)
+        Ot = orc.Oracle(tdi_tab, w.dt, w.t0, w.order)
+    out = Rt.tdi(y)
+    torch.cuda.synchronize()
+    oh = out.cpu().numpy()
+    _, mf, mb = Rt.margins()
+    assert np.all(oh[:, :, :mf] == 0) and np.all(oh[:, :, n - mb:] == 0)
+    for k, b in enumerate(idx):
+        for lo, hi in (wins or [(mf, n - mb)]):
+            lo, hi = max(lo, mf), min(hi, n - mb)
+            oo = Ot.tdi(yh[k], g2, nested=(chain == "nested"), channels=ORC_CH[channels], lo=lo, hi=hi)
+            errs[("tdi", b, lo)] = assert_parity(oh[k][:, lo:hi], oo[:, lo:hi],
+                                                 f"{w.name} tdi gen{g2} {chain} b={b} [{lo},{hi})", CH_NAMES[channels])
+    return errs, yh, oh
+
+
+# ------------------------------------------------------------------------------------------- config 1
+def test_config1_tiny_full(lr):
+    """BASELINE.json configs[0] at its full size: EQ orbits, constant equal light times, TDI-1 XYZ."""
+    check_workload(lr, inputs.config(1))
+
+
+def test_config1_tiny_fixed_point_ltt(lr):
+    """Same with the flat-space fixed-point light times (L_ij != L_ji), nested and eq. 20 sums, gen 1 and 2."""
+    w = inputs.config(1)
+    tab = inputs.orbit_table("eq", w.t0, w.t0 + w.n * w.dt)
+    for chain in ("nested", "sum"):
+        for gen in (1, 2):
+            check_workload(lr, w, tab=tab, chain=chain, gen=gen, channels="XYZ_AET")
+
+
+# ------------------------------------------------------------------------------------------- config 2
+@pytest.mark.parametrize("f0", [None, 1e-4, 1e-3, 1e-2])
+@pytest.mark.parametrize("chain", ["nested", "sum"])
+def test_config2_year_reduced(lr, f0, chain):
+    """configs[1] shortened to 20,011 samples (79 tiles, ragged tail): Keplerian, TDI-2, XYZ+AET; the seeded
+    source and the three fixed-frequency strata of SURVEY.md §8(c)."""
+    check_workload(lr, inputs.config(2, n=20011, f0=f0, t0=3.0e7), chain=chain)
+
+
+def test_config2_paper_sources(lr):
+    """The paper's own three (f, fdot) points with its angles as seed-free sources."""
+    w = inputs.config(2, n=6007, t0=1.0e7)
+    for f, fd in ((6e-4, 1.5e-18), (2e-3, 1.2e-17), (6e-3, 1.3e-16)):
+        w.sources = [inputs.Source(A=1e-22, f0=f, fdot=fd, iota=1.11, phi0=4.58, psi=0.45, lam=5.23, beta=0.09)]
+        check_workload(lr, w)
+
+
+# ------------------------------------------------------------------------------------------- config 3
+def test_config3_batch_reduced(lr):
+    """configs[2] with 7 templates of 9,001 samples in ONE launch: batch indexing, AET output."""
+    w = inputs.config(3, batch=7, n=9001)
+    check_workload(lr, w, idx=tuple(range(7)))
+
+
+# ------------------------------------------------------------------------------------------- config 4
+def test_config4_numerical_orbits_reduced(lr):
+    """configs[3] shortened: perturbed-orbit tables (L_ij != L_ji), dt = 5 s, order 41, TDI-2 XYZ."""
+    check_workload(lr, inputs.config(4, n=12345, t0=5.0e7))
+    check_workload(lr, inputs.config(4, n=5000, t0=1.0e8, f0=1e-4), chain="sum")
+
+
+# ------------------------------------------------------------------------------------------- config 5
+def test_config5_chirp_reduced(lr):
+    """configs[4] shortened (the last 30,001 samples of the chirp, where f sweeps fastest): full TDI-2 and
+    the hybrid mode (projection on Keplerian orbits, TDI-1 on equal-arm constant delays)."""
+    full = inputs.config(5)
+    n = 30001
+    w = inputs.config(5, n=n, t0=full.t0 + (full.n - n) * full.dt)
+    hp, hc = full.waveform(0)
+    w.waveform = lambda b=0: (hp[-n:].copy(), hc[-n:].copy())
+    check_workload(lr, w)
+    eq = inputs.orbit_table("eq", w.t0, w.t0 + n * w.dt, const_ltt=inputs.ARM / inputs.C_LIGHT)
+    check_workload(lr, w, tdi_tab=eq, tdi_gen=1, proj=False)
+
+
+# --------------------------------------------------------------------------------------------- orders
+@pytest.mark.parametrize("order", [1, 3, 5, 9, 13, 31, 65])
+def test_orders(lr, order):
+    """Compile-time-P kernels (1, 3, 9) and the run-time-P path (5, 13, 31, 65)."""
+    w = inputs.config(2, n=3001, f0=2e-3, t0=2.0e7)
+    w.order = order
+    check_workload(lr, w, channels="XYZ")
+
+
+# ---------------------------------------------------------------------------------------------- pins
+def test_gpu_laser_noise_suppression(lr):
+    """Pin P3 run on the GPU TDI: three independent band-limited laser-noise series, y_ij = p_j(t - L_ij(t))
+    - p_i(t) evaluated analytically; second-generation NESTED TDI must cancel them to interpolation level,
+    eq. 20 sums and first generation must not."""
+    import torch
+    dt, n, t0, order = 10.0, 6000, 3.0e7, 25
+    tab = inputs.orbit_table("kepler", t0, t0 + n * dt)
+    O = orc.Oracle(tab, dt, t0, order)
+    par = inputs.band_limited_noise(7)
+    t = (np.longdouble(t0) + np.longdouble(dt) * np.arange(n)).astype(np.longdouble)
+    y = np.zeros((6, n))
+    for s, (i, j) in enumerate(inputs.LINKS):
+        L = O.spline(9 + s, t)
+        y[s] = (inputs.eval_tones(par, j - 1, t - L) - inputs.eval_tones(par, i - 1, t)).astype(np.float64)
+    rms_p = float(np.sqrt(np.mean(inputs.eval_tones(par, 0, t).astype(np.float64) ** 2)))
+    res = {}
+    for gen in (1, 2):
+        for chain in ("nested", "sum"):
+            R = lr.Response(tab, dt, order, gen, t0=t0, chain=chain)
+            _, mf, mb = R.margins()
+            out = R.tdi(to_dev(y)[None]).cpu().numpy()[0]
+            torch.cuda.synchronize()
+            res[(gen, chain)] = float(np.sqrt(np.mean(out[0, mf:n - mb] ** 2))) / rms_p
+    # fp64 y limits the residual to ~1e-16/rms; the survey's long-double value is 7.4e-14
+    assert res[(2, "nested")] < 1e-12, res
+    for key in ((2, "sum"), (1, "nested"), (1, "sum")):
+        assert res[key] > 1e-10, res
+
+
+def test_gpu_relabelling(lr):
+    """Pin P4 on the GPU: cyclic relabelling of the spacecraft permutes (X,Y,Z) -> (Z,X,Y) of the relabelled
+    run back onto (X,Y,Z); the reflection 2<->3 flips the sign of X."""
+    w = inputs.config(2, n=4001, f0=3e-3, t0=2.5e7)
+    tab = w.table()
+    s = w.sources[0]
+    hp, hc = w.waveform(0)
+
+    def run(table):
+        R = lr.Response(table, w.dt, w.order, 2, t0=w.t0)
+        y = R.project(to_dev(hp)[None], to_dev(hc)[None], [s.beta], [s.lam], [s.psi])
+        return R.tdi(y).cpu().numpy()[0], R.margins()
+
+    base, (mp, mf, mb) = run(tab)
+    cyc, _ = run(tab.relabel({1: 2, 2: 3, 3: 1}))   # new spacecraft 1 is old 2: new X = old Y
+    ref, _ = run(tab.relabel({1: 1, 2: 3, 3: 2}))
+    v = slice(mf, w.n - mb)
+    scale = np.abs(base[:, v]).max()
+    assert np.abs(cyc[0, v] - base[1, v]).max() < 1e-13 * scale
+    assert np.abs(cyc[1, v] - base[2, v]).max() < 1e-13 * scale
+    assert np.abs(cyc[2, v] - base[0, v]).max() < 1e-13 * scale
+    assert np.abs(ref[0, v] + base[0, v]).max() < 1e-13 * scale
+    assert np.abs(ref[1, v] + base[2, v]).max() < 1e-13 * scale
+
+
+def test_gpu_hybrid_same_handle_bitwise(lr):
+    """Pin P11: lr_tdi through a second handle built from the same table equals the same-handle run bit for
+    bit; lr_response_host equals lr_project + lr_tdi bit for bit."""
+    import torch
+    w = inputs.config(2, n=5003, t0=1.5e7)
+    tab = w.table()
+    s = w.sources[0]
+    hp, hc = w.waveform(0)
+    R1 = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="XYZ_AET")
+    R2 = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="XYZ_AET")
+    y = R1.project(to_dev(hp)[None], to_dev(hc)[None], [s.beta], [s.lam], [s.psi])
+    a, b = R1.tdi(y).cpu().numpy(), R2.tdi(y).cpu().numpy()
+    assert np.array_equal(a, b)
+    out = np.empty((1, 6, w.n))
+    R1.response_host(hp[None].copy(), hc[None].copy(), [s.beta], [s.lam], [s.psi], out)
+    torch.cuda.synchronize()
+    assert np.array_equal(out, a)
+
+
+def test_gpu_orbit_spline_matches_oracle(lr):
+    """Orbit ingestion (lr_create's device spline) against the oracle's spline and scipy's not-a-knot
+    CubicSpline at random times: positions to 1e-15 relative, light times to 1e-15 s."""
+    import torch
+    from scipy.interpolate import CubicSpline
+    w = inputs.config(4, n=1000)
+    tab = w.table()
+    R = lr.Response(tab, w.dt, w.order, 2, t0=w.t0)
+    O = orc.Oracle(tab, w.dt, w.t0, w.order)
+    rng = np.random.default_rng(3)
+    t_end = tab.t_start + (tab.n_knots - 1) * tab.knot_dt
+    t = np.sort(rng.uniform(tab.t_start, t_end, size=5000))
+    tk = tab.t_start + tab.knot_dt * np.arange(tab.n_knots)
+    td = to_dev(t)
+    for ch in range(15):
+        out = torch.empty_like(td)
+        lr.lr_eval_orbit(R.handle, ch, td, out)
+        g = out.cpu().numpy()
+        o = O.spline(ch, t.astype(np.longdouble))
+        table = tab.x.reshape(9, -1)[ch] if ch < 9 else tab.ltt[ch - 9]
+        sp = CubicSpline(tk, table, bc_type="not-a-knot")(t)
+        scale = np.abs(table).max()
+        assert np.abs(g - o.astype(np.float64)).max() < 4e-15 * scale, ch
+        assert np.abs(g - sp).max() < 1e-13 * scale, ch
+
+
+# ---------------------------------------------------------------------------------------- edge cases
+def test_edge_cases_and_errors(lr):
+    import torch
+    B = lr.binding
+    w = inputs.config(1)
+    tab = w.table()
+    for bad_order in (0, 2, 26, 67):
+        with pytest.raises(lr.LrError) as e:
+            lr.lr_create(tab, w.dt, bad_order, 1)
+        assert e.value.code == lr.LR_EINVAL
+    with pytest.raises(lr.LrError):
+        lr.lr_create(tab, w.dt, 25, 3)
+    with pytest.raises(lr.LrError):
+        lr.lr_create(tab, -1.0, 25, 1)
+    R = lr.Response(tab, w.dt, w.order, 1, t0=w.t0)
+    mp, mf, mb = R.margins()
+    s = w.sources[0]
+    # n <= 2 m_proj: nothing valid -> LR_EINVAL ("empty" input)
+    n = 2 * mp
+    h = torch.zeros((1, n), dtype=torch.float64, device="cuda")
+    with pytest.raises(lr.LrError) as e:
+        R.project(h, h, [s.beta], [s.lam], [s.psi])
+    assert e.value.code == lr.LR_EINVAL
+    # smallest legal sizes: one valid sample per stage
+    n = 2 * mp + 1
+    hp, hc = inputs.gb_waveform(n, w.dt, w.t0, s.A, s.f0, s.fdot, s.iota, s.phi0)
+    y = R.project(to_dev(hp)[None], to_dev(hc)[None], [s.beta], [s.lam], [s.psi]).cpu().numpy()[0]
+    O = orc.Oracle(tab, w.dt, w.t0, w.order)
+    yo = O.project(hp, hc, s.beta, s.lam, s.psi)
+    assert np.count_nonzero(y) == 6
+    assert_parity(y[:, mp:mp + 1], yo[:, mp:mp + 1], "single valid sample")
+    n = mf + mb + 1
+    yy = np.random.default_rng(0).normal(size=(6, n)) * 1e-22
+    out = R.tdi(to_dev(yy)[None]).cpu().numpy()[0]
+    oo = O.tdi(yy, 1)
+    assert np.count_nonzero(out) == 3
+    # (white-noise y: the interpolation is the same linear map on both sides)
+    assert_parity(out[:, mf:mf + 1], oo[:, mf:mf + 1], "single valid tdi sample", rel_tol=1e-9, abs_tol=1e-9)
+    with pytest.raises(lr.LrError) as e:
+        R.tdi(to_dev(yy[:, :-1])[None])
+    assert e.value.code == lr.LR_EINVAL
+    # sample span outside the knot table -> LR_ERANGE, no extrapolation
+    R2 = lr.Response(tab, w.dt, w.order, 1, t0=w.t0 + 40 * 86400.0)
+    hp, hc = w.waveform(0)
+    with pytest.raises(lr.LrError) as e:
+        R2.project(to_dev(hp)[None], to_dev(hc)[None], [s.beta], [s.lam], [s.psi])
+    assert e.value.code == lr.LR_ERANGE
+    assert "orbit table" in B.lr_strerror(lr.LR_ERANGE)
+    # NaN propagates, does not crash
+    hp2 = hp.copy()
+    hp2[5000] = np.nan
+    R3 = lr.Response(tab, w.dt, w.order, 1, t0=w.t0)
+    y = R3.project(to_dev(hp2)[None], to_dev(hc)[None], [s.beta], [s.lam], [s.psi]).cpu().numpy()[0]
+    assert np.isnan(y).any() and np.isfinite(y[:, mp:4000]).all()
