@@ -106,7 +106,7 @@ class ClockSampler:
                 self.reasons.update(k for k, bit in names.items() if r & bit)
             except Exception:
                 pass
-            self._stop.wait(0.02)
+            self._stop.wait(0.005)
 
     def __enter__(self):
         if self._nv:
@@ -168,7 +168,7 @@ def time_oracle(w, target_s=12.0):
     mp, mf, mb = O.margins(w.tdi_gen)
     ch = {"XYZ": 0, "AET": 1, "XYZ_AET": 2}[w.channels]
     cores = os.cpu_count() or 1
-    mid = w.n // 2
+    mid = max(mf, w.n // 8)
 
     def run(m):
         lo, hi = mid, min(mid + m, w.n - mb)
@@ -181,7 +181,7 @@ def time_oracle(w, target_s=12.0):
     m = int(max(2000, min(w.n - mb - mid, m_probe * target_s / max(t_probe, 1e-6))))
     t, m = run(m)
     return m / t, {"cores": cores, "kind": "oracle",
-                   "sample": f"{m} consecutive samples from the middle of template 0 (projection + TDI-{w.tdi_gen}, "
+                   "sample": f"{m} consecutive samples starting at n/8 of template 0 (projection + TDI-{w.tdi_gen}, "
                              f"fp64 build of the oracle, OpenMP over samples), {t:.1f} s wall"}
 
 
@@ -364,7 +364,7 @@ def run_gpu(args, rank, world, local_rank):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="year", choices=["year", "batch", "tiny"])
