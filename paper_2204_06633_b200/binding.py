@@ -13,7 +13,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "liblr.so")
+LIB_PATH = os.environ.get("LR_LIBRARY", os.path.join(_HERE, "liblr.so"))  # override: A/B builds
 
 LR_OK, LR_EINVAL, LR_ERANGE, LR_ECUDA, LR_ENOMEM = 0, -1, -2, -3, -4
 LR_OPT_T0, LR_OPT_CHAIN, LR_OPT_CHANNELS, LR_OPT_TDI_GEN = 1, 2, 3, 4

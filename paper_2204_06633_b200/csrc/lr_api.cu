@@ -90,7 +90,7 @@ lr::Params make_params(const lr_handle* h, int64_t n) {
 
 bool size_ok(int64_t batch, int64_t n) {
   return batch >= 1 && n >= 1 && n < ((int64_t)1 << 31) - ((int64_t)1 << 20) &&
-         batch <= (((int64_t)1 << 31) - 1) / ((n + 255) / 256);
+         batch <= (((int64_t)1 << 31) - 1) / ((n + 63) / 64);
 }
 
 // the times the kernels evaluate the splines at must lie inside the knot table (no extrapolation)

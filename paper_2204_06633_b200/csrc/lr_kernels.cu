@@ -42,11 +42,13 @@ int launch_project(const Params& prm, int order, const double* hp, const double*
                    double* y, int64_t batch, void* stream) {
   cudaStream_t st = (cudaStream_t)stream;
   switch (order) {
+#ifndef LR_DEV_ONLY_P13
     case 1: return launch_project_t<1>(prm, hp, hc, basis, y, batch, st);
     case 3: return launch_project_t<2>(prm, hp, hc, basis, y, batch, st);
     case 9: return launch_project_t<5>(prm, hp, hc, basis, y, batch, st);
-    case 25: return launch_project_t<13>(prm, hp, hc, basis, y, batch, st);
     case 41: return launch_project_t<21>(prm, hp, hc, basis, y, batch, st);
+#endif
+    case 25: return launch_project_t<13>(prm, hp, hc, basis, y, batch, st);
     default: return launch_project_t<0>(prm, hp, hc, basis, y, batch, st);
   }
 }
@@ -79,11 +81,13 @@ int launch_tdi(const Params& prm, int order, int gen, int mode, int channels, co
                int64_t batch, void* stream) {
   cudaStream_t st = (cudaStream_t)stream;
   switch (order) {
+#ifndef LR_DEV_ONLY_P13
     case 1: return launch_tdi_p<1>(prm, gen, mode, channels, y, out, batch, st);
     case 3: return launch_tdi_p<2>(prm, gen, mode, channels, y, out, batch, st);
     case 9: return launch_tdi_p<5>(prm, gen, mode, channels, y, out, batch, st);
-    case 25: return launch_tdi_p<13>(prm, gen, mode, channels, y, out, batch, st);
     case 41: return launch_tdi_p<21>(prm, gen, mode, channels, y, out, batch, st);
+#endif
+    case 25: return launch_tdi_p<13>(prm, gen, mode, channels, y, out, batch, st);
     default: return launch_tdi_p<0>(prm, gen, mode, channels, y, out, batch, st);
   }
 }

@@ -12,14 +12,19 @@
 
 namespace lr {
 
-constexpr int kProjThreads = 256;
+// Launch shapes, tuned on B200 (profiles/r1_tuning.md): both kernels are bound by the FP64 pipe and want
+// 12-24 resident warps per SM; letting ptxas take 160-250 registers per thread (one CTA per SM) halves the
+// throughput.  The caps below keep the order-25 kernels spill-free.
+constexpr int kProjThreads = 128;
 constexpr int kTdiThreads = 256;
+__host__ __device__ constexpr int proj_min_blocks(int PT) { return PT == 0 ? 2 : PT <= 13 ? 4 : 3; }
+__host__ __device__ constexpr int tdi_min_blocks(int PT) { return PT == 0 ? 2 : PT <= 13 ? 3 : 2; }
 
 // ---------------------------------------------------------------------------------------------- stage 1
 // grid.x = ntiles * batch; tile = blockIdx.x % ntiles, template = blockIdx.x / ntiles.
 // dynamic smem: D2 raw[W], D2 dif[W] with W = kProjThreads + halo_lo + halo_hi  (x = h+, y = hx)
 template <int PT>
-__global__ void __launch_bounds__(kProjThreads)
+__global__ void __launch_bounds__(kProjThreads, proj_min_blocks(PT))
 project_kernel(const Params prm, const double* __restrict__ hp, const double* __restrict__ hc,
                const double* __restrict__ basis /* [batch][9] */, double* __restrict__ y) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -68,7 +73,7 @@ project_kernel(const Params prm, const double* __restrict__ hp, const double* __
 // dynamic smem: double raw[6][W], dif[6][W], W = kTdiThreads + halo_lo + halo_hi
 // CH: LR_XYZ 0 | LR_AET 1 | LR_XYZ_AET 2 ; MODE: 0 nested, 1 sum
 template <int PT, int GEN, int MODE>
-__global__ void __launch_bounds__(kTdiThreads)
+__global__ void __launch_bounds__(kTdiThreads, tdi_min_blocks(PT))
 tdi_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ out, int channels) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int W = kTdiThreads + prm.halo_lo + prm.halo_hi;
