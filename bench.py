@@ -209,7 +209,7 @@ def run_reference(args, rank, world):
 def workload_config(w, batch, args):
     return {"workload": f"BASELINE.json configs[{ {'tiny': 0, 'year': 1, 'batch': 2}[args.workload] }] ({w.name})",
             "batch": batch, "n": w.n, "dt": w.dt, "lagrange_order": w.order, "tdi_gen": w.tdi_gen,
-            "chain": "nested", "channels": w.channels, "orbits": w.orbit_kind,
+            "chain": "nested", "channels": w.channels, "orbits": w.orbit_kind, "tdi_path": args.tdi_path,
             "l2": "flushed between steps (256 MiB memset outside the per-step event pairs)"}
 
 
@@ -224,7 +224,8 @@ def run_gpu(args, rank, world, local_rank):
     chunk = min(batch, args.chunk)
     n, T = w.n, w.order + 1
     nout = 6 if w.channels == "XYZ_AET" else 3
-    R = lr.Response(w.table(), w.dt, w.order, w.tdi_gen, t0=w.t0, chain="nested", channels=w.channels)
+    R = lr.Response(w.table(), w.dt, w.order, w.tdi_gen, t0=w.t0, chain="nested", channels=w.channels,
+                    tdi_path=args.tdi_path)
     stream = torch.cuda.current_stream()
 
     y = torch.empty((chunk, 6, n), dtype=torch.float64, device=dev)
@@ -373,6 +374,7 @@ def main():
     ap.add_argument("--peak-seconds", type=float, default=1.0)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tdi-path", default="auto", choices=["auto", "per_sample", "fir3", "fir4"])
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 

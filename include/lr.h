@@ -57,6 +57,18 @@ typedef struct {
 #define LR_OPT_CHAIN 2    /* LR_CHAIN_NESTED (default) | LR_CHAIN_SUM */
 #define LR_OPT_CHANNELS 3 /* LR_XYZ (default) | LR_AET | LR_XYZ_AET */
 #define LR_OPT_TDI_GEN 4  /* 1 | 2: changes the generation given to lr_create */
+#define LR_OPT_TDI_PATH 5 /* LR_TDI_AUTO (default) | LR_TDI_PER_SAMPLE | LR_TDI_FIR3 | LR_TDI_FIR4 */
+
+/* How lr_tdi evaluates the Lagrange weights (same result to rounding).
+ *   LR_TDI_PER_SAMPLE : every delayed term gets its own weight set at every sample.
+ *   LR_TDI_FIR3/4     : per tile of 224 samples the weights are a quadratic/cubic polynomial in time fitted
+ *                       through 3/4 nodes, and all terms of a series merge into one short FIR filter; tiles
+ *                       in which a delay crosses a whole number of samples use the per-sample code.
+ *   LR_TDI_AUTO       : FIR3 / FIR4 / PER_SAMPLE by the largest light-time rate of the orbit table. */
+#define LR_TDI_AUTO (-1)
+#define LR_TDI_PER_SAMPLE 0
+#define LR_TDI_FIR3 3
+#define LR_TDI_FIR4 4
 
 /* Chained delays D_{i1 i2 ... in} (eqs. 19-20).
  *   LR_CHAIN_SUM    : eq. 20 verbatim, the sum of the L's all taken at t.

@@ -10,7 +10,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "liblr.so")
 SOURCES = ("lr_api.cu", "lr_kernels.cu", "lr_peak.cu")
-HEADERS = ("lr_device.cuh", "lr_kernels.cuh", "lr_host.hpp", os.path.join("..", "..", "include", "lr.h"))
+INST_PT = (13, 21, 0, 5, 2, 1)   # lr_inst.cu is compiled once per compile-time pair count (0 = run-time P)
+HEADERS = ("lr_inst.cu", "lr_device.cuh", "lr_kernels.cuh", "lr_tdi_fir.cuh", "lr_host.hpp", os.path.join("..", "..", "include", "lr.h"))
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--fmad=true", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 
@@ -38,18 +39,22 @@ def build(force=False, verbose=False):
     objdir = os.path.join(_HERE, "build")
     os.makedirs(objdir, exist_ok=True)
 
-    def compile_one(src):
-        obj = os.path.join(objdir, src.replace(".cu", ".o"))
+    def compile_one(job):
+        src, pt = job
+        obj = os.path.join(objdir, src.replace(".cu", ".o") if pt is None else f"lr_inst_p{pt}.o")
         cmd = [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
+        if pt is not None:
+            cmd.insert(1, f"-DLR_INST_PT={pt}")
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
-            raise RuntimeError(f"nvcc failed on {src}:\n{r.stdout}\n{r.stderr}")
+            raise RuntimeError(f"nvcc failed on {src} (PT={pt}):\n{r.stdout}\n{r.stderr}")
         return obj, r.stderr
 
-    with concurrent.futures.ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
-        results = list(ex.map(compile_one, SOURCES))
+    jobs = [("lr_inst.cu", pt) for pt in INST_PT] + [(src, None) for src in SOURCES]
+    with concurrent.futures.ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
+        results = list(ex.map(compile_one, jobs))
     objs = [o for o, _ in results]
     tmp = LIB + ".tmp"
     r = subprocess.run([nvcc, "-shared", "-o", tmp, *objs, "-cudart", "static"], capture_output=True, text=True)

@@ -40,6 +40,8 @@ struct lr_handle {
   int64_t n_knots = 0;
   int order = 0, p = 0, gen = 2, chain = LR_CHAIN_NESTED, channels = LR_XYZ;
   double r_max = 0, l_max = 0;
+  double max_ldot = 0;   // max |dL_ij/dt| over the table (dimensionless), from the spline
+  int tdi_path = -1;     // LR_OPT_TDI_PATH: -1 auto | 0 generic | 3 | 4
   double bk[lr::kPMax + 1];
   // device state
   lr::D4* coef = nullptr;
@@ -84,6 +86,7 @@ lr::Params make_params(const lr_handle* h, int64_t n) {
   P.m_proj = (int)h->m_proj();
   P.m_front = (int)h->m_front(h->gen);
   P.m_back = (int)h->m_back();
+  P.chain_sum = h->chain == LR_CHAIN_SUM ? 1 : 0;
   memcpy(P.bk, h->bk, sizeof(P.bk));
   return P;
 }
@@ -162,6 +165,19 @@ int lr_create(const lr_orbits* orb, double dt, int order, int tdi_gen, lr_handle
     for (int s = 0; s < 6; ++s) lr::fit_channel(orb->ltt + (int64_t)s * nk, nk, orb->knot_dt, coef.data() + (size_t)(9 + s) * (nk - 1));
   } catch (...) { delete h; return LR_ENOMEM; }
 
+  // largest light-time rate of the table: decides whether lr_tdi may treat the delays of a tile as a
+  // low-degree polynomial in time (lr_tdi_fir.cuh)
+  for (int s = 0; s < 6; ++s)
+    for (int64_t i = 0; i + 1 < nk; ++i) {
+      const lr::D4& c = coef[(size_t)(9 + s) * (nk - 1) + i];
+      double m = fmax(fabs(c.y), fabs(c.y + 2.0 * c.z + 3.0 * c.w));
+      if (c.w != 0.0) {
+        const double u = -c.z / (3.0 * c.w);
+        if (u > 0.0 && u < 1.0) m = fmax(m, fabs(c.y + u * (2.0 * c.z + 3.0 * c.w * u)));
+      }
+      h->max_ldot = fmax(h->max_ldot, m / orb->knot_dt);
+    }
+
   cudaError_t e = cudaMalloc(&h->coef, coef.size() * sizeof(lr::D4));
   if (e == cudaSuccess) e = cudaMemcpy(h->coef, coef.data(), coef.size() * sizeof(lr::D4), cudaMemcpyHostToDevice);
   if (e != cudaSuccess) {
@@ -201,6 +217,10 @@ int lr_set_option(lr_handle* h, int key, double value) {
     case LR_OPT_TDI_GEN:
       if (value != 1 && value != 2) return LR_EINVAL;
       h->gen = (int)value; return LR_OK;
+    case LR_OPT_TDI_PATH:
+      if (value != LR_TDI_AUTO && value != LR_TDI_PER_SAMPLE && value != LR_TDI_FIR3 && value != LR_TDI_FIR4)
+        return LR_EINVAL;
+      h->tdi_path = (int)value; return LR_OK;
     default: return LR_EINVAL;
   }
 }
@@ -240,9 +260,30 @@ int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out,
   const double reach = (double)(h->gen == 1 ? 4 : 8) * 1.001 * h->l_max;
   if (!in_table(h, mf, n - mb - 1, reach)) return LR_ERANGE;
   lr::Params P = make_params(h, n);
-  P.halo_lo = (int)(mf - h->m_proj()); P.halo_hi = h->p + 2;
-  P.ntiles = (int)((n + lr::kTdiThreads - 1) / lr::kTdiThreads);
-  const int e = lr::launch_tdi(P, h->order, h->gen, h->chain, h->channels, y, out, batch, stream);
+  // path: per-tile polynomial FIR when the delays drift slowly enough, else exact per-sample weights
+  const int nlinks = h->gen == 1 ? 3 : 7;  // links in the longest delayed term
+  const double de = (double)nlinks * h->max_ldot * (double)lr::kFirTile;  // change of eps over one tile
+  int path = h->tdi_path;
+  if (path == LR_TDI_AUTO) path = de <= 6e-6 ? LR_TDI_FIR3 : de <= 1.5e-4 ? LR_TDI_FIR4 : LR_TDI_PER_SAMPLE;
+  if (path != LR_TDI_PER_SAMPLE) {
+    const int imax = (int)h->tdi_reach(h->gen);
+    const int wc = ((imax + 2 * h->p - 2 + lr::kFirR - 1) / lr::kFirR) * lr::kFirR;
+    const int back = wc - (h->p - 1);
+    P.fir_wc = wc;
+    P.halo_lo = back > (int)(mf - h->m_proj()) ? back : (int)(mf - h->m_proj());
+    P.halo_hi = h->p + lr::kFirR;
+    P.ntiles = (int)((n + lr::kFirTile - 1) / lr::kFirTile);
+    const int W = lr::kFirTile + P.halo_lo + P.halo_hi;
+    const size_t smem = path == LR_TDI_FIR3
+        ? (h->gen == 1 ? lr::FirSmem<1, 3>(W, wc, h->p).total : lr::FirSmem<2, 3>(W, wc, h->p).total)
+        : (h->gen == 1 ? lr::FirSmem<1, 4>(W, wc, h->p).total : lr::FirSmem<2, 4>(W, wc, h->p).total);
+    if (smem > 200 * 1024) path = LR_TDI_PER_SAMPLE;
+  }
+  if (path == LR_TDI_PER_SAMPLE) {
+    P.halo_lo = (int)(mf - h->m_proj()); P.halo_hi = h->p + 2;
+    P.ntiles = (int)((n + lr::kTdiThreads - 1) / lr::kTdiThreads);
+  }
+  const int e = lr::launch_tdi(P, h->order, h->gen, path, h->channels, y, out, batch, stream);
   if (e != 0) { h->last_cuda = e; return LR_ECUDA; }
   return LR_OK;
 }

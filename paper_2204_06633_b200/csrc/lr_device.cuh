@@ -60,6 +60,8 @@ struct Params {
   int m_proj, m_front, m_back;
   int halo_lo, halo_hi;  // staged window = [n0 - halo_lo, n0 + B + halo_hi)
   int ntiles;
+  int fir_wc;            // FIR path: taps per series (multiple of kFirR)
+  int chain_sum;         // 0: nested delays (default), 1: eq. 20 sums of the L at t
   double bk[kPMax + 1];  // bk[k] = 1 / prod_{m != k} (k - m), m = -P+1..P, for k = 1..P
 };
 
@@ -212,16 +214,17 @@ __host__ __device__ constexpr int chain_a(int k) { return k == 0 ? 3 : k == 1 ? 
 __host__ __device__ constexpr int chain_b(int k) { return k == 0 ? 0 : k == 1 ? 5 : k == 2 ? 3 : k == 3 ? 2 : k == 4 ? 3 : k == 5 ? 2 : k == 6 ? 0 : 5; }
 
 // One time sample of eqs. 17-18 for X, Y, Z.  raw/dif: six staged series [6][W] and first differences.
-// MODE 0: nested delays, 1: eq. 20 sums.
-template <int PT, int GEN, int MODE>
+// prm.chain_sum 0: nested delays, 1: eq. 20 sums.
+template <int PT, int GEN>
 LR_HD void tdi_sample(const Params& prm, const double* raw, const double* dif, int W, int nl, double trel,
                       double (&xyz)[3]) {
   constexpr int NK = GEN == 1 ? 4 : 8;
   const int a_min = PT > 0 ? PT : prm.p, a_max = W - (PT > 0 ? PT : prm.p);
   auto clampi = [](int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); };
 
-  double Lt[6];
-  if (MODE == 1) {  // eq. 20: every L at t
+  const bool sum_mode = prm.chain_sum != 0;
+  double Lt[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+  if (sum_mode) {  // eq. 20: every L at t
 #pragma unroll
     for (int s = 0; s < 6; ++s) Lt[s] = spline_eval(prm, 9 + s, trel);
   }
@@ -244,7 +247,7 @@ LR_HD void tdi_sample(const Params& prm, const double* raw, const double* dif, i
           interp_sbp<PT, 1>(prm, eps, aA[k], [&](int m, double (&o)[1]) { o[0] = ds[m]; }, S);
           acc -= S[0];
         }
-        if (k + 1 < NK) d += MODE == 1 ? Lt[s] : spline_eval(prm, 9 + s, trel - d);
+        if (k + 1 < NK) d += sum_mode ? Lt[s] : spline_eval(prm, 9 + s, trel - d);
       }
     }
     {
@@ -263,7 +266,7 @@ LR_HD void tdi_sample(const Params& prm, const double* raw, const double* dif, i
         }
         // same series: + y_s at the anchor of A's term k^2, - y_s at this term's anchor
         acc += raw[s * W + aA[k ^ 2]] - raw[s * W + aB];
-        if (k + 1 < NK) d += MODE == 1 ? Lt[s] : spline_eval(prm, 9 + s, trel - d);
+        if (k + 1 < NK) d += sum_mode ? Lt[s] : spline_eval(prm, 9 + s, trel - d);
       }
     }
     xyz[ch] = acc;

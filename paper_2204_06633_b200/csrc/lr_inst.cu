@@ -1,0 +1,80 @@
+// lr_inst.cu — kernel instantiations for ONE compile-time pair count LR_INST_PT (build.py compiles this file
+// once per fast order; LR_INST_PT = 0 is the run-time-P build that serves every other odd order).
+#include <cuda_runtime.h>
+
+#include <atomic>
+
+#include "lr_kernels.cuh"
+
+#ifndef LR_INST_PT
+#error "compile with -DLR_INST_PT=<P>"
+#endif
+
+namespace lr {
+
+extern std::atomic<int64_t> g_launches;
+
+template <class K>
+static cudaError_t prepare(K kernel, size_t smem) {
+  if (smem > 48 * 1024) return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  return cudaSuccess;
+}
+
+template <int PT>
+int launch_project_t(const Params& prm, const double* hp, const double* hc, const double* basis, double* y,
+                     int64_t batch, void* stream) {
+  const size_t W = (size_t)kProjThreads + prm.halo_lo + prm.halo_hi;
+  const size_t smem = 2 * W * sizeof(D2);
+  cudaError_t e = prepare(project_kernel<PT>, smem);
+  if (e != cudaSuccess) return (int)e;
+  const int64_t grid = (int64_t)prm.ntiles * batch;
+  project_kernel<PT><<<(unsigned)grid, kProjThreads, smem, (cudaStream_t)stream>>>(prm, hp, hc, basis, y);
+  g_launches.fetch_add(1);
+  return (int)cudaGetLastError();
+}
+
+template <int PT, int GEN>
+static int launch_tdi_generic(const Params& prm, int channels, const double* y, double* out, int64_t batch,
+                              cudaStream_t st) {
+  const size_t W = (size_t)kTdiThreads + prm.halo_lo + prm.halo_hi;
+  const size_t smem = 12 * W * sizeof(double);
+  cudaError_t e = prepare(tdi_kernel<PT, GEN>, smem);
+  if (e != cudaSuccess) return (int)e;
+  const int64_t grid = (int64_t)prm.ntiles * batch;
+  tdi_kernel<PT, GEN><<<(unsigned)grid, kTdiThreads, smem, st>>>(prm, y, out, channels);
+  g_launches.fetch_add(1);
+  return (int)cudaGetLastError();
+}
+
+template <int PT, int GEN, int NN>
+static int launch_tdi_fir(const Params& prm, int channels, const double* y, double* out, int64_t batch,
+                          cudaStream_t st) {
+  const int W = kFirTile + prm.halo_lo + prm.halo_hi;
+  const FirSmem<GEN, NN> plan(W, prm.fir_wc, PT > 0 ? PT : prm.p);
+  cudaError_t e = prepare(tdi_fir_kernel<PT, GEN, NN>, plan.total);
+  if (e != cudaSuccess) return (int)e;
+  const int64_t grid = (int64_t)prm.ntiles * batch;
+  tdi_fir_kernel<PT, GEN, NN><<<(unsigned)grid, kFirThreads, plan.total, st>>>(prm, y, out, channels);
+  g_launches.fetch_add(1);
+  return (int)cudaGetLastError();
+}
+
+template <int PT>
+int launch_tdi_t(const Params& prm, int gen, int path, int channels, const double* y, double* out, int64_t batch,
+                 void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  if (path == kPathFir3)
+    return gen == 1 ? launch_tdi_fir<PT, 1, 3>(prm, channels, y, out, batch, st)
+                    : launch_tdi_fir<PT, 2, 3>(prm, channels, y, out, batch, st);
+  if (path == kPathFir4)
+    return gen == 1 ? launch_tdi_fir<PT, 1, 4>(prm, channels, y, out, batch, st)
+                    : launch_tdi_fir<PT, 2, 4>(prm, channels, y, out, batch, st);
+  return gen == 1 ? launch_tdi_generic<PT, 1>(prm, channels, y, out, batch, st)
+                  : launch_tdi_generic<PT, 2>(prm, channels, y, out, batch, st);
+}
+
+template int launch_project_t<LR_INST_PT>(const Params&, const double*, const double*, const double*, double*,
+                                          int64_t, void*);
+template int launch_tdi_t<LR_INST_PT>(const Params&, int, int, int, const double*, double*, int64_t, void*);
+
+}  // namespace lr

@@ -1,7 +1,7 @@
 // lr_kernels.cuh — the two CUDA kernels of liblr (sm_100a) and their launchers' declarations.
 //
 //   project_kernel<PT>       : PAPER.md eqs. 10-16, one thread per time sample, all six links
-//   tdi_kernel<PT,GEN,MODE>  : PAPER.md eqs. 17-21, one thread per time sample, X, Y, Z (+ A, E, T)
+//   tdi_kernel<PT,GEN>       : PAPER.md eqs. 17-21, one thread per time sample, X, Y, Z (+ A, E, T)
 //
 // Both stage the window a tile of samples needs (raw samples and their exact first differences) in
 // shared memory with coalesced loads, keep the Lagrange pair products in registers, and write coalesced
@@ -71,8 +71,8 @@ project_kernel(const Params prm, const double* __restrict__ hp, const double* __
 
 // ---------------------------------------------------------------------------------------------- stage 2
 // dynamic smem: double raw[6][W], dif[6][W], W = kTdiThreads + halo_lo + halo_hi
-// CH: LR_XYZ 0 | LR_AET 1 | LR_XYZ_AET 2 ; MODE: 0 nested, 1 sum
-template <int PT, int GEN, int MODE>
+// channels: LR_XYZ 0 | LR_AET 1 | LR_XYZ_AET 2
+template <int PT, int GEN>
 __global__ void __launch_bounds__(kTdiThreads, tdi_min_blocks(PT))
 tdi_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ out, int channels) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -107,7 +107,7 @@ tdi_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ 
   }
 
   double xyz[3];
-  tdi_sample<PT, GEN, MODE>(prm, raw, dif, W, n - g0, sample_trel(prm, n), xyz);
+  tdi_sample<PT, GEN>(prm, raw, dif, W, n - g0, sample_trel(prm, n), xyz);
 
   const int64_t N = prm.n;
   if (channels != 1) { ob[0] = xyz[0]; ob[N] = xyz[1]; ob[2 * N] = xyz[2]; }
@@ -120,14 +120,34 @@ tdi_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ 
   }
 }
 
+}  // namespace lr
+
+#include "lr_tdi_fir.cuh"
+
+namespace lr {
+
+// lr_tdi paths
+constexpr int kPathGeneric = 0;  // tdi_kernel: exact per-sample weights
+constexpr int kPathFir3 = 3;     // tdi_fir_kernel, quadratic in tile time
+constexpr int kPathFir4 = 4;     // tdi_fir_kernel, cubic in tile time
+
 // small helper kernel: spline channel at arbitrary absolute times (lr_eval_orbit)
 __global__ void eval_orbit_kernel(const Params prm, int ch, double t_start, const double* __restrict__ t,
                                   int64_t m, double* __restrict__ out);
 
-// launchers (lr_kernels_*.cu); return cudaError_t as int
+// Launchers, one explicit instantiation per compile-time pair count PT (lr_inst.cu is compiled once per
+// PT; PT = 0 reads P at run time).  They return cudaError_t as int.
+template <int PT>
+int launch_project_t(const Params& prm, const double* hp, const double* hc, const double* basis, double* y,
+                     int64_t batch, void* stream);
+template <int PT>
+int launch_tdi_t(const Params& prm, int gen, int path, int channels, const double* y, double* out, int64_t batch,
+                 void* stream);
+
+// dispatch on the Lagrange order (lr_kernels.cu)
 int launch_project(const Params& prm, int order, const double* hp, const double* hc, const double* basis,
                    double* y, int64_t batch, void* stream);
-int launch_tdi(const Params& prm, int order, int gen, int mode, int channels, const double* y, double* out,
+int launch_tdi(const Params& prm, int order, int gen, int path, int channels, const double* y, double* out,
                int64_t batch, void* stream);
 
 }  // namespace lr

@@ -1,0 +1,370 @@
+// lr_tdi_fir.cuh — TDI as a slowly time-varying FIR filter (the fast path of lr_tdi).
+//
+// TDI delays drift by ~1e-8..1e-6 samples per sample (armlength rates of 1-100 m/s against c), so inside
+// a tile of a few hundred samples the Lagrange weights of every delayed term are, to rounding, a low-degree
+// polynomial in the tile time tau in [-1,1].  Per tile the CTA therefore
+//   A  walks the delay chains of eqs. 17-20 at NN nodes of the tile                      (fir_chain_nodes)
+//   B  splits every term's delay into an integer shift, fixed over the tile, and eps(node); tiles where a
+//      shift could change inside the tile, or where the polynomial model is not safe, are flagged and run
+//      the exact per-sample code instead                                                   (fir_split_terms)
+//   C  evaluates the summation-by-parts coefficients of every term at the nodes           (fir_node_coeffs)
+//   D  merges all terms that act on one series, anchors included, into one coefficient array per
+//      (channel, series, power of tau)                                                     (fir_merge)
+//   E  applies X(n) = sum_p tau_n^p sum_series sum_m K_p[series][m] * dif_series[n + m]   (fir_apply)
+// so the per-sample work drops from 36 weight sets + 36 dot products to 4 series x NN short FIR filters per
+// channel.  Interpolating the coefficients through NN Chebyshev-Lobatto nodes costs a relative error
+// <= 2 (de/2)^3 (NN = 3) or 1.3 (de/2)^4 (NN = 4) with de the change of eps over the tile; lr_tdi picks NN
+// so that this stays below 1e-16 and falls back to the per-sample kernel otherwise.
+//
+// Each phase is a function of (tid, nthreads) that strides over its work items, so the kernel calls it with
+// (threadIdx.x, blockDim.x) between __syncthreads() and a host harness can call it with (0, 1).
+#pragma once
+#include "lr_device.cuh"
+
+namespace lr {
+
+constexpr int kFirR = 7;          // consecutive samples per thread (odd: conflict-free 64-bit smem reads)
+constexpr int kFirKStride = 4;    // doubles per (series, m) coefficient record (NN <= 4)
+
+// series used by channel X, in "local" order 13, 31, 12, 21; Y and Z rotate the slots
+__host__ __device__ constexpr int fir_base_slot(int sl) { return sl == 0 ? 3 : sl == 1 ? 2 : sl == 2 ? 0 : 5; }
+// local series of term k of chain A / chain B
+__host__ __device__ constexpr int fir_sl_a(int k) { return k == 0 ? 0 : k == 1 ? 1 : k == 2 ? 2 : k == 3 ? 3 : k == 4 ? 2 : k == 5 ? 3 : k == 6 ? 0 : 1; }
+__host__ __device__ constexpr int fir_sl_b(int k) { return fir_sl_a(k ^ 2); }
+
+LR_HD int rot_slot_rt(int s, int r) {
+  const int rx = (s == 0 || s == 3) ? 0 : (s == 1 || s == 5) ? 1 : 2;
+  const int tx = (s == 2 || s == 5) ? 0 : (s == 0 || s == 4) ? 1 : 2;
+  const int i = (rx + r) % 3, j = (tx + r) % 3;
+  return (i == 0 && j == 1) ? 0 : (i == 1 && j == 2) ? 1 : (i == 2 && j == 0) ? 2
+       : (i == 0 && j == 2) ? 3 : (i == 2 && j == 1) ? 4 : 5;
+}
+
+template <int NN> LR_HD double fir_node(int i);
+template <> LR_HD double fir_node<3>(int i) { return i == 0 ? -1.0 : i == 1 ? 0.0 : 1.0; }
+template <> LR_HD double fir_node<4>(int i) { return i == 0 ? -1.0 : i == 1 ? -0.5 : i == 2 ? 0.5 : 1.0; }
+
+// Per-tile scratch in shared memory (the kernel carves it out of dynamic smem).
+template <int GEN, int NN>
+struct FirTile {
+  static constexpr int NK = GEN == 1 ? 4 : 8;        // terms per chain (term 0 has no delay)
+  static constexpr int NT = 6 * (NK - 1);            // delayed terms of X, Y, Z
+  double dnode[6][NN][NK];                           // chain delay d_k [s] at the nodes, [ch*2+chain]
+  double eps[NT][NN];                                // eps of term (ch*2+chain)*(NK-1) + k-1 at the nodes
+  int shift[NT];                                     // integer part I = ceil(D), fixed over the tile
+  int generic;                                       // != 0: run the per-sample code for this tile
+};
+
+// A: chain delays at the nodes.  x0 = sample index of the tile's first sample, B = tile length.
+template <int GEN, int NN>
+LR_HD void fir_chain_nodes(const Params& prm, FirTile<GEN, NN>& T, int n0, int B, int tid, int nthreads) {
+  constexpr int NK = FirTile<GEN, NN>::NK;
+  for (int w = tid; w < 6 * NN; w += nthreads) {
+    const int cc = w / NN, node = w - cc * NN;       // cc = ch*2 + chain
+    const int ch = cc >> 1, chain = cc & 1;
+    const double xs = 0.5 * (double)(B - 1) * (1.0 + fir_node<NN>(node));  // position inside the tile [samples]
+    const double trel = fma((double)n0 + xs, prm.dt, prm.trel0);
+    double d = 0.0;
+    T.dnode[cc][node][0] = 0.0;
+#pragma unroll
+    for (int k = 0; k + 1 < NK; ++k) {
+      const int s = rot_slot_rt(chain == 0 ? chain_a(k) : chain_b(k), ch);
+      d += spline_eval(prm, 9 + s, prm.chain_sum ? trel : trel - d);
+      T.dnode[cc][node][k + 1] = d;
+    }
+  }
+}
+
+// B: integer shift and eps(node) per delayed term; decide whether the tile may use the FIR path.
+template <int GEN, int NN>
+LR_HD void fir_split_terms(const Params& prm, FirTile<GEN, NN>& T, int tid, int nthreads) {
+  constexpr int NK = FirTile<GEN, NN>::NK;
+  constexpr int NT = FirTile<GEN, NN>::NT;
+  for (int term = tid; term < NT; term += nthreads) {
+    const int cc = term / (NK - 1), k = term - cc * (NK - 1) + 1;
+    double D[NN], lo = 1e300, hi = -1e300;
+#pragma unroll
+    for (int i = 0; i < NN; ++i) {
+      D[i] = T.dnode[cc][i][k] * prm.inv_dt;
+      lo = D[i] < lo ? D[i] : lo;
+      hi = D[i] > hi ? D[i] : hi;
+    }
+    const double I = ceil(lo);
+    const double spread = hi - lo;
+    // every sample of the tile must see ceil(D) == I: the nodes include both ends of the tile, an interior
+    // extremum can exceed the node range by less than `spread`
+    const double guard = spread + 1e-12;
+    const bool safe = (spread == 0.0) || ((I - hi) >= guard && (lo - (I - 1.0)) >= guard);
+    T.shift[term] = (int)I;
+#pragma unroll
+    for (int i = 0; i < NN; ++i) T.eps[term][i] = I - D[i];
+    if (!safe) T.generic = 1;   // benign race: every writer stores 1
+  }
+}
+
+// The 2P-1 summation-by-parts coefficients of one interpolation: value = raw[a] - sum_j c[j+P-1] dif[a-1+j],
+// j = 1-P..P-1, with c_j = C_j (j <= 0) and -E_j (j >= 1)   (cf. interp_sbp).
+template <int PT>
+LR_HD void sbp_coeffs(const Params& prm, double eps, double* c) {
+  const int P = PT > 0 ? PT : prm.p;
+  double R[PT > 0 ? PT : kPMax];
+  const double z = fma(eps, eps, -eps);
+  double pre = 1.0;
+#pragma unroll
+  for (int k = 1; k <= P; ++k) {
+    R[k - 1] = pre * prm.bk[k];
+    pre *= z - (double)(k * (k - 1));
+  }
+  double suf = 1.0, C = 0.0, E = 0.0;
+#pragma unroll
+  for (int k = P; k >= 1; --k) {
+    const double Rk = R[k - 1] * suf;
+    suf *= z - (double)(k * (k - 1));
+    C = fma(Rk, (double)k - eps, C);
+    c[(1 - k) + P - 1] = C;                       // j = 1-k
+    if (k >= 2) {
+      E = fma(Rk, eps + (double)(k - 1), E);
+      c[(k - 1) + P - 1] = -E;                    // j = k-1
+    }
+  }
+}
+
+// C: coefficients of every delayed term at every node: cnode[term][node][2P-1]
+template <int PT, int GEN, int NN>
+LR_HD void fir_node_coeffs(const Params& prm, const FirTile<GEN, NN>& T, double* cnode, int tid, int nthreads) {
+  constexpr int NT = FirTile<GEN, NN>::NT;
+  const int P = PT > 0 ? PT : prm.p;
+  const int L = 2 * P - 1;
+  for (int w = tid; w < NT * NN; w += nthreads) {
+    const int term = w / NN, node = w - term * NN;
+    sbp_coeffs<PT>(prm, T.eps[term][node], cnode + (size_t)w * L);
+  }
+}
+
+// D: merge.  K[((ch*4 + sl)*Wc + m)*kFirKStride + p] = coefficient of tau^p of dif_series[nl + m - back]
+// where back = Wc - (P - 1) is the number of staged differences behind the sample.  m_rel = m - back.
+template <int PT, int GEN, int NN>
+LR_HD void fir_merge(const Params& prm, const FirTile<GEN, NN>& T, const double* cnode, double* K, int Wc,
+                     int tid, int nthreads) {
+  constexpr int NK = FirTile<GEN, NN>::NK;
+  const int P = PT > 0 ? PT : prm.p;
+  const int L = 2 * P - 1;
+  const int back = Wc - (P - 1);
+  for (int w = tid; w < 12 * Wc; w += nthreads) {
+    const int cs = w / Wc, m = w - cs * Wc;       // cs = ch*4 + sl
+    const int ch = cs >> 2, sl = cs & 3;
+    const int m_rel = m - back;
+    double v[NN];
+#pragma unroll
+    for (int i = 0; i < NN; ++i) v[i] = 0.0;
+#pragma unroll
+    for (int chain = 0; chain < 2; ++chain) {
+      const double sign = chain == 0 ? 1.0 : -1.0;
+#pragma unroll
+      for (int k = 0; k < NK; ++k) {
+        if ((chain == 0 ? fir_sl_a(k) : fir_sl_b(k)) != sl) continue;
+        const int term = (ch * 2 + chain) * (NK - 1) + (k - 1);
+        const int I = k == 0 ? 0 : T.shift[term];
+        const int o = k == 0 ? 0 : 1 - I;         // anchor offset of the term: value = raw[nl+o] - S
+        // anchors: term k of chain B and term k^2 of chain A carry the same series with opposite signs;
+        // raw[nl+oA] - raw[nl+oB] = +/- the sum of the first differences between the two anchors
+        double step = 0.0;
+        if (chain == 1) {
+          const int ka = k ^ 2;
+          const int oa = ka == 0 ? 0 : 1 - T.shift[(ch * 2) * (NK - 1) + (ka - 1)];
+          step = (m_rel >= o && m_rel < oa) ? 1.0 : (m_rel >= oa && m_rel < o) ? -1.0 : 0.0;
+        }
+        const int j = m_rel + I;                  // dif index nl - I + j
+        const bool in = k > 0 && j >= 1 - P && j <= P - 1;
+#pragma unroll
+        for (int i = 0; i < NN; ++i) {
+          double c = step;
+          if (in) c -= sign * cnode[((size_t)term * NN + i) * L + (j + P - 1)];
+          v[i] += c;
+        }
+      }
+    }
+    double* out = K + (size_t)w * kFirKStride;
+    if (NN == 3) {          // nodes -1, 0, 1
+      out[0] = v[1];
+      out[1] = 0.5 * (v[2] - v[0]);
+      out[2] = 0.5 * (v[0] + v[2]) - v[1];
+      out[3] = 0.0;
+    } else {                // nodes -1, -1/2, 1/2, 1
+      const double s1 = 0.5 * (v[NN - 1] + v[0]), d1 = 0.5 * (v[NN - 1] - v[0]);
+      const double s2 = 0.5 * (v[NN - 2] + v[1]), d2 = 0.5 * (v[NN - 2] - v[1]);
+      const double a2 = (s1 - s2) * (4.0 / 3.0), a3 = (d1 - 2.0 * d2) * (4.0 / 3.0);
+      out[0] = s2 - 0.25 * a2;
+      out[1] = d1 - a3;
+      out[2] = a2;
+      out[3] = a3;
+    }
+  }
+}
+
+// E: apply.  One work item = kFirR consecutive samples of one channel.  dif: [6][W]; res: [3][B] (tile
+// staging of X, Y, Z).  nl0 = staged index of the tile's first sample; Wc is a multiple of kFirR.
+template <int NN>
+LR_HD void fir_apply(const double* dif, int W, const double* K, int Wc, int P, int nl0, int B, double* res,
+                     int tid, int nthreads) {
+  constexpr int R = kFirR;
+  const int groups = (B + R - 1) / R;
+  const int back = Wc - (P - 1);
+  for (int w = tid; w < 3 * groups; w += nthreads) {
+    const int ch = w / groups, g = w - ch * groups;
+    const int i0 = g * R;                                  // first sample of the group inside the tile
+    double acc[NN][R];
+#pragma unroll
+    for (int p = 0; p < NN; ++p)
+#pragma unroll
+      for (int r = 0; r < R; ++r) acc[p][r] = 0.0;
+#pragma unroll 1
+    for (int sl = 0; sl < 4; ++sl) {
+      const double* d = dif + rot_slot_rt(fir_base_slot(sl), ch) * W + (nl0 + i0 - back);
+      const double* kk = K + (size_t)((ch * 4 + sl) * Wc) * kFirKStride;
+      double win[2 * R];
+#pragma unroll
+      for (int r = 0; r < R; ++r) win[r] = d[r];
+#pragma unroll 1
+      for (int m0 = 0; m0 < Wc; m0 += R) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) win[R + r] = d[m0 + R + r];
+#pragma unroll
+        for (int mm = 0; mm < R; ++mm) {
+          double kc[NN];
+#pragma unroll
+          for (int p = 0; p < NN; ++p) kc[p] = kk[(m0 + mm) * kFirKStride + p];
+#pragma unroll
+          for (int r = 0; r < R; ++r)
+#pragma unroll
+            for (int p = 0; p < NN; ++p) acc[p][r] = fma(kc[p], win[mm + r], acc[p][r]);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) win[r] = win[R + r];
+      }
+    }
+    const double half = 0.5 * (double)(B - 1);
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      const int i = i0 + r;
+      if (i < B) {
+        const double tau = ((double)i - half) / half;
+        double v = acc[NN - 1][r];
+#pragma unroll
+        for (int p = NN - 2; p >= 0; --p) v = fma(v, tau, acc[p][r]);
+        res[ch * B + i] = v;
+      }
+    }
+  }
+}
+
+}  // namespace lr
+
+#ifdef __CUDACC__
+namespace lr {
+
+constexpr int kFirGroups = 32;                    // groups of kFirR samples per channel and tile
+constexpr int kFirTile = kFirGroups * kFirR;      // 224 samples per tile
+constexpr int kFirThreads = 3 * kFirGroups;       // one warp per channel
+
+// shared-memory plan of tdi_fir_kernel (bytes), used by the launcher too
+template <int GEN, int NN>
+struct FirSmem {
+  size_t raw, dif, tile, cnode, K, total;
+  __host__ __device__ FirSmem(int W, int Wc, int P) {
+    const size_t nt = FirTile<GEN, NN>::NT;
+    raw = 0;
+    dif = raw + (size_t)6 * W * sizeof(double);
+    tile = dif + (size_t)6 * W * sizeof(double);
+    cnode = tile + ((sizeof(FirTile<GEN, NN>) + 15) / 16) * 16;
+    size_t cn = nt * NN * (size_t)(2 * P - 1) * sizeof(double);
+    const size_t rs = (size_t)3 * kFirTile * sizeof(double);   // res aliases cnode
+    if (cn < rs) cn = rs;
+    K = cnode + ((cn + 15) / 16) * 16;
+    total = K + (size_t)12 * Wc * kFirKStride * sizeof(double);
+  }
+};
+
+// grid.x = ntiles * batch (tiles of kFirTile samples).  prm.halo_lo/hi describe the staged window.
+template <int PT, int GEN, int NN>
+__global__ void __launch_bounds__(kFirThreads)
+tdi_fir_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ out, int channels) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int B = kFirTile;
+  const int P = PT > 0 ? PT : prm.p;
+  const int W = B + prm.halo_lo + prm.halo_hi;
+  const int Wc = prm.fir_wc;
+  const FirSmem<GEN, NN> plan(W, Wc, P);
+  double* raw = reinterpret_cast<double*>(smem_raw + plan.raw);
+  double* dif = reinterpret_cast<double*>(smem_raw + plan.dif);
+  FirTile<GEN, NN>& T = *reinterpret_cast<FirTile<GEN, NN>*>(smem_raw + plan.tile);
+  double* cnode = reinterpret_cast<double*>(smem_raw + plan.cnode);
+  double* res = cnode;
+  double* K = reinterpret_cast<double*>(smem_raw + plan.K);
+
+  const int tid = threadIdx.x;
+  const int tile = blockIdx.x % prm.ntiles;
+  const int64_t b = blockIdx.x / prm.ntiles;
+  const int n0 = tile * B;
+  const int g0 = n0 - prm.halo_lo;
+  const int64_t N = prm.n;
+  const int nout = channels == 2 ? 6 : 3;
+  double* ob = out + b * nout * N;
+
+  const int v_lo = prm.m_front, v_hi = prm.n - prm.m_back;   // valid samples [v_lo, v_hi)
+  if (n0 + B <= v_lo || n0 >= v_hi) {                        // tile entirely inside a margin
+    for (int i = tid; i < B; i += kFirThreads)
+      if (n0 + i < prm.n)
+        for (int c = 0; c < nout; ++c) ob[(int64_t)c * N + n0 + i] = 0.0;
+    return;
+  }
+
+  const double* yb = y + b * 6 * N;
+  for (int m = tid; m < 6 * W; m += kFirThreads) {
+    const int s = m / W, g = g0 + (m - s * W);
+    raw[m] = (g >= 0 && g < prm.n) ? __ldg(yb + (int64_t)s * N + g) : 0.0;
+  }
+  if (tid == 0) T.generic = 0;
+  __syncthreads();
+  for (int m = tid; m < 6 * W; m += kFirThreads) {
+    const int w = m % W;
+    dif[m] = (w < W - 1) ? raw[m + 1] - raw[m] : 0.0;
+  }
+  fir_chain_nodes<GEN, NN>(prm, T, n0, B, tid, kFirThreads);
+  __syncthreads();
+  fir_split_terms<GEN, NN>(prm, T, tid, kFirThreads);
+  __syncthreads();
+  const int nl0 = prm.halo_lo;
+  if (T.generic) {
+    // exact per-sample path: a delay's integer part may change inside this tile
+    for (int i = tid; i < B; i += kFirThreads) {
+      const int n = n0 + i;
+      double xyz[3] = {0.0, 0.0, 0.0};
+      if (n >= v_lo && n < v_hi) tdi_sample<PT, GEN>(prm, raw, dif, W, nl0 + i, sample_trel(prm, n), xyz);
+      res[i] = xyz[0]; res[B + i] = xyz[1]; res[2 * B + i] = xyz[2];
+    }
+  } else {
+    fir_node_coeffs<PT, GEN, NN>(prm, T, cnode, tid, kFirThreads);
+    __syncthreads();
+    fir_merge<PT, GEN, NN>(prm, T, cnode, K, Wc, tid, kFirThreads);
+    __syncthreads();
+    fir_apply<NN>(dif, W, K, Wc, P, nl0, B, res, tid, kFirThreads);
+  }
+  __syncthreads();
+  for (int i = tid; i < B; i += kFirThreads) {
+    const int n = n0 + i;
+    if (n >= prm.n) break;
+    const bool valid = n >= v_lo && n < v_hi;
+    const double X = valid ? res[i] : 0.0, Y = valid ? res[B + i] : 0.0, Z = valid ? res[2 * B + i] : 0.0;
+    if (channels != 1) { ob[n] = X; ob[N + n] = Y; ob[2 * N + n] = Z; }
+    if (channels != 0) {  // eq. 21
+      double* oa = channels == 2 ? ob + 3 * N : ob;
+      oa[n] = (Z - X) * 0.70710678118654752440;
+      oa[N + n] = (X - 2.0 * Y + Z) * 0.40824829046386301637;
+      oa[2 * N + n] = (X + Y + Z) * 0.57735026918962576451;
+    }
+  }
+}
+
+}  // namespace lr
+#endif

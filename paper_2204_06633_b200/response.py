@@ -22,7 +22,7 @@ def shard_templates(batch, rank, world):
 class Response:
     """One orbit table + (dt, order, TDI generation): owns an lr_handle."""
 
-    def __init__(self, table, dt, order=25, tdi_gen=2, t0=None, chain="nested", channels="XYZ"):
+    def __init__(self, table, dt, order=25, tdi_gen=2, t0=None, chain="nested", channels="XYZ", tdi_path="auto"):
         self._h = None
         self._h = B.lr_create(table, dt, order, tdi_gen)
         self.dt, self.order, self.tdi_gen = dt, order, tdi_gen
@@ -30,6 +30,8 @@ class Response:
             B.lr_set_option(self._h, B.LR_OPT_T0, t0)
         self.set_chain(chain)
         self.set_channels(channels)
+        if tdi_path != "auto":
+            self.set_tdi_path(tdi_path)
 
     @property
     def handle(self):
@@ -41,6 +43,11 @@ class Response:
     def set_channels(self, channels):
         B.lr_set_option(self._h, B.LR_OPT_CHANNELS, _CHANNELS[channels])
         self.n_out = 6 if channels == "XYZ_AET" else 3
+
+    def set_tdi_path(self, path):
+        """"auto" | "per_sample" | "fir3" | "fir4" (LR_OPT_TDI_PATH)."""
+        B.lr_set_option(self._h, B.LR_OPT_TDI_PATH, {"auto": B.LR_TDI_AUTO, "per_sample": B.LR_TDI_PER_SAMPLE,
+                                                     "fir3": B.LR_TDI_FIR3, "fir4": B.LR_TDI_FIR4}[path])
 
     def set_tdi_gen(self, gen):
         B.lr_set_option(self._h, B.LR_OPT_TDI_GEN, gen)

@@ -1,0 +1,69 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times.
+
+The oracle cannot run 3e6-2.5e7 samples in long double within a test, so each case runs the whole workload on
+the GPU and compares sampled windows (the first and last valid samples, plus seeded random windows) that the
+oracle computes one by one; outside the margins every output must be exactly 0.  Same bar as the reduced
+cases: 1e-10 per channel (parity_util).
+"""
+import numpy as np
+import pytest
+
+from paper_2204_06633_b200 import inputs
+from parity_util import windows
+from test_gpu_parity import check_workload, lr  # noqa: F401  (fixture)
+
+pytestmark = pytest.mark.gpu
+
+
+def _wins(w, lr_mod, count, width=384, seed=0, gen=None):
+    """Windows over the TDI-valid region (the projection is checked on the same windows)."""
+    R = lr_mod.Response(w.table(), w.dt, w.order, gen or w.tdi_gen, t0=w.t0)
+    mp, mf, mb = R.margins()
+    R.close()
+    return windows(mf, w.n - mb, width, count, seed)
+
+
+def test_full_size_config2_year(lr):  # noqa: F811
+    """configs[1]: 3,153,600 samples, one launch per stage, XYZ+AET, nested and eq. 20 sums."""
+    w = inputs.config(2)
+    assert w.n == 3153600
+    wins = _wins(w, lr, 8, seed=22)
+    check_workload(lr, w, wins=wins)
+    check_workload(lr, w, wins=wins[:3], chain="sum", proj=False)
+
+
+def test_full_size_config3_batch_chunk(lr):  # noqa: F811
+    """configs[2]: one chunk of 16 templates at the full 1,576,800 samples (the chunked launch bench.py
+    uses); the first, the last and one middle template of the chunk are compared on sampled windows."""
+    w = inputs.config(3, batch=16)
+    assert w.n == 1576800
+    wins = _wins(w, lr, 4, seed=33)
+    errs, yh, oh = check_workload(lr, w, idx=tuple(range(16)), wins=wins[:1], proj=True)
+    # templates differ: no two outputs may coincide (batch indexing)
+    assert not np.array_equal(oh[0], oh[15])
+    del errs, yh, oh
+
+
+def test_full_size_config3_sampled_templates(lr):  # noqa: F811
+    w = inputs.config(3, batch=16)
+    wins = _wins(w, lr, 4, seed=34)
+    w.sources = [w.sources[i] for i in (0, 7, 15)]
+    check_workload(lr, w, idx=(0, 1, 2), wins=wins)
+
+
+def test_full_size_config4_four_years(lr):  # noqa: F811
+    """configs[3]: 25,228,800 samples at dt = 5 s, order 41, perturbed orbits, TDI-2 XYZ (the maximum size of
+    the configs: 1.2 GB of y)."""
+    w = inputs.config(4)
+    assert w.n == 25228800
+    check_workload(lr, w, wins=_wins(w, lr, 6, width=256, seed=44))
+
+
+def test_full_size_config5_chirp(lr):  # noqa: F811
+    """configs[4]: 1,555,200 samples, full TDI-2 and the hybrid mode (TDI-1 on equal-arm constant delays)."""
+    w = inputs.config(5)
+    assert w.n == 1555200
+    wins = _wins(w, lr, 6, seed=55)
+    check_workload(lr, w, wins=wins)
+    eq = inputs.orbit_table("eq", w.t0, w.t0 + w.n * w.dt, const_ltt=inputs.ARM / inputs.C_LIGHT)
+    check_workload(lr, w, tdi_tab=eq, tdi_gen=1, proj=False, wins=_wins(w, lr, 4, seed=56, gen=1))

@@ -33,7 +33,7 @@ def _stack(w, idx):
 
 
 def check_workload(lr, w, *, chain="nested", channels=None, gen=None, idx=(0,), wins=None, tab=None,
-                   tdi_tab=None, tdi_gen=None, proj=True):
+                   tdi_tab=None, tdi_gen=None, proj=True, tdi_path="auto"):
     """Run w's templates `idx` through lr_project and lr_tdi and compare with the oracle.
     wins: list of (lo, hi) sample windows to compare on (None = the whole valid region)."""
     import torch
@@ -66,6 +66,7 @@ def check_workload(lr, w, *, chain="nested", channels=None, gen=None, idx=(0,), 
         g2 = tdi_gen or gen
         Rt = lr.Response(tdi_tab, w.dt, w.order, g2, t0=w.t0, chain=chain, channels=channels)
         Ot = orc.Oracle(tdi_tab, w.dt, w.t0, w.order)
+    Rt.set_tdi_path(tdi_path)
     out = Rt.tdi(y)
     torch.cuda.synchronize()
     oh = out.cpu().numpy()
@@ -87,21 +88,76 @@ def test_config1_tiny_full(lr):
 
 
 def test_config1_tiny_fixed_point_ltt(lr):
-    """Same with the flat-space fixed-point light times (L_ij != L_ji), nested and eq. 20 sums, gen 1 and 2."""
+    """Same with the flat-space fixed-point light times (L_ij != L_ji), nested and eq. 20 sums, gen 1 and 2,
+    every lr_tdi path.  (X, Y, Z here: with exactly equal arms T is a null channel, |T| = 3e-5 |A|, and its
+    relative error only measures that suppression; SURVEY.md §8(c) worked example.  A, E, T are covered on the
+    Keplerian configs.)"""
     w = inputs.config(1)
     tab = inputs.orbit_table("eq", w.t0, w.t0 + w.n * w.dt)
     for chain in ("nested", "sum"):
         for gen in (1, 2):
-            check_workload(lr, w, tab=tab, chain=chain, gen=gen, channels="XYZ_AET")
+            for path in ("per_sample", "fir3", "fir4"):
+                check_workload(lr, w, tab=tab, chain=chain, gen=gen, channels="XYZ", tdi_path=path,
+                               proj=(path == "per_sample"))
+
+
+def test_tdi_null_channel_absolute(lr):
+    """The same equal-arm case with A, E, T: the error of the null channel T is bounded relative to max|A|
+    (1e-10 of the live channels), for every path."""
+    w = inputs.config(1)
+    tab = inputs.orbit_table("eq", w.t0, w.t0 + w.n * w.dt)
+    O = orc.Oracle(tab, w.dt, w.t0, w.order)
+    s = w.sources[0]
+    hp, hc = w.waveform(0)
+    for path in ("per_sample", "fir3", "fir4"):
+        R = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="AET", tdi_path=path)
+        mp, mf, mb = R.margins()
+        y = R.project(to_dev(hp)[None], to_dev(hc)[None], [s.beta], [s.lam], [s.psi])
+        out = R.tdi(y).cpu().numpy()[0]
+        oo = O.tdi(y.cpu().numpy()[0], 2, nested=True, channels=orc.CH_AET)
+        v = slice(mf, w.n - mb)
+        assert_parity(out[:2, v], oo[:2, v], f"equal-arm A,E ({path})", ["A", "E"])
+        scale = float(np.abs(oo[0, v]).max())
+        assert float(np.abs(out[2, v] - oo[2, v].astype(np.float64)).max()) <= 1e-10 * scale
+
+
+def test_tdi_delay_crossing_whole_sample(lr):
+    """Degenerate case of the FIR path: light times that drift THROUGH a whole number of samples inside the
+    series (L = 10 s +- at dt = 10 s), so the integer part of several delays changes mid-tile; those tiles must
+    fall back to the exact per-sample weights.  Also L exactly constant = 1 sample (eps = 0 everywhere)."""
+    import torch
+    dt, n, t0, order = 10.0, 5000, 3.0e7, 25
+    base = inputs.orbit_table("kepler", t0, t0 + n * dt)
+    tk = base.t_start + base.knot_dt * np.arange(base.n_knots)
+    t_mid = t0 + 0.5 * n * dt
+    rng = np.random.default_rng(5)
+    t = t0 + dt * np.arange(n)
+    y = np.stack([np.sin(2 * np.pi * f * t + p) for f, p in zip(rng.uniform(1e-3, 2e-2, 6), rng.uniform(0, 6, 6))])
+    for ltt in (np.tile(10.0 + 2e-8 * (tk - t_mid), (6, 1)) * (1 + 1e-4 * np.arange(6))[:, None],
+                np.full((6, base.n_knots), 10.0)):
+        tab = inputs.OrbitTable(base.t_start, base.knot_dt, base.x, np.ascontiguousarray(ltt))
+        O = orc.Oracle(tab, dt, t0, order)
+        for gen in (1, 2):
+            oo = None
+            for path in ("per_sample", "fir3", "fir4"):
+                R = lr.Response(tab, dt, order, gen, t0=t0, tdi_path=path)
+                _, mf, mb = R.margins()
+                out = R.tdi(to_dev(y)[None]).cpu().numpy()[0]
+                torch.cuda.synchronize()
+                if oo is None:
+                    oo = O.tdi(y, gen, nested=True)
+                assert_parity(out[:, mf:n - mb], oo[:, mf:n - mb], f"crossing gen{gen} {path}", CH_NAMES["XYZ"])
 
 
 # ------------------------------------------------------------------------------------------- config 2
 @pytest.mark.parametrize("f0", [None, 1e-4, 1e-3, 1e-2])
 @pytest.mark.parametrize("chain", ["nested", "sum"])
-def test_config2_year_reduced(lr, f0, chain):
-    """configs[1] shortened to 20,011 samples (79 tiles, ragged tail): Keplerian, TDI-2, XYZ+AET; the seeded
-    source and the three fixed-frequency strata of SURVEY.md §8(c)."""
-    check_workload(lr, inputs.config(2, n=20011, f0=f0, t0=3.0e7), chain=chain)
+@pytest.mark.parametrize("tdi_path", ["auto", "per_sample", "fir3", "fir4"])
+def test_config2_year_reduced(lr, f0, chain, tdi_path):
+    """configs[1] shortened to 20,011 samples (79-90 tiles, ragged tail): Keplerian, TDI-2, XYZ+AET; the seeded
+    source and the three fixed-frequency strata of SURVEY.md §8(c); every lr_tdi path."""
+    check_workload(lr, inputs.config(2, n=20011, f0=f0, t0=3.0e7), chain=chain, tdi_path=tdi_path,
+                   proj=(tdi_path == "auto"))
 
 
 def test_config2_paper_sources(lr):
@@ -120,10 +176,11 @@ def test_config3_batch_reduced(lr):
 
 
 # ------------------------------------------------------------------------------------------- config 4
-def test_config4_numerical_orbits_reduced(lr):
+@pytest.mark.parametrize("tdi_path", ["auto", "per_sample", "fir4"])
+def test_config4_numerical_orbits_reduced(lr, tdi_path):
     """configs[3] shortened: perturbed-orbit tables (L_ij != L_ji), dt = 5 s, order 41, TDI-2 XYZ."""
-    check_workload(lr, inputs.config(4, n=12345, t0=5.0e7))
-    check_workload(lr, inputs.config(4, n=5000, t0=1.0e8, f0=1e-4), chain="sum")
+    check_workload(lr, inputs.config(4, n=12345, t0=5.0e7), tdi_path=tdi_path)
+    check_workload(lr, inputs.config(4, n=5000, t0=1.0e8, f0=1e-4), chain="sum", tdi_path=tdi_path)
 
 
 # ------------------------------------------------------------------------------------------- config 5
@@ -147,6 +204,7 @@ def test_orders(lr, order):
     w = inputs.config(2, n=3001, f0=2e-3, t0=2.0e7)
     w.order = order
     check_workload(lr, w, channels="XYZ")
+    check_workload(lr, w, channels="XYZ", tdi_path="per_sample", proj=False)
 
 
 # ---------------------------------------------------------------------------------------------- pins
