@@ -58,12 +58,18 @@ typedef struct {
 #define LR_OPT_CHANNELS 3 /* LR_XYZ (default) | LR_AET | LR_XYZ_AET */
 #define LR_OPT_TDI_GEN 4  /* 1 | 2: changes the generation given to lr_create */
 #define LR_OPT_TDI_PATH 5 /* LR_TDI_AUTO (default) | LR_TDI_PER_SAMPLE | LR_TDI_FIR3 | LR_TDI_FIR4 */
+#define LR_OPT_TDI_PLAN_CACHE 6 /* 1 (default): keep the FIR plan between lr_tdi calls; 0: rebuild every call */
 
 /* How lr_tdi evaluates the Lagrange weights (same result to rounding).
  *   LR_TDI_PER_SAMPLE : every delayed term gets its own weight set at every sample.
  *   LR_TDI_FIR3/4     : per tile of 224 samples the weights are a quadratic/cubic polynomial in time fitted
  *                       through 3/4 nodes, and all terms of a series merge into one short FIR filter; tiles
  *                       in which a delay crosses a whole number of samples use the per-sample code.
+ *                       The per-tile filters (the "plan") depend on the orbits and the time grid (n, t0, dt,
+ *                       generation, chain mode) only, not on y: one plan serves every template of a batch and,
+ *                       with LR_OPT_TDI_PLAN_CACHE = 1, every later call on the same grid (the paper keeps its
+ *                       orbit arrays on the device "for the entirety of the sampling run").  The
+ *                       plan costs 12*Wc*32 B per tile (about 60 B per sample at order 25) of device memory.
  *   LR_TDI_AUTO       : FIR3 / FIR4 / PER_SAMPLE by the largest light-time rate of the orbit table. */
 #define LR_TDI_AUTO (-1)
 #define LR_TDI_PER_SAMPLE 0

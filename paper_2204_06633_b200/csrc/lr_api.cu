@@ -34,6 +34,18 @@ struct Stage {
 
 }  // namespace
 
+// lr_tdi's FIR plan (lr_tdi_fir.cuh): a function of the orbits and the time grid only, kept between calls
+struct Plan {
+  double* coef = nullptr;
+  int* flags = nullptr;
+  size_t coef_cap = 0, flags_cap = 0;   // elements
+  bool valid = false;
+  int64_t n = 0;
+  double t0 = 0;
+  int gen = 0, chain = 0, path = 0;
+  cudaEvent_t ready = nullptr;
+};
+
 struct lr_handle {
   // configuration
   double dt = 0, t_start = 0, knot_dt = 0, t0 = 0;
@@ -42,6 +54,8 @@ struct lr_handle {
   double r_max = 0, l_max = 0;
   double max_ldot = 0;   // max |dL_ij/dt| over the table (dimensionless), from the spline
   int tdi_path = -1;     // LR_OPT_TDI_PATH: -1 auto | 0 generic | 3 | 4
+  int plan_cache = 1;    // LR_OPT_TDI_PLAN_CACHE
+  Plan plan;
   double bk[lr::kPMax + 1];
   // device state
   lr::D4* coef = nullptr;
@@ -199,6 +213,9 @@ void lr_destroy(lr_handle* h) {
     if (S.host) cudaFreeHost(S.host);
     if (S.dev) cudaFree(S.dev);
   }
+  if (h->plan.ready) cudaEventDestroy(h->plan.ready);
+  if (h->plan.coef) cudaFree(h->plan.coef);
+  if (h->plan.flags) cudaFree(h->plan.flags);
   if (h->scratch) cudaFree(h->scratch);
   if (h->coef) cudaFree(h->coef);
   delete h;
@@ -221,6 +238,9 @@ int lr_set_option(lr_handle* h, int key, double value) {
       if (value != LR_TDI_AUTO && value != LR_TDI_PER_SAMPLE && value != LR_TDI_FIR3 && value != LR_TDI_FIR4)
         return LR_EINVAL;
       h->tdi_path = (int)value; return LR_OK;
+    case LR_OPT_TDI_PLAN_CACHE:
+      if (value != 0 && value != 1) return LR_EINVAL;
+      h->plan_cache = (int)value; h->plan.valid = false; return LR_OK;
     default: return LR_EINVAL;
   }
 }
@@ -265,6 +285,8 @@ int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out,
   const double de = (double)nlinks * h->max_ldot * (double)lr::kFirTile;  // change of eps over one tile
   int path = h->tdi_path;
   if (path == LR_TDI_AUTO) path = de <= 6e-6 ? LR_TDI_FIR3 : de <= 1.5e-4 ? LR_TDI_FIR4 : LR_TDI_PER_SAMPLE;
+  cudaStream_t st = (cudaStream_t)stream;
+  lr::FirPlanArgs pa{nullptr, nullptr, false};
   if (path != LR_TDI_PER_SAMPLE) {
     const int imax = (int)h->tdi_reach(h->gen);
     const int wc = ((imax + 2 * h->p - 2 + lr::kFirR - 1) / lr::kFirR) * lr::kFirR;
@@ -273,18 +295,43 @@ int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out,
     P.halo_lo = back > (int)(mf - h->m_proj()) ? back : (int)(mf - h->m_proj());
     P.halo_hi = h->p + lr::kFirR;
     P.ntiles = (int)((n + lr::kFirTile - 1) / lr::kFirTile);
-    const int W = lr::kFirTile + P.halo_lo + P.halo_hi;
-    const size_t smem = path == LR_TDI_FIR3
-        ? (h->gen == 1 ? lr::FirSmem<1, 3>(W, wc, h->p).total : lr::FirSmem<2, 3>(W, wc, h->p).total)
-        : (h->gen == 1 ? lr::FirSmem<1, 4>(W, wc, h->p).total : lr::FirSmem<2, 4>(W, wc, h->p).total);
-    if (smem > 200 * 1024) path = LR_TDI_PER_SAMPLE;
+    const size_t W = (size_t)lr::kFirTile + P.halo_lo + P.halo_hi;
+    const size_t smem = (12 * W + lr::fir_plan_doubles_per_tile(wc) + 3 * (size_t)lr::kFirTile) * sizeof(double);
+    if (smem > 200 * 1024) path = LR_TDI_PER_SAMPLE;   // very long stencils: keep the per-sample kernel
   }
-  if (path == LR_TDI_PER_SAMPLE) {
+  if (path != LR_TDI_PER_SAMPLE) {
+    Plan& pl = h->plan;
+    const bool reuse = h->plan_cache && pl.valid && pl.n == n && pl.t0 == h->t0 && pl.gen == h->gen &&
+                       pl.chain == h->chain && pl.path == path;
+    if (!reuse) {
+      const size_t need = (size_t)P.ntiles * lr::fir_plan_doubles_per_tile(P.fir_wc);
+      pl.valid = false;
+      if (pl.coef_cap < need) {
+        if (pl.coef) { cudaFree(pl.coef); pl.coef = nullptr; pl.coef_cap = 0; }
+        LR_CUDA(h, cudaMalloc(&pl.coef, need * sizeof(double)));
+        pl.coef_cap = need;
+      }
+      if (pl.flags_cap < (size_t)P.ntiles) {
+        if (pl.flags) { cudaFree(pl.flags); pl.flags = nullptr; pl.flags_cap = 0; }
+        LR_CUDA(h, cudaMalloc(&pl.flags, (size_t)P.ntiles * sizeof(int)));
+        pl.flags_cap = (size_t)P.ntiles;
+      }
+      if (!pl.ready) LR_CUDA(h, cudaEventCreateWithFlags(&pl.ready, cudaEventDisableTiming));
+    } else {
+      LR_CUDA(h, cudaStreamWaitEvent(st, pl.ready, 0));   // the plan may have been built on another stream
+    }
+    pa.coef = pl.coef; pa.flags = pl.flags; pa.build = !reuse;
+  } else {
     P.halo_lo = (int)(mf - h->m_proj()); P.halo_hi = h->p + 2;
     P.ntiles = (int)((n + lr::kTdiThreads - 1) / lr::kTdiThreads);
   }
-  const int e = lr::launch_tdi(P, h->order, h->gen, path, h->channels, y, out, batch, stream);
+  const int e = lr::launch_tdi(P, h->order, h->gen, path, h->channels, y, out, batch, pa, stream);
   if (e != 0) { h->last_cuda = e; return LR_ECUDA; }
+  if (pa.build) {
+    Plan& pl = h->plan;
+    LR_CUDA(h, cudaEventRecord(pl.ready, st));
+    pl.valid = true; pl.n = n; pl.t0 = h->t0; pl.gen = h->gen; pl.chain = h->chain; pl.path = path;
+  }
   return LR_OK;
 }
 

@@ -46,35 +46,49 @@ static int launch_tdi_generic(const Params& prm, int channels, const double* y, 
   return (int)cudaGetLastError();
 }
 
+// FIR path: (re)build the plan if asked, then apply it
 template <int PT, int GEN, int NN>
 static int launch_tdi_fir(const Params& prm, int channels, const double* y, double* out, int64_t batch,
-                          cudaStream_t st) {
-  const int W = kFirTile + prm.halo_lo + prm.halo_hi;
-  const FirSmem<GEN, NN> plan(W, prm.fir_wc, PT > 0 ? PT : prm.p);
-  cudaError_t e = prepare(tdi_fir_kernel<PT, GEN, NN>, plan.total);
+                          const FirPlanArgs& plan, cudaStream_t st) {
+  const int P = PT > 0 ? PT : prm.p;
+  if (plan.build) {
+    const size_t smem = ((sizeof(FirTile<GEN, NN>) + 15) / 16) * 16 +
+                        (size_t)FirTile<GEN, NN>::NT * NN * (2 * P - 1) * sizeof(double);
+    cudaError_t e = prepare(tdi_fir_setup_kernel<PT, GEN, NN>, smem);
+    if (e != cudaSuccess) return (int)e;
+    tdi_fir_setup_kernel<PT, GEN, NN><<<(unsigned)prm.ntiles, kFirSetupThreads, smem, st>>>(prm, plan.coef, plan.flags);
+    g_launches.fetch_add(1);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return (int)e;
+  }
+  const size_t W = (size_t)kFirTile + prm.halo_lo + prm.halo_hi;
+  const size_t smem = (12 * W + fir_plan_doubles_per_tile(prm.fir_wc) + 3 * (size_t)kFirTile) * sizeof(double);
+  cudaError_t e = prepare(tdi_fir_apply_kernel<PT, GEN, NN>, smem);
   if (e != cudaSuccess) return (int)e;
   const int64_t grid = (int64_t)prm.ntiles * batch;
-  tdi_fir_kernel<PT, GEN, NN><<<(unsigned)grid, kFirThreads, plan.total, st>>>(prm, y, out, channels);
+  tdi_fir_apply_kernel<PT, GEN, NN><<<(unsigned)grid, kFirThreads, smem, st>>>(prm, y, out, channels, plan.coef,
+                                                                               plan.flags, (int)batch);
   g_launches.fetch_add(1);
   return (int)cudaGetLastError();
 }
 
 template <int PT>
 int launch_tdi_t(const Params& prm, int gen, int path, int channels, const double* y, double* out, int64_t batch,
-                 void* stream) {
+                 const FirPlanArgs& plan, void* stream) {
   cudaStream_t st = (cudaStream_t)stream;
   if (path == kPathFir3)
-    return gen == 1 ? launch_tdi_fir<PT, 1, 3>(prm, channels, y, out, batch, st)
-                    : launch_tdi_fir<PT, 2, 3>(prm, channels, y, out, batch, st);
+    return gen == 1 ? launch_tdi_fir<PT, 1, 3>(prm, channels, y, out, batch, plan, st)
+                    : launch_tdi_fir<PT, 2, 3>(prm, channels, y, out, batch, plan, st);
   if (path == kPathFir4)
-    return gen == 1 ? launch_tdi_fir<PT, 1, 4>(prm, channels, y, out, batch, st)
-                    : launch_tdi_fir<PT, 2, 4>(prm, channels, y, out, batch, st);
+    return gen == 1 ? launch_tdi_fir<PT, 1, 4>(prm, channels, y, out, batch, plan, st)
+                    : launch_tdi_fir<PT, 2, 4>(prm, channels, y, out, batch, plan, st);
   return gen == 1 ? launch_tdi_generic<PT, 1>(prm, channels, y, out, batch, st)
                   : launch_tdi_generic<PT, 2>(prm, channels, y, out, batch, st);
 }
 
 template int launch_project_t<LR_INST_PT>(const Params&, const double*, const double*, const double*, double*,
                                           int64_t, void*);
-template int launch_tdi_t<LR_INST_PT>(const Params&, int, int, int, const double*, double*, int64_t, void*);
+template int launch_tdi_t<LR_INST_PT>(const Params&, int, int, int, const double*, double*, int64_t,
+                                      const FirPlanArgs&, void*);
 
 }  // namespace lr

@@ -34,16 +34,16 @@ int launch_project(const Params& prm, int order, const double* hp, const double*
 }
 
 int launch_tdi(const Params& prm, int order, int gen, int path, int channels, const double* y, double* out,
-               int64_t batch, void* stream) {
+               int64_t batch, const FirPlanArgs& plan, void* stream) {
   switch (order) {
 #ifndef LR_DEV_ONLY_P13
-    case 1: return launch_tdi_t<1>(prm, gen, path, channels, y, out, batch, stream);
-    case 3: return launch_tdi_t<2>(prm, gen, path, channels, y, out, batch, stream);
-    case 9: return launch_tdi_t<5>(prm, gen, path, channels, y, out, batch, stream);
-    case 41: return launch_tdi_t<21>(prm, gen, path, channels, y, out, batch, stream);
+    case 1: return launch_tdi_t<1>(prm, gen, path, channels, y, out, batch, plan, stream);
+    case 3: return launch_tdi_t<2>(prm, gen, path, channels, y, out, batch, plan, stream);
+    case 9: return launch_tdi_t<5>(prm, gen, path, channels, y, out, batch, plan, stream);
+    case 41: return launch_tdi_t<21>(prm, gen, path, channels, y, out, batch, plan, stream);
 #endif
-    case 25: return launch_tdi_t<13>(prm, gen, path, channels, y, out, batch, stream);
-    default: return launch_tdi_t<0>(prm, gen, path, channels, y, out, batch, stream);
+    case 25: return launch_tdi_t<13>(prm, gen, path, channels, y, out, batch, plan, stream);
+    default: return launch_tdi_t<0>(prm, gen, path, channels, y, out, batch, plan, stream);
   }
 }
 

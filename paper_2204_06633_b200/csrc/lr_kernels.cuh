@@ -2,6 +2,7 @@
 //
 //   project_kernel<PT>       : PAPER.md eqs. 10-16, one thread per time sample, all six links
 //   tdi_kernel<PT,GEN>       : PAPER.md eqs. 17-21, one thread per time sample, X, Y, Z (+ A, E, T)
+//   (lr_tdi_fir.cuh holds the fast TDI path: tdi_fir_setup_kernel + tdi_fir_apply_kernel)
 //
 // Both stage the window a tile of samples needs (raw samples and their exact first differences) in
 // shared memory with coalesced loads, keep the Lagrange pair products in registers, and write coalesced
@@ -131,6 +132,13 @@ constexpr int kPathGeneric = 0;  // tdi_kernel: exact per-sample weights
 constexpr int kPathFir3 = 3;     // tdi_fir_kernel, quadratic in tile time
 constexpr int kPathFir4 = 4;     // tdi_fir_kernel, cubic in tile time
 
+// FIR plan buffers (owned by the handle) and whether this launch must (re)build them
+struct FirPlanArgs {
+  double* coef;   // DEVICE [ntiles][12][Wc][kFirKStride]
+  int* flags;     // DEVICE [ntiles]
+  bool build;
+};
+
 // small helper kernel: spline channel at arbitrary absolute times (lr_eval_orbit)
 __global__ void eval_orbit_kernel(const Params prm, int ch, double t_start, const double* __restrict__ t,
                                   int64_t m, double* __restrict__ out);
@@ -142,12 +150,12 @@ int launch_project_t(const Params& prm, const double* hp, const double* hc, cons
                      int64_t batch, void* stream);
 template <int PT>
 int launch_tdi_t(const Params& prm, int gen, int path, int channels, const double* y, double* out, int64_t batch,
-                 void* stream);
+                 const FirPlanArgs& plan, void* stream);
 
 // dispatch on the Lagrange order (lr_kernels.cu)
 int launch_project(const Params& prm, int order, const double* hp, const double* hc, const double* basis,
                    double* y, int64_t batch, void* stream);
 int launch_tdi(const Params& prm, int order, int gen, int path, int channels, const double* y, double* out,
-               int64_t batch, void* stream);
+               int64_t batch, const FirPlanArgs& plan, void* stream);
 
 }  // namespace lr

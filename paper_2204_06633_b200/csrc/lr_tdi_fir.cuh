@@ -258,53 +258,67 @@ LR_HD void fir_apply(const double* dif, int W, const double* K, int Wc, int P, i
   }
 }
 
-}  // namespace lr
-
-#ifdef __CUDACC__
-namespace lr {
-
 constexpr int kFirGroups = 32;                    // groups of kFirR samples per channel and tile
 constexpr int kFirTile = kFirGroups * kFirR;      // 224 samples per tile
-constexpr int kFirThreads = 3 * kFirGroups;       // one warp per channel
+constexpr int kFirThreads = 3 * kFirGroups;       // apply kernel: one warp per channel
+constexpr int kFirSetupThreads = 128;
 
-// shared-memory plan of tdi_fir_kernel (bytes), used by the launcher too
-template <int GEN, int NN>
-struct FirSmem {
-  size_t raw, dif, tile, cnode, K, total;
-  __host__ __device__ FirSmem(int W, int Wc, int P) {
-    const size_t nt = FirTile<GEN, NN>::NT;
-    raw = 0;
-    dif = raw + (size_t)6 * W * sizeof(double);
-    tile = dif + (size_t)6 * W * sizeof(double);
-    cnode = tile + ((sizeof(FirTile<GEN, NN>) + 15) / 16) * 16;
-    size_t cn = nt * NN * (size_t)(2 * P - 1) * sizeof(double);
-    const size_t rs = (size_t)3 * kFirTile * sizeof(double);   // res aliases cnode
-    if (cn < rs) cn = rs;
-    K = cnode + ((cn + 15) / 16) * 16;
-    total = K + (size_t)12 * Wc * kFirKStride * sizeof(double);
+// The plan of one tile in global memory: K[12][Wc][kFirKStride] doubles; flags[tile] != 0 marks a tile that
+// must run the exact per-sample code.  The plan depends on the orbits and the time grid only (not on y), so
+// one plan serves every template of a batch and every later lr_tdi call on the same grid.
+LR_HD size_t fir_plan_doubles_per_tile(int Wc) { return (size_t)12 * Wc * kFirKStride; }
+
+#ifdef __CUDACC__
+// ------------------------------------------------------------------------------------------ plan kernel
+// grid.x = ntiles; dynamic smem: FirTile + cnode[NT][NN][2P-1]
+template <int PT, int GEN, int NN>
+__global__ void __launch_bounds__(kFirSetupThreads)
+tdi_fir_setup_kernel(const Params prm, double* __restrict__ plan, int* __restrict__ flags) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int B = kFirTile;
+  FirTile<GEN, NN>& T = *reinterpret_cast<FirTile<GEN, NN>*>(smem_raw);
+  double* cnode = reinterpret_cast<double*>(smem_raw + ((sizeof(FirTile<GEN, NN>) + 15) / 16) * 16);
+  const int tid = threadIdx.x;
+  const int tile = blockIdx.x;
+  const int n0 = tile * B;
+  const int Wc = prm.fir_wc;
+  if (n0 + B <= prm.m_front || n0 >= prm.n - prm.m_back) {   // tile entirely inside a margin: never applied
+    if (tid == 0) flags[tile] = 0;
+    return;
   }
-};
+  if (tid == 0) T.generic = 0;
+  fir_chain_nodes<GEN, NN>(prm, T, n0, B, tid, kFirSetupThreads);
+  __syncthreads();
+  fir_split_terms<GEN, NN>(prm, T, tid, kFirSetupThreads);
+  __syncthreads();
+  if (tid == 0) flags[tile] = T.generic;
+  if (T.generic) return;
+  fir_node_coeffs<PT, GEN, NN>(prm, T, cnode, tid, kFirSetupThreads);
+  __syncthreads();
+  fir_merge<PT, GEN, NN>(prm, T, cnode, plan + (size_t)tile * fir_plan_doubles_per_tile(Wc), Wc, tid,
+                         kFirSetupThreads);
+}
 
-// grid.x = ntiles * batch (tiles of kFirTile samples).  prm.halo_lo/hi describe the staged window.
+// ----------------------------------------------------------------------------------------- apply kernel
+// grid.x = ntiles * batch, template index fastest (the tiles of one time span share their plan through L2).
+// dynamic smem: raw[6][W], dif[6][W], K[12][Wc][4], res[3][B]
 template <int PT, int GEN, int NN>
 __global__ void __launch_bounds__(kFirThreads)
-tdi_fir_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ out, int channels) {
+tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ out, int channels,
+                     const double* __restrict__ plan, const int* __restrict__ flags, int batch) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int B = kFirTile;
   const int P = PT > 0 ? PT : prm.p;
   const int W = B + prm.halo_lo + prm.halo_hi;
   const int Wc = prm.fir_wc;
-  const FirSmem<GEN, NN> plan(W, Wc, P);
-  double* raw = reinterpret_cast<double*>(smem_raw + plan.raw);
-  double* dif = reinterpret_cast<double*>(smem_raw + plan.dif);
-  FirTile<GEN, NN>& T = *reinterpret_cast<FirTile<GEN, NN>*>(smem_raw + plan.tile);
-  double* cnode = reinterpret_cast<double*>(smem_raw + plan.cnode);
-  double* res = cnode;
-  double* K = reinterpret_cast<double*>(smem_raw + plan.K);
+  double* raw = reinterpret_cast<double*>(smem_raw);
+  double* dif = raw + 6 * W;
+  double* K = dif + 6 * W;
+  double* res = K + fir_plan_doubles_per_tile(Wc);
 
   const int tid = threadIdx.x;
-  const int tile = blockIdx.x % prm.ntiles;
-  const int64_t b = blockIdx.x / prm.ntiles;
+  const int tile = blockIdx.x / batch;
+  const int64_t b = blockIdx.x - (int64_t)tile * batch;
   const int n0 = tile * B;
   const int g0 = n0 - prm.halo_lo;
   const int64_t N = prm.n;
@@ -318,24 +332,27 @@ tdi_fir_kernel(const Params prm, const double* __restrict__ y, double* __restric
         for (int c = 0; c < nout; ++c) ob[(int64_t)c * N + n0 + i] = 0.0;
     return;
   }
+  const bool generic = flags[tile] != 0;
 
   const double* yb = y + b * 6 * N;
   for (int m = tid; m < 6 * W; m += kFirThreads) {
     const int s = m / W, g = g0 + (m - s * W);
     raw[m] = (g >= 0 && g < prm.n) ? __ldg(yb + (int64_t)s * N + g) : 0.0;
   }
-  if (tid == 0) T.generic = 0;
+  if (!generic) {
+    const double2* src = reinterpret_cast<const double2*>(plan + (size_t)tile * fir_plan_doubles_per_tile(Wc));
+    double2* dst = reinterpret_cast<double2*>(K);
+    const int cnt = (int)(fir_plan_doubles_per_tile(Wc) / 2);
+    for (int m = tid; m < cnt; m += kFirThreads) dst[m] = __ldg(src + m);
+  }
   __syncthreads();
   for (int m = tid; m < 6 * W; m += kFirThreads) {
     const int w = m % W;
     dif[m] = (w < W - 1) ? raw[m + 1] - raw[m] : 0.0;
   }
-  fir_chain_nodes<GEN, NN>(prm, T, n0, B, tid, kFirThreads);
-  __syncthreads();
-  fir_split_terms<GEN, NN>(prm, T, tid, kFirThreads);
   __syncthreads();
   const int nl0 = prm.halo_lo;
-  if (T.generic) {
+  if (generic) {
     // exact per-sample path: a delay's integer part may change inside this tile
     for (int i = tid; i < B; i += kFirThreads) {
       const int n = n0 + i;
@@ -344,10 +361,6 @@ tdi_fir_kernel(const Params prm, const double* __restrict__ y, double* __restric
       res[i] = xyz[0]; res[B + i] = xyz[1]; res[2 * B + i] = xyz[2];
     }
   } else {
-    fir_node_coeffs<PT, GEN, NN>(prm, T, cnode, tid, kFirThreads);
-    __syncthreads();
-    fir_merge<PT, GEN, NN>(prm, T, cnode, K, Wc, tid, kFirThreads);
-    __syncthreads();
     fir_apply<NN>(dif, W, K, Wc, P, nl0, B, res, tid, kFirThreads);
   }
   __syncthreads();
@@ -365,6 +378,6 @@ tdi_fir_kernel(const Params prm, const double* __restrict__ y, double* __restric
     }
   }
 }
+#endif
 
 }  // namespace lr
-#endif

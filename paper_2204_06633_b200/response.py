@@ -49,6 +49,9 @@ class Response:
         B.lr_set_option(self._h, B.LR_OPT_TDI_PATH, {"auto": B.LR_TDI_AUTO, "per_sample": B.LR_TDI_PER_SAMPLE,
                                                      "fir3": B.LR_TDI_FIR3, "fir4": B.LR_TDI_FIR4}[path])
 
+    def set_plan_cache(self, on):
+        B.lr_set_option(self._h, B.LR_OPT_TDI_PLAN_CACHE, 1 if on else 0)
+
     def set_tdi_gen(self, gen):
         B.lr_set_option(self._h, B.LR_OPT_TDI_GEN, gen)
         self.tdi_gen = gen

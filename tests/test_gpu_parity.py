@@ -307,6 +307,34 @@ def test_gpu_orbit_spline_matches_oracle(lr):
         assert np.abs(g - sp).max() < 1e-13 * scale, ch
 
 
+def test_tdi_plan_cache(lr):
+    """The FIR plan is a function of the orbits and the time grid only: with the cache on, a second call with
+    another y, a call after a change of t0 / n / chain mode, and a cache-off call all give bit-identical
+    results to a fresh handle."""
+    w = inputs.config(2, n=6007, f0=3e-3, t0=3.0e7)
+    tab = w.table()
+    rng = np.random.default_rng(11)
+
+    def fresh(y, n, t0, chain):
+        R = lr.Response(tab, w.dt, w.order, 2, t0=t0, chain=chain, tdi_path="fir3")
+        R.set_plan_cache(False)
+        return R.tdi(to_dev(y[:, :n])[None]).cpu().numpy()
+
+    ya, yb = (np.cumsum(rng.normal(size=(6, w.n)), axis=1) * 1e-3 for _ in range(2))
+    R = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, tdi_path="fir3")
+    assert np.array_equal(R.tdi(to_dev(ya)[None]).cpu().numpy(), fresh(ya, w.n, w.t0, "nested"))
+    assert np.array_equal(R.tdi(to_dev(yb)[None]).cpu().numpy(), fresh(yb, w.n, w.t0, "nested"))   # plan reused
+    R.set_chain("sum")
+    assert np.array_equal(R.tdi(to_dev(yb)[None]).cpu().numpy(), fresh(yb, w.n, w.t0, "sum"))
+    R.set_chain("nested")
+    lr.lr_set_option(R.handle, lr.LR_OPT_T0, w.t0 + 12345.0)
+    assert np.array_equal(R.tdi(to_dev(ya)[None]).cpu().numpy(), fresh(ya, w.n, w.t0 + 12345.0, "nested"))
+    assert np.array_equal(R.tdi(to_dev(ya[:, :5000].copy())[None]).cpu().numpy(), fresh(ya, 5000, w.t0 + 12345.0, "nested"))
+    # one plan, several templates in one launch
+    both = R.tdi(to_dev(np.stack([ya[:, :5000], yb[:, :5000]]))).cpu().numpy()
+    assert np.array_equal(both[1:], fresh(yb, 5000, w.t0 + 12345.0, "nested"))
+
+
 # ---------------------------------------------------------------------------------------- edge cases
 def test_edge_cases_and_errors(lr):
     import torch
