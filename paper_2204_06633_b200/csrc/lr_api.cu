@@ -37,7 +37,7 @@ struct Stage {
 // lr_tdi's FIR plan (lr_tdi_fir.cuh): a function of the orbits and the time grid only, kept between calls
 struct Plan {
   double* coef = nullptr;
-  int* flags = nullptr;
+  int* flags = nullptr;                 // [2 * ntiles + 1]: flags, then count + list of flagged tiles
   size_t coef_cap = 0, flags_cap = 0;   // elements
   bool valid = false;
   int64_t n = 0;
@@ -55,6 +55,7 @@ struct lr_handle {
   double max_ldot = 0;   // max |dL_ij/dt| over the table (dimensionless), from the spline
   int tdi_path = -1;     // LR_OPT_TDI_PATH: -1 auto | 0 generic | 3 | 4
   int plan_cache = 1;    // LR_OPT_TDI_PLAN_CACHE
+  int sm_count = 0;
   Plan plan;
   double bk[lr::kPMax + 1];
   // device state
@@ -286,7 +287,7 @@ int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out,
   int path = h->tdi_path;
   if (path == LR_TDI_AUTO) path = de <= 6e-6 ? LR_TDI_FIR3 : de <= 1.5e-4 ? LR_TDI_FIR4 : LR_TDI_PER_SAMPLE;
   cudaStream_t st = (cudaStream_t)stream;
-  lr::FirPlanArgs pa{nullptr, nullptr, false};
+  lr::FirPlanArgs pa{nullptr, nullptr, nullptr, 0, false};
   if (path != LR_TDI_PER_SAMPLE) {
     const int imax = (int)h->tdi_reach(h->gen);
     const int wc = ((imax + 2 * h->p - 2 + lr::kFirR - 1) / lr::kFirR) * lr::kFirR;
@@ -295,8 +296,7 @@ int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out,
     P.halo_lo = back > (int)(mf - h->m_proj()) ? back : (int)(mf - h->m_proj());
     P.halo_hi = h->p + lr::kFirR;
     P.ntiles = (int)((n + lr::kFirTile - 1) / lr::kFirTile);
-    const size_t W = (size_t)lr::kFirTile + P.halo_lo + P.halo_hi;
-    const size_t smem = (12 * W + lr::fir_plan_doubles_per_tile(wc) + 3 * (size_t)lr::kFirTile) * sizeof(double);
+    const size_t smem = lr::fir_apply_smem_bytes(lr::kFirTile + P.halo_lo + P.halo_hi, wc);
     if (smem > 200 * 1024) path = LR_TDI_PER_SAMPLE;   // very long stencils: keep the per-sample kernel
   }
   if (path != LR_TDI_PER_SAMPLE) {
@@ -313,14 +313,20 @@ int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out,
       }
       if (pl.flags_cap < (size_t)P.ntiles) {
         if (pl.flags) { cudaFree(pl.flags); pl.flags = nullptr; pl.flags_cap = 0; }
-        LR_CUDA(h, cudaMalloc(&pl.flags, (size_t)P.ntiles * sizeof(int)));
+        LR_CUDA(h, cudaMalloc(&pl.flags, (2 * (size_t)P.ntiles + 1) * sizeof(int)));
         pl.flags_cap = (size_t)P.ntiles;
       }
       if (!pl.ready) LR_CUDA(h, cudaEventCreateWithFlags(&pl.ready, cudaEventDisableTiming));
     } else {
       LR_CUDA(h, cudaStreamWaitEvent(st, pl.ready, 0));   // the plan may have been built on another stream
     }
-    pa.coef = pl.coef; pa.flags = pl.flags; pa.build = !reuse;
+    pa.coef = pl.coef; pa.flags = pl.flags; pa.list = pl.flags + P.ntiles; pa.build = !reuse;
+    if (h->sm_count == 0) {
+      int dev = 0;
+      LR_CUDA(h, cudaGetDevice(&dev));
+      LR_CUDA(h, cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev));
+    }
+    pa.fixup_grid = 2 * h->sm_count;
   } else {
     P.halo_lo = (int)(mf - h->m_proj()); P.halo_hi = h->p + 2;
     P.ntiles = (int)((n + lr::kTdiThreads - 1) / lr::kTdiThreads);

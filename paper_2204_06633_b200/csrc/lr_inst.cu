@@ -46,28 +46,34 @@ static int launch_tdi_generic(const Params& prm, int channels, const double* y, 
   return (int)cudaGetLastError();
 }
 
-// FIR path: (re)build the plan if asked, then apply it
+// FIR path: (re)build the plan if asked, apply it, then run the flagged tiles with per-sample weights
 template <int PT, int GEN, int NN>
 static int launch_tdi_fir(const Params& prm, int channels, const double* y, double* out, int64_t batch,
                           const FirPlanArgs& plan, cudaStream_t st) {
   const int P = PT > 0 ? PT : prm.p;
+  cudaError_t e;
   if (plan.build) {
     const size_t smem = ((sizeof(FirTile<GEN, NN>) + 15) / 16) * 16 +
                         (size_t)FirTile<GEN, NN>::NT * NN * (2 * P - 1) * sizeof(double);
-    cudaError_t e = prepare(tdi_fir_setup_kernel<PT, GEN, NN>, smem);
-    if (e != cudaSuccess) return (int)e;
-    tdi_fir_setup_kernel<PT, GEN, NN><<<(unsigned)prm.ntiles, kFirSetupThreads, smem, st>>>(prm, plan.coef, plan.flags);
+    if ((e = prepare(tdi_fir_setup_kernel<PT, GEN, NN>, smem)) != cudaSuccess) return (int)e;
+    if ((e = cudaMemsetAsync(plan.list, 0, sizeof(int), st)) != cudaSuccess) return (int)e;
+    tdi_fir_setup_kernel<PT, GEN, NN><<<(unsigned)prm.ntiles, kFirSetupThreads, smem, st>>>(prm, plan.coef, plan.flags,
+                                                                                        plan.list);
     g_launches.fetch_add(1);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return (int)e;
+    if ((e = cudaGetLastError()) != cudaSuccess) return (int)e;
   }
-  const size_t W = (size_t)kFirTile + prm.halo_lo + prm.halo_hi;
-  const size_t smem = (12 * W + fir_plan_doubles_per_tile(prm.fir_wc) + 3 * (size_t)kFirTile) * sizeof(double);
-  cudaError_t e = prepare(tdi_fir_apply_kernel<PT, GEN, NN>, smem);
-  if (e != cudaSuccess) return (int)e;
+  const int W = kFirTile + prm.halo_lo + prm.halo_hi;
+  const size_t smem = fir_apply_smem_bytes(W, prm.fir_wc);
+  if ((e = prepare(tdi_fir_apply_kernel<NN>, smem)) != cudaSuccess) return (int)e;
   const int64_t grid = (int64_t)prm.ntiles * batch;
-  tdi_fir_apply_kernel<PT, GEN, NN><<<(unsigned)grid, kFirThreads, smem, st>>>(prm, y, out, channels, plan.coef,
-                                                                               plan.flags, (int)batch);
+  tdi_fir_apply_kernel<NN><<<(unsigned)grid, kFirThreads, smem, st>>>(prm, y, out, channels, plan.coef, plan.flags,
+                                                                    (int)batch);
+  g_launches.fetch_add(1);
+  if ((e = cudaGetLastError()) != cudaSuccess) return (int)e;
+  const size_t smem_fix = (size_t)12 * W * sizeof(double);
+  if ((e = prepare(tdi_fir_fixup_kernel<PT, GEN>, smem_fix)) != cudaSuccess) return (int)e;
+  tdi_fir_fixup_kernel<PT, GEN><<<plan.fixup_grid, kFirTile, smem_fix, st>>>(prm, y, out, channels, plan.list,
+                                                                             (int)batch);
   g_launches.fetch_add(1);
   return (int)cudaGetLastError();
 }

@@ -135,7 +135,9 @@ constexpr int kPathFir4 = 4;     // tdi_fir_kernel, cubic in tile time
 // FIR plan buffers (owned by the handle) and whether this launch must (re)build them
 struct FirPlanArgs {
   double* coef;   // DEVICE [ntiles][12][Wc][kFirKStride]
-  int* flags;     // DEVICE [ntiles]
+  int* flags;     // DEVICE [ntiles]: != 0 marks a tile that needs per-sample weights
+  int* list;      // DEVICE [1 + ntiles]: count, then the flagged tiles
+  int fixup_grid; // CTAs of the fix-up kernel (2 per SM)
   bool build;
 };
 

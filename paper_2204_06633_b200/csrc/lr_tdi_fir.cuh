@@ -204,20 +204,21 @@ LR_HD void fir_merge(const Params& prm, const FirTile<GEN, NN>& T, const double*
 
 // E: apply.  One work item = kFirR consecutive samples of one channel.  dif: [6][W]; res: [3][B] (tile
 // staging of X, Y, Z).  nl0 = staged index of the tile's first sample; Wc is a multiple of kFirR.
+// Per tap the coefficient is evaluated at each sample's own tau (Horner over the NN powers) and applied to
+// the sliding window of first differences: NN FMAs per (tap, sample), one accumulator per sample.
 template <int NN>
 LR_HD void fir_apply(const double* dif, int W, const double* K, int Wc, int P, int nl0, int B, double* res,
                      int tid, int nthreads) {
   constexpr int R = kFirR;
   const int groups = (B + R - 1) / R;
   const int back = Wc - (P - 1);
+  const double half = 0.5 * (double)(B - 1), inv_half = 1.0 / half;
   for (int w = tid; w < 3 * groups; w += nthreads) {
     const int ch = w / groups, g = w - ch * groups;
     const int i0 = g * R;                                  // first sample of the group inside the tile
-    double acc[NN][R];
+    double acc[R], tau[R];
 #pragma unroll
-    for (int p = 0; p < NN; ++p)
-#pragma unroll
-      for (int r = 0; r < R; ++r) acc[p][r] = 0.0;
+    for (int r = 0; r < R; ++r) { acc[r] = 0.0; tau[r] = ((double)(i0 + r) - half) * inv_half; }
 #pragma unroll 1
     for (int sl = 0; sl < 4; ++sl) {
       const double* d = dif + rot_slot_rt(fir_base_slot(sl), ch) * W + (nl0 + i0 - back);
@@ -235,26 +236,20 @@ LR_HD void fir_apply(const double* dif, int W, const double* K, int Wc, int P, i
 #pragma unroll
           for (int p = 0; p < NN; ++p) kc[p] = kk[(m0 + mm) * kFirKStride + p];
 #pragma unroll
-          for (int r = 0; r < R; ++r)
+          for (int r = 0; r < R; ++r) {
+            double c = kc[NN - 1];
 #pragma unroll
-            for (int p = 0; p < NN; ++p) acc[p][r] = fma(kc[p], win[mm + r], acc[p][r]);
+            for (int p = NN - 2; p >= 0; --p) c = fma(c, tau[r], kc[p]);
+            acc[r] = fma(c, win[mm + r], acc[r]);
+          }
         }
 #pragma unroll
         for (int r = 0; r < R; ++r) win[r] = win[R + r];
       }
     }
-    const double half = 0.5 * (double)(B - 1);
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-      const int i = i0 + r;
-      if (i < B) {
-        const double tau = ((double)i - half) / half;
-        double v = acc[NN - 1][r];
-#pragma unroll
-        for (int p = NN - 2; p >= 0; --p) v = fma(v, tau, acc[p][r]);
-        res[ch * B + i] = v;
-      }
-    }
+    for (int r = 0; r < R; ++r)
+      if (i0 + r < B) res[ch * B + i0 + r] = acc[r];
   }
 }
 
@@ -273,7 +268,8 @@ LR_HD size_t fir_plan_doubles_per_tile(int Wc) { return (size_t)12 * Wc * kFirKS
 // grid.x = ntiles; dynamic smem: FirTile + cnode[NT][NN][2P-1]
 template <int PT, int GEN, int NN>
 __global__ void __launch_bounds__(kFirSetupThreads)
-tdi_fir_setup_kernel(const Params prm, double* __restrict__ plan, int* __restrict__ flags) {
+tdi_fir_setup_kernel(const Params prm, double* __restrict__ plan, int* __restrict__ flags,
+                     int* __restrict__ list /* [0] = count, [1..] = flagged tiles */) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int B = kFirTile;
   FirTile<GEN, NN>& T = *reinterpret_cast<FirTile<GEN, NN>*>(smem_raw);
@@ -291,7 +287,10 @@ tdi_fir_setup_kernel(const Params prm, double* __restrict__ plan, int* __restric
   __syncthreads();
   fir_split_terms<GEN, NN>(prm, T, tid, kFirSetupThreads);
   __syncthreads();
-  if (tid == 0) flags[tile] = T.generic;
+  if (tid == 0) {
+    flags[tile] = T.generic;
+    if (T.generic) list[1 + atomicAdd(list, 1)] = tile;
+  }
   if (T.generic) return;
   fir_node_coeffs<PT, GEN, NN>(prm, T, cnode, tid, kFirSetupThreads);
   __syncthreads();
@@ -301,18 +300,32 @@ tdi_fir_setup_kernel(const Params prm, double* __restrict__ plan, int* __restric
 
 // ----------------------------------------------------------------------------------------- apply kernel
 // grid.x = ntiles * batch, template index fastest (the tiles of one time span share their plan through L2).
-// dynamic smem: raw[6][W], dif[6][W], K[12][Wc][4], res[3][B]
-template <int PT, int GEN, int NN>
-__global__ void __launch_bounds__(kFirThreads)
+// Tiles flagged by the plan are left to tdi_fir_fixup_kernel.
+// dynamic smem: dif[6][W] | K[12][Wc][4] | res[3][B]
+LR_HD size_t fir_apply_smem_bytes(int W, int Wc) {
+  return ((size_t)6 * W + fir_plan_doubles_per_tile(Wc) + 3 * (size_t)kFirTile) * sizeof(double);
+}
+
+// eq. 21 and the coalesced store of one sample (shared by the apply and fix-up kernels)
+__device__ __forceinline__ void fir_store(double* ob, int64_t N, int n, int channels, double X, double Y, double Z) {
+  if (channels != 1) { ob[n] = X; ob[N + n] = Y; ob[2 * N + n] = Z; }
+  if (channels != 0) {
+    double* oa = channels == 2 ? ob + 3 * N : ob;
+    oa[n] = (Z - X) * 0.70710678118654752440;
+    oa[N + n] = (X - 2.0 * Y + Z) * 0.40824829046386301637;
+    oa[2 * N + n] = (X + Y + Z) * 0.57735026918962576451;
+  }
+}
+
+template <int NN>
+__global__ void __launch_bounds__(kFirThreads, 7)
 tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ out, int channels,
                      const double* __restrict__ plan, const int* __restrict__ flags, int batch) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int B = kFirTile;
-  const int P = PT > 0 ? PT : prm.p;
   const int W = B + prm.halo_lo + prm.halo_hi;
   const int Wc = prm.fir_wc;
-  double* raw = reinterpret_cast<double*>(smem_raw);
-  double* dif = raw + 6 * W;
+  double* dif = reinterpret_cast<double*>(smem_raw);
   double* K = dif + 6 * W;
   double* res = K + fir_plan_doubles_per_tile(Wc);
 
@@ -332,49 +345,71 @@ tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __r
         for (int c = 0; c < nout; ++c) ob[(int64_t)c * N + n0 + i] = 0.0;
     return;
   }
-  const bool generic = flags[tile] != 0;
+  if (flags[tile] != 0) return;                              // exact per-sample tile: the fix-up kernel's
 
+  // first differences straight from global memory (the second load of each pair hits L1)
   const double* yb = y + b * 6 * N;
   for (int m = tid; m < 6 * W; m += kFirThreads) {
     const int s = m / W, g = g0 + (m - s * W);
-    raw[m] = (g >= 0 && g < prm.n) ? __ldg(yb + (int64_t)s * N + g) : 0.0;
+    const double* ys = yb + (int64_t)s * N;
+    const double a = (g >= 0 && g < prm.n) ? __ldg(ys + g) : 0.0;
+    const double c = (g + 1 >= 0 && g + 1 < prm.n) ? __ldg(ys + g + 1) : 0.0;
+    dif[m] = c - a;
   }
-  if (!generic) {
-    const double2* src = reinterpret_cast<const double2*>(plan + (size_t)tile * fir_plan_doubles_per_tile(Wc));
-    double2* dst = reinterpret_cast<double2*>(K);
-    const int cnt = (int)(fir_plan_doubles_per_tile(Wc) / 2);
-    for (int m = tid; m < cnt; m += kFirThreads) dst[m] = __ldg(src + m);
-  }
+  const double2* src = reinterpret_cast<const double2*>(plan + (size_t)tile * fir_plan_doubles_per_tile(Wc));
+  double2* dst = reinterpret_cast<double2*>(K);
+  const int cnt = (int)(fir_plan_doubles_per_tile(Wc) / 2);
+  for (int m = tid; m < cnt; m += kFirThreads) dst[m] = __ldg(src + m);
   __syncthreads();
-  for (int m = tid; m < 6 * W; m += kFirThreads) {
-    const int w = m % W;
-    dif[m] = (w < W - 1) ? raw[m + 1] - raw[m] : 0.0;
-  }
-  __syncthreads();
-  const int nl0 = prm.halo_lo;
-  if (generic) {
-    // exact per-sample path: a delay's integer part may change inside this tile
-    for (int i = tid; i < B; i += kFirThreads) {
-      const int n = n0 + i;
-      double xyz[3] = {0.0, 0.0, 0.0};
-      if (n >= v_lo && n < v_hi) tdi_sample<PT, GEN>(prm, raw, dif, W, nl0 + i, sample_trel(prm, n), xyz);
-      res[i] = xyz[0]; res[B + i] = xyz[1]; res[2 * B + i] = xyz[2];
-    }
-  } else {
-    fir_apply<NN>(dif, W, K, Wc, P, nl0, B, res, tid, kFirThreads);
-  }
+  fir_apply<NN>(dif, W, K, Wc, prm.p, prm.halo_lo, B, res, tid, kFirThreads);
   __syncthreads();
   for (int i = tid; i < B; i += kFirThreads) {
     const int n = n0 + i;
     if (n >= prm.n) break;
     const bool valid = n >= v_lo && n < v_hi;
-    const double X = valid ? res[i] : 0.0, Y = valid ? res[B + i] : 0.0, Z = valid ? res[2 * B + i] : 0.0;
-    if (channels != 1) { ob[n] = X; ob[N + n] = Y; ob[2 * N + n] = Z; }
-    if (channels != 0) {  // eq. 21
-      double* oa = channels == 2 ? ob + 3 * N : ob;
-      oa[n] = (Z - X) * 0.70710678118654752440;
-      oa[N + n] = (X - 2.0 * Y + Z) * 0.40824829046386301637;
-      oa[2 * N + n] = (X + Y + Z) * 0.57735026918962576451;
+    fir_store(ob, N, n, channels, valid ? res[i] : 0.0, valid ? res[B + i] : 0.0, valid ? res[2 * B + i] : 0.0);
+  }
+}
+
+// ---------------------------------------------------------------------------------------- fix-up kernel
+// The tiles the plan flagged (a delay crosses a whole number of samples inside them) with the exact
+// per-sample weights of tdi_sample.  Fixed grid; work item = (flagged tile, template).
+// dynamic smem: raw[6][W], dif[6][W]
+template <int PT, int GEN>
+__global__ void __launch_bounds__(kFirTile)
+tdi_fir_fixup_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ out, int channels,
+                     const int* __restrict__ list, int batch) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int B = kFirTile;
+  const int W = B + prm.halo_lo + prm.halo_hi;
+  double* raw = reinterpret_cast<double*>(smem_raw);
+  double* dif = raw + 6 * W;
+  const int tid = threadIdx.x;
+  const int64_t N = prm.n;
+  const int nout = channels == 2 ? 6 : 3;
+  const int v_lo = prm.m_front, v_hi = prm.n - prm.m_back;
+  const int64_t items = (int64_t)list[0] * batch;
+  for (int64_t w = blockIdx.x; w < items; w += gridDim.x) {
+    const int tile = list[1 + (int)(w / batch)];
+    const int64_t b = w % batch;
+    const int n0 = tile * B, g0 = n0 - prm.halo_lo;
+    const double* yb = y + b * 6 * N;
+    __syncthreads();
+    for (int m = tid; m < 6 * W; m += B) {
+      const int s = m / W, g = g0 + (m - s * W);
+      raw[m] = (g >= 0 && g < prm.n) ? __ldg(yb + (int64_t)s * N + g) : 0.0;
+    }
+    __syncthreads();
+    for (int m = tid; m < 6 * W; m += B) {
+      const int ww = m % W;
+      dif[m] = (ww < W - 1) ? raw[m + 1] - raw[m] : 0.0;
+    }
+    __syncthreads();
+    const int n = n0 + tid;
+    if (n < prm.n) {
+      double xyz[3] = {0.0, 0.0, 0.0};
+      if (n >= v_lo && n < v_hi) tdi_sample<PT, GEN>(prm, raw, dif, W, prm.halo_lo + tid, sample_trel(prm, n), xyz);
+      fir_store(out + b * nout * N, N, n, channels, xyz[0], xyz[1], xyz[2]);
     }
   }
 }
