@@ -44,6 +44,8 @@ struct Plan {
   double t0 = 0;
   int gen = 0, chain = 0, path = 0;
   cudaEvent_t ready = nullptr;
+  cudaStream_t side = nullptr;          // the fix-up kernel's stream (forked from / joined to the caller's)
+  cudaEvent_t fork = nullptr, join = nullptr;
 };
 
 struct lr_handle {
@@ -215,6 +217,9 @@ void lr_destroy(lr_handle* h) {
     if (S.dev) cudaFree(S.dev);
   }
   if (h->plan.ready) cudaEventDestroy(h->plan.ready);
+  if (h->plan.fork) cudaEventDestroy(h->plan.fork);
+  if (h->plan.join) cudaEventDestroy(h->plan.join);
+  if (h->plan.side) cudaStreamDestroy(h->plan.side);
   if (h->plan.coef) cudaFree(h->plan.coef);
   if (h->plan.flags) cudaFree(h->plan.flags);
   if (h->scratch) cudaFree(h->scratch);
@@ -287,7 +292,7 @@ int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out,
   int path = h->tdi_path;
   if (path == LR_TDI_AUTO) path = de <= 6e-6 ? LR_TDI_FIR3 : de <= 1.5e-4 ? LR_TDI_FIR4 : LR_TDI_PER_SAMPLE;
   cudaStream_t st = (cudaStream_t)stream;
-  lr::FirPlanArgs pa{nullptr, nullptr, nullptr, 0, false};
+  lr::FirPlanArgs pa{nullptr, nullptr, nullptr, 0, nullptr, nullptr, nullptr, false};
   if (path != LR_TDI_PER_SAMPLE) {
     const int imax = (int)h->tdi_reach(h->gen);
     const int wc = ((imax + 2 * h->p - 2 + lr::kFirR - 1) / lr::kFirR) * lr::kFirR;
@@ -327,6 +332,12 @@ int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out,
       LR_CUDA(h, cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev));
     }
     pa.fixup_grid = 2 * h->sm_count;
+    if (!pl.side) {
+      LR_CUDA(h, cudaStreamCreateWithFlags(&pl.side, cudaStreamNonBlocking));
+      LR_CUDA(h, cudaEventCreateWithFlags(&pl.fork, cudaEventDisableTiming));
+      LR_CUDA(h, cudaEventCreateWithFlags(&pl.join, cudaEventDisableTiming));
+    }
+    pa.side = pl.side; pa.fork = pl.fork; pa.join = pl.join;
   } else {
     P.halo_lo = (int)(mf - h->m_proj()); P.halo_hi = h->p + 2;
     P.ntiles = (int)((n + lr::kTdiThreads - 1) / lr::kTdiThreads);

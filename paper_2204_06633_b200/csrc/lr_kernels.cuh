@@ -138,6 +138,9 @@ struct FirPlanArgs {
   int* flags;     // DEVICE [ntiles]: != 0 marks a tile that needs per-sample weights
   int* list;      // DEVICE [1 + ntiles]: count, then the flagged tiles
   int fixup_grid; // CTAs of the fix-up kernel (2 per SM)
+  void* side;     // cudaStream_t owned by the handle: the fix-up kernel runs there, beside the apply kernel
+  void* fork;     // cudaEvent_t: the caller's stream reached the plan
+  void* join;     // cudaEvent_t: the fix-up kernel finished
   bool build;
 };
 
