@@ -125,8 +125,15 @@ class ClockSampler:
 
 
 # -------------------------------------------------------------------------------------------- workloads
-def make_workload(kind, rank):
+def make_workload(kind, rank, order=None):
     """The benchmarked workload of this rank: (Workload descriptor, number of templates per step)."""
+    w, b = _make_workload(kind, rank)
+    if order is not None:
+        w.order = order   # order sweep (SURVEY.md §8(f) NEXT-3)
+    return w, b
+
+
+def _make_workload(kind, rank):
     from paper_2204_06633_b200 import inputs
     if kind == "year":
         w = inputs.config(2)
@@ -139,6 +146,10 @@ def make_workload(kind, rank):
         return w, hi - lo
     if kind == "tiny":
         return inputs.config(1), 1
+    if kind == "4yr":
+        return inputs.config(4), 1
+    if kind == "chirp":
+        return inputs.config(5), 1
     raise ValueError(kind)
 
 
@@ -189,7 +200,7 @@ def run_reference(args, rank, world):
     """--impl reference: the oracle on the host cores, same metric/config; rank 0 only."""
     if rank != 0:
         return
-    w, _ = make_workload(args.workload, 0)
+    w, _ = make_workload(args.workload, 0, args.order)
     vals, info = [], None
     per_step = max(1.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
     for i in range(args.warmup + args.steps):
@@ -207,7 +218,7 @@ def run_reference(args, rank, world):
 
 
 def workload_config(w, batch, args):
-    return {"workload": f"BASELINE.json configs[{ {'tiny': 0, 'year': 1, 'batch': 2}[args.workload] }] ({w.name})",
+    return {"workload": f"BASELINE.json configs[{ {'tiny': 0, 'year': 1, 'batch': 2, '4yr': 3, 'chirp': 4}[args.workload] }] ({w.name})",
             "batch": batch, "n": w.n, "dt": w.dt, "lagrange_order": w.order, "tdi_gen": w.tdi_gen,
             "chain": "nested", "channels": w.channels, "orbits": w.orbit_kind, "tdi_path": args.tdi_path,
             "l2": "flushed between steps (256 MiB memset outside the per-step event pairs)"}
@@ -220,7 +231,7 @@ def run_gpu(args, rank, world, local_rank):
     lr.binding.lib()  # no CUDA extension -> fail loudly, there is no fallback
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    w, batch = make_workload(args.workload, rank)
+    w, batch = make_workload(args.workload, rank, args.order)
     chunk = min(batch, args.chunk)
     n, T = w.n, w.order + 1
     nout = 6 if w.channels == "XYZ_AET" else 3
@@ -381,7 +392,8 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="year", choices=["year", "batch", "tiny"])
+    ap.add_argument("--workload", default="year", choices=["year", "batch", "tiny", "4yr", "chirp"])
+    ap.add_argument("--order", type=int, default=None, help="override the Lagrange order (order sweep)")
     ap.add_argument("--chunk", type=int, default=64, help="templates per launch (batch workload)")
     ap.add_argument("--e2e-templates", type=int, default=4)
     ap.add_argument("--peak-seconds", type=float, default=1.0)

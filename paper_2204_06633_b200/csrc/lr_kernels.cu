@@ -1,6 +1,6 @@
 // lr_kernels.cu — dispatch on the Lagrange order, and the small helper kernel.
 //
-// Orders 1, 3, 9, 25 and 41 have kernels with the pair count P = (order+1)/2 fixed at compile time (fully
+// Orders 1-15 (odd), 21, 25, 31 and 41 have kernels with the pair count P = (order+1)/2 fixed at compile time (fully
 // unrolled weight recurrences, everything in registers; instantiated by lr_inst.cu); any other odd order up
 // to LR_MAX_ORDER runs the same code with P read at run time.
 #include <cuda_runtime.h>
@@ -25,7 +25,14 @@ int launch_project(const Params& prm, int order, const double* hp, const double*
 #ifndef LR_DEV_ONLY_P13
     case 1: return launch_project_t<1>(prm, hp, hc, basis, y, batch, stream);
     case 3: return launch_project_t<2>(prm, hp, hc, basis, y, batch, stream);
+    case 5: return launch_project_t<3>(prm, hp, hc, basis, y, batch, stream);
+    case 7: return launch_project_t<4>(prm, hp, hc, basis, y, batch, stream);
     case 9: return launch_project_t<5>(prm, hp, hc, basis, y, batch, stream);
+    case 11: return launch_project_t<6>(prm, hp, hc, basis, y, batch, stream);
+    case 13: return launch_project_t<7>(prm, hp, hc, basis, y, batch, stream);
+    case 15: return launch_project_t<8>(prm, hp, hc, basis, y, batch, stream);
+    case 21: return launch_project_t<11>(prm, hp, hc, basis, y, batch, stream);
+    case 31: return launch_project_t<16>(prm, hp, hc, basis, y, batch, stream);
     case 41: return launch_project_t<21>(prm, hp, hc, basis, y, batch, stream);
 #endif
     case 25: return launch_project_t<13>(prm, hp, hc, basis, y, batch, stream);
@@ -39,7 +46,14 @@ int launch_tdi(const Params& prm, int order, int gen, int path, int channels, co
 #ifndef LR_DEV_ONLY_P13
     case 1: return launch_tdi_t<1>(prm, gen, path, channels, y, out, batch, plan, stream);
     case 3: return launch_tdi_t<2>(prm, gen, path, channels, y, out, batch, plan, stream);
+    case 5: return launch_tdi_t<3>(prm, gen, path, channels, y, out, batch, plan, stream);
+    case 7: return launch_tdi_t<4>(prm, gen, path, channels, y, out, batch, plan, stream);
     case 9: return launch_tdi_t<5>(prm, gen, path, channels, y, out, batch, plan, stream);
+    case 11: return launch_tdi_t<6>(prm, gen, path, channels, y, out, batch, plan, stream);
+    case 13: return launch_tdi_t<7>(prm, gen, path, channels, y, out, batch, plan, stream);
+    case 15: return launch_tdi_t<8>(prm, gen, path, channels, y, out, batch, plan, stream);
+    case 21: return launch_tdi_t<11>(prm, gen, path, channels, y, out, batch, plan, stream);
+    case 31: return launch_tdi_t<16>(prm, gen, path, channels, y, out, batch, plan, stream);
     case 41: return launch_tdi_t<21>(prm, gen, path, channels, y, out, batch, plan, stream);
 #endif
     case 25: return launch_tdi_t<13>(prm, gen, path, channels, y, out, batch, plan, stream);

@@ -198,9 +198,10 @@ def test_config5_chirp_reduced(lr):
 
 
 # --------------------------------------------------------------------------------------------- orders
-@pytest.mark.parametrize("order", [1, 3, 5, 9, 13, 31, 65])
+@pytest.mark.parametrize("order", [1, 3, 5, 7, 9, 11, 13, 15, 17, 21, 31, 35, 65])
 def test_orders(lr, order):
-    """Compile-time-P kernels (1, 3, 9) and the run-time-P path (5, 13, 31, 65)."""
+    """Compile-time-P kernels (1-15, 21, 31; 25 and 41 are the configs' orders) and the run-time-P path
+    (17, 35, 65)."""
     w = inputs.config(2, n=3001, f0=2e-3, t0=2.0e7)
     w.order = order
     check_workload(lr, w, channels="XYZ")
