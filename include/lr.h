@@ -58,6 +58,7 @@ typedef struct {
 #define LR_OPT_CHANNELS 3 /* LR_XYZ (default) | LR_AET | LR_XYZ_AET */
 #define LR_OPT_TDI_GEN 4  /* 1 | 2: changes the generation given to lr_create */
 #define LR_OPT_TDI_PATH 5 /* LR_TDI_AUTO (default) | LR_TDI_PER_SAMPLE | LR_TDI_FIR3 | LR_TDI_FIR4 */
+#define LR_OPT_CHUNK_SAMPLES 7 /* time-chunk length of lr_response / lr_response_host (rounded up to 1792); 0 = automatic */
 #define LR_OPT_TDI_PLAN_CACHE 6 /* 1 (default): keep the FIR plan between lr_tdi calls; 0: rebuild every call */
 
 /* How lr_tdi evaluates the Lagrange weights (same result to rounding).
@@ -128,9 +129,21 @@ int lr_project(lr_handle* h, const double* h_plus, const double* h_cross, const 
  * Errors: LR_EINVAL, LR_ERANGE, LR_ECUDA. */
 int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out, void* cuda_stream);
 
+/* Both stages with DEVICE buffers and no [batch][6][n] array: h_plus, h_cross DEVICE [batch][n] -> out DEVICE
+ * [batch][3|6][n], bit-identical to lr_project followed by lr_tdi.  The path runs in chunks of time (and of
+ * 8 templates) through a y scratch of <= 40 MB owned by h_proj, which stays L2-resident, so the device footprint
+ * is h + out (the paper's real call is waveform -> projection -> TDI with nothing
+ * in between leaving the GPU).  Enqueues on `cuda_stream` and returns without synchronising.
+ * beta, lambda, psi: HOST [batch].  Errors: as lr_project / lr_tdi. */
+int lr_response(lr_handle* h_proj, lr_handle* h_tdi, const double* h_plus, const double* h_cross,
+                const double* beta, const double* lambda, const double* psi, int64_t batch, int64_t n, double* out,
+                void* cuda_stream);
+
 /* Both stages with HOST buffers: copies h_plus/h_cross [batch][n] to the device, runs lr_project on
  * `h_proj` and lr_tdi on `h_tdi` (may be the same handle), copies out [batch][3|6][n] back and waits.
- * Device scratch is owned by h_proj and grown on demand (kept until lr_destroy).
+ * The call is a three-stage pipeline over chunks of time: the H2D copy of the next chunk and the D2H copy of
+ * the previous one overlap the kernels (pinned host buffers are needed for the overlap; pageable ones work,
+ * serially).  Device scratch is owned by h_proj and grown on demand (kept until lr_destroy).
  * `cuda_stream` as above.  Errors: as lr_project / lr_tdi, LR_ECUDA for a failed allocation or copy. */
 int lr_response_host(lr_handle* h_proj, lr_handle* h_tdi, const double* h_plus, const double* h_cross,
                      const double* beta, const double* lambda, const double* psi, int64_t batch, int64_t n,

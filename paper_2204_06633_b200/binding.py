@@ -18,6 +18,7 @@ LIB_PATH = os.environ.get("LR_LIBRARY", os.path.join(_HERE, "liblr.so"))  # over
 LR_OK, LR_EINVAL, LR_ERANGE, LR_ECUDA, LR_ENOMEM = 0, -1, -2, -3, -4
 LR_OPT_T0, LR_OPT_CHAIN, LR_OPT_CHANNELS, LR_OPT_TDI_GEN, LR_OPT_TDI_PATH = 1, 2, 3, 4, 5
 LR_OPT_TDI_PLAN_CACHE = 6
+LR_OPT_CHUNK_SAMPLES = 7
 LR_TDI_AUTO, LR_TDI_PER_SAMPLE, LR_TDI_FIR3, LR_TDI_FIR4 = -1, 0, 3, 4
 LR_CHAIN_NESTED, LR_CHAIN_SUM = 0, 1
 LR_XYZ, LR_AET, LR_XYZ_AET = 0, 1, 2
@@ -25,7 +26,7 @@ LR_MAX_ORDER = 65
 
 # every symbol include/lr.h declares
 SYMBOLS = ("lr_create", "lr_destroy", "lr_set_option", "lr_get_margins", "lr_project", "lr_tdi",
-           "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count",
+           "lr_response", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count",
            "lr_last_cuda_error", "lr_strerror")
 
 
@@ -71,6 +72,7 @@ def lib():
     L.lr_get_margins.argtypes = [vp, pi64, pi64, pi64]
     L.lr_project.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
     L.lr_tdi.argtypes = [vp, vp, i64, i64, vp, vp]
+    L.lr_response.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
     L.lr_response_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
     L.lr_eval_orbit.argtypes = [vp, ci, vp, i64, vp, vp]
     L.lr_measure_fp64_peak.argtypes = [dbl, ctypes.POINTER(dbl)]
@@ -161,6 +163,21 @@ def lr_tdi(h, y, out, batch, stream=None):
     if out.numel() not in (3 * batch * n, 6 * batch * n):
         raise ValueError("out must be [batch,3,n] or [batch,6,n]")
     _check(lib().lr_tdi(h, _dev_ptr(y, "y"), batch, n, _dev_ptr(out, "out"), _stream(stream)), "lr_tdi", h)
+    return out
+
+
+def lr_response(h_proj, h_tdi, h_plus, h_cross, beta, lam, psi, out, stream=None):
+    """lr_response: h_plus, h_cross CUDA [B,N] -> out CUDA [B,3|6,N], no y array (chunked through L2)."""
+    beta, lam, psi = _host(beta), _host(lam), _host(psi)
+    B = beta.size
+    if h_plus.numel() % B:
+        raise ValueError("h_plus size is not a multiple of the batch")
+    n = h_plus.numel() // B
+    if out.numel() not in (3 * B * n, 6 * B * n):
+        raise ValueError("out must be [batch,3,n] or [batch,6,n]")
+    _check(lib().lr_response(h_proj, h_tdi, _dev_ptr(h_plus, "h_plus"), _dev_ptr(h_cross, "h_cross", B * n),
+                             beta.ctypes.data, lam.ctypes.data, psi.ctypes.data, B, n, _dev_ptr(out, "out"),
+                             _stream(stream)), "lr_response", h_proj)
     return out
 
 

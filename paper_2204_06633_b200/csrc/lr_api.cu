@@ -58,15 +58,20 @@ struct lr_handle {
   int tdi_path = -1;     // LR_OPT_TDI_PATH: -1 auto | 0 generic | 3 | 4
   int plan_cache = 1;    // LR_OPT_TDI_PLAN_CACHE
   int sm_count = 0;
+  int64_t chunk_samples = 0;   // LR_OPT_CHUNK_SAMPLES: 0 = automatic
   Plan plan;
   double bk[lr::kPMax + 1];
   // device state
   lr::D4* coef = nullptr;
   Stage stage[kSlots];
   int next_slot = 0;
-  // scratch of lr_response_host
-  double* scratch = nullptr;
-  size_t scratch_bytes = 0;
+  // scratch of lr_response / lr_response_host: y of one chunk, and for the host variant two staging
+  // buffers each for h and out plus the copy streams of the three-stage pipeline
+  double* y_scr = nullptr; size_t y_cap = 0;        // elements
+  double* h_buf = nullptr; size_t h_cap = 0;
+  double* o_buf = nullptr; size_t o_cap = 0;
+  cudaStream_t s_in = nullptr, s_out = nullptr;
+  cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
   int last_cuda = 0;
 
   int64_t m_proj() const {
@@ -99,7 +104,9 @@ lr::Params make_params(const lr_handle* h, int64_t n) {
   P.inv_h = 1.0 / h->knot_dt;
   P.inv_dt = 1.0 / h->dt;
   P.inv_cdt = 1.0 / (lr::kC * h->dt);
-  P.n = (int)n;
+  P.n = (int)n; P.n_off = 0; P.n_glob = (int)n;          // default window: the whole series
+  P.rd_lo = 0; P.rd_hi = (int)n;
+  P.in_stride = n; P.out_stride = n;
   P.m_proj = (int)h->m_proj();
   P.m_front = (int)h->m_front(h->gen);
   P.m_back = (int)h->m_back();
@@ -222,7 +229,16 @@ void lr_destroy(lr_handle* h) {
   if (h->plan.side) cudaStreamDestroy(h->plan.side);
   if (h->plan.coef) cudaFree(h->plan.coef);
   if (h->plan.flags) cudaFree(h->plan.flags);
-  if (h->scratch) cudaFree(h->scratch);
+  if (h->y_scr) cudaFree(h->y_scr);
+  if (h->h_buf) cudaFree(h->h_buf);
+  if (h->o_buf) cudaFree(h->o_buf);
+  for (int i = 0; i < 2; ++i) {
+    if (h->ev_in[i]) cudaEventDestroy(h->ev_in[i]);
+    if (h->ev_comp[i]) cudaEventDestroy(h->ev_comp[i]);
+    if (h->ev_out[i]) cudaEventDestroy(h->ev_out[i]);
+  }
+  if (h->s_in) cudaStreamDestroy(h->s_in);
+  if (h->s_out) cudaStreamDestroy(h->s_out);
   if (h->coef) cudaFree(h->coef);
   delete h;
 }
@@ -244,6 +260,9 @@ int lr_set_option(lr_handle* h, int key, double value) {
       if (value != LR_TDI_AUTO && value != LR_TDI_PER_SAMPLE && value != LR_TDI_FIR3 && value != LR_TDI_FIR4)
         return LR_EINVAL;
       h->tdi_path = (int)value; return LR_OK;
+    case LR_OPT_CHUNK_SAMPLES:
+      if (value < 0 || value > 2147483647.0 || value != floor(value)) return LR_EINVAL;
+      h->chunk_samples = (int64_t)value; return LR_OK;
     case LR_OPT_TDI_PLAN_CACHE:
       if (value != 0 && value != 1) return LR_EINVAL;
       h->plan_cache = (int)value; h->plan.valid = false; return LR_OK;
@@ -259,54 +278,75 @@ int lr_get_margins(const lr_handle* h, int64_t* m_proj, int64_t* m_front, int64_
   return LR_OK;
 }
 
-int lr_project(lr_handle* h, const double* hp, const double* hc, const double* beta, const double* lam,
-               const double* psi, int64_t batch, int64_t n, double* y, void* stream) {
-  if (!h || !hp || !hc || !beta || !lam || !psi || !y) return LR_EINVAL;
-  if (!size_ok(batch, n) || n <= 2 * h->m_proj()) return LR_EINVAL;
+}  // extern "C"
+
+namespace {
+
+// A launch window: the kernels process global samples [off, off + n) of a series of n_glob samples; `in`
+// points at the input row element of global sample `off` and may be read for global samples
+// [rd_a, rd_b); rows of the input / output arrays are in_stride / out_stride elements apart.
+struct Window {
+  int64_t n_glob, off, n, rd_a, rd_b, in_stride, out_stride;
+};
+
+void apply_window(lr::Params& P, const Window& w) {
+  P.n = (int)w.n; P.n_off = (int)w.off; P.n_glob = (int)w.n_glob;
+  P.rd_lo = (int)(w.rd_a - w.off); P.rd_hi = (int)(w.rd_b - w.off);
+  P.in_stride = w.in_stride; P.out_stride = w.out_stride;
+}
+
+int project_window(lr_handle* h, const double* hp, const double* hc, const double* basis_dev, int64_t batch,
+                   const Window& w, double* y, void* stream) {
+  lr::Params P = make_params(h, w.n_glob);
+  apply_window(P, w);
   const int64_t mp = h->m_proj();
-  if (!in_table(h, mp, n - mp - 1, 0.0)) return LR_ERANGE;
-  cudaStream_t st = (cudaStream_t)stream;
-  Stage* S = nullptr;
-  int rc = stage_basis(h, beta, lam, psi, batch, st, &S);
-  if (rc != LR_OK) return rc;
-  lr::Params P = make_params(h, n);
   P.halo_lo = (int)mp; P.halo_hi = (int)mp;
-  P.ntiles = (int)((n + lr::kProjThreads - 1) / lr::kProjThreads);
-  const int e = lr::launch_project(P, h->order, hp, hc, S->dev, y, batch, stream);
+  P.ntiles = (int)((w.n + lr::kProjThreads - 1) / lr::kProjThreads);
+  const int e = lr::launch_project(P, h->order, hp, hc, basis_dev, y, batch, stream);
   if (e != 0) { h->last_cuda = e; return LR_ECUDA; }
-  LR_CUDA(h, cudaEventRecord(S->done, st));
-  S->pending = true;
   return LR_OK;
 }
 
-int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out, void* stream) {
-  if (!h || !y || !out) return LR_EINVAL;
-  const int64_t mf = h->m_front(h->gen), mb = h->m_back();
-  if (!size_ok(batch, n) || n <= mf + mb) return LR_EINVAL;
-  const double reach = (double)(h->gen == 1 ? 4 : 8) * 1.001 * h->l_max;
-  if (!in_table(h, mf, n - mb - 1, reach)) return LR_ERANGE;
-  lr::Params P = make_params(h, n);
-  // path: per-tile polynomial FIR when the delays drift slowly enough, else exact per-sample weights
+// which lr_tdi path this handle takes, and the staged halo of that path's kernels
+struct TdiShape { int path, wc, halo_lo, halo_hi; };
+
+TdiShape tdi_shape(const lr_handle* h) {
+  TdiShape t{h->tdi_path, 0, 0, 0};
+  const int64_t mf = h->m_front(h->gen);
+  // per-tile polynomial FIR when the delays drift slowly enough, else exact per-sample weights
   const int nlinks = h->gen == 1 ? 3 : 7;  // links in the longest delayed term
   const double de = (double)nlinks * h->max_ldot * (double)lr::kFirTile;  // change of eps over one tile
-  int path = h->tdi_path;
-  if (path == LR_TDI_AUTO) path = de <= 6e-6 ? LR_TDI_FIR3 : de <= 1.5e-4 ? LR_TDI_FIR4 : LR_TDI_PER_SAMPLE;
-  cudaStream_t st = (cudaStream_t)stream;
-  lr::FirPlanArgs pa{nullptr, nullptr, nullptr, 0, nullptr, nullptr, nullptr, false};
-  if (path != LR_TDI_PER_SAMPLE) {
+  if (t.path == LR_TDI_AUTO) t.path = de <= 6e-6 ? LR_TDI_FIR3 : de <= 1.5e-4 ? LR_TDI_FIR4 : LR_TDI_PER_SAMPLE;
+  if (t.path != LR_TDI_PER_SAMPLE) {
     const int imax = (int)h->tdi_reach(h->gen);
-    const int wc = ((imax + 2 * h->p - 2 + lr::kFirR - 1) / lr::kFirR) * lr::kFirR;
-    const int back = wc - (h->p - 1);
-    P.fir_wc = wc;
-    P.halo_lo = back > (int)(mf - h->m_proj()) ? back : (int)(mf - h->m_proj());
-    P.halo_hi = h->p + lr::kFirR;
-    P.ntiles = (int)((n + lr::kFirTile - 1) / lr::kFirTile);
-    const size_t smem = lr::fir_apply_smem_bytes(lr::kFirTile + P.halo_lo + P.halo_hi, wc);
-    if (smem > 200 * 1024) path = LR_TDI_PER_SAMPLE;   // very long stencils: keep the per-sample kernel
+    t.wc = ((imax + 2 * h->p - 2 + lr::kFirR - 1) / lr::kFirR) * lr::kFirR;
+    const int back = t.wc - (h->p - 1);
+    t.halo_lo = back > (int)(mf - h->m_proj()) ? back : (int)(mf - h->m_proj());
+    t.halo_hi = h->p + lr::kFirR;
+    // very long stencils: keep the per-sample kernel
+    if (lr::fir_apply_smem_bytes(lr::kFirTile + t.halo_lo + t.halo_hi, t.wc) > 200 * 1024) t.path = LR_TDI_PER_SAMPLE;
   }
+  if (t.path == LR_TDI_PER_SAMPLE) {
+    t.wc = 0;
+    t.halo_lo = (int)(mf - h->m_proj());
+    t.halo_hi = h->p + 2;
+  }
+  return t;
+}
+
+int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, double* out, void* stream) {
+  lr::Params P = make_params(h, w.n_glob);
+  const TdiShape ts = tdi_shape(h);
+  const int path = ts.path;
+  cudaStream_t st = (cudaStream_t)stream;
+  lr::FirPlanArgs pa{nullptr, nullptr, nullptr, 0, 0, nullptr, nullptr, nullptr, false};
+  P.halo_lo = ts.halo_lo; P.halo_hi = ts.halo_hi; P.fir_wc = ts.wc;
   if (path != LR_TDI_PER_SAMPLE) {
+    if (w.off % lr::kFirTile != 0) return LR_EINVAL;   // windows of the FIR path start on a tile
+    // the plan always covers the whole series (global tiles)
+    P.ntiles = (int)((w.n_glob + lr::kFirTile - 1) / lr::kFirTile);
     Plan& pl = h->plan;
-    const bool reuse = h->plan_cache && pl.valid && pl.n == n && pl.t0 == h->t0 && pl.gen == h->gen &&
+    const bool reuse = h->plan_cache && pl.valid && pl.n == w.n_glob && pl.t0 == h->t0 && pl.gen == h->gen &&
                        pl.chain == h->chain && pl.path == path;
     if (!reuse) {
       const size_t need = (size_t)P.ntiles * lr::fir_plan_doubles_per_tile(P.fir_wc);
@@ -326,6 +366,7 @@ int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out,
       LR_CUDA(h, cudaStreamWaitEvent(st, pl.ready, 0));   // the plan may have been built on another stream
     }
     pa.coef = pl.coef; pa.flags = pl.flags; pa.list = pl.flags + P.ntiles; pa.build = !reuse;
+    pa.plan_tiles = P.ntiles;
     if (h->sm_count == 0) {
       int dev = 0;
       LR_CUDA(h, cudaGetDevice(&dev));
@@ -338,16 +379,134 @@ int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out,
       LR_CUDA(h, cudaEventCreateWithFlags(&pl.join, cudaEventDisableTiming));
     }
     pa.side = pl.side; pa.fork = pl.fork; pa.join = pl.join;
+    apply_window(P, w);
+    P.ntiles = (int)((w.n + lr::kFirTile - 1) / lr::kFirTile);
   } else {
-    P.halo_lo = (int)(mf - h->m_proj()); P.halo_hi = h->p + 2;
-    P.ntiles = (int)((n + lr::kTdiThreads - 1) / lr::kTdiThreads);
+    apply_window(P, w);
+    P.ntiles = (int)((w.n + lr::kTdiThreads - 1) / lr::kTdiThreads);
   }
   const int e = lr::launch_tdi(P, h->order, h->gen, path, h->channels, y, out, batch, pa, stream);
   if (e != 0) { h->last_cuda = e; return LR_ECUDA; }
   if (pa.build) {
     Plan& pl = h->plan;
     LR_CUDA(h, cudaEventRecord(pl.ready, st));
-    pl.valid = true; pl.n = n; pl.t0 = h->t0; pl.gen = h->gen; pl.chain = h->chain; pl.path = path;
+    pl.valid = true; pl.n = w.n_glob; pl.t0 = h->t0; pl.gen = h->gen; pl.chain = h->chain; pl.path = path;
+  }
+  return LR_OK;
+}
+
+int check_project(const lr_handle* h, int64_t batch, int64_t n) {
+  if (!size_ok(batch, n) || n <= 2 * h->m_proj()) return LR_EINVAL;
+  const int64_t mp = h->m_proj();
+  return in_table(h, mp, n - mp - 1, 0.0) ? LR_OK : LR_ERANGE;
+}
+
+int check_tdi(const lr_handle* h, int64_t batch, int64_t n) {
+  const int64_t mf = h->m_front(h->gen), mb = h->m_back();
+  if (!size_ok(batch, n) || n <= mf + mb) return LR_EINVAL;
+  const double reach = (double)(h->gen == 1 ? 4 : 8) * 1.001 * h->l_max;
+  return in_table(h, mf, n - mb - 1, reach) ? LR_OK : LR_ERANGE;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lr_project(lr_handle* h, const double* hp, const double* hc, const double* beta, const double* lam,
+               const double* psi, int64_t batch, int64_t n, double* y, void* stream) {
+  if (!h || !hp || !hc || !beta || !lam || !psi || !y) return LR_EINVAL;
+  int rc = check_project(h, batch, n);
+  if (rc != LR_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  Stage* S = nullptr;
+  rc = stage_basis(h, beta, lam, psi, batch, st, &S);
+  if (rc != LR_OK) return rc;
+  const Window w{n, 0, n, 0, n, n, n};
+  rc = project_window(h, hp, hc, S->dev, batch, w, y, stream);
+  if (rc != LR_OK) return rc;
+  LR_CUDA(h, cudaEventRecord(S->done, st));
+  S->pending = true;
+  return LR_OK;
+}
+
+int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out, void* stream) {
+  if (!h || !y || !out) return LR_EINVAL;
+  const int rc = check_tdi(h, batch, n);
+  if (rc != LR_OK) return rc;
+  const Window w{n, 0, n, 0, n, n, n};
+  return tdi_window(h, y, batch, w, out, stream);
+}
+
+}  // extern "C"
+
+namespace {
+
+constexpr int64_t kChunkUnit = 1792;   // lcm of the kernels' tile sizes (128, 224, 256)
+
+int ensure(lr_handle* h, double** buf, size_t* cap, size_t need) {
+  if (*cap >= need) return LR_OK;
+  if (*buf) { cudaFree(*buf); *buf = nullptr; *cap = 0; }
+  LR_CUDA(h, cudaMalloc(buf, need * sizeof(double)));
+  *cap = need;
+  return LR_OK;
+}
+
+// One (template chunk, time chunk) of the two-stage path through the y scratch.  hp/hc: DEVICE rows of
+// stride h_stride whose element 0 is global sample h_a and that hold global samples [h_a, h_b).
+// out_chunk: DEVICE rows of stride o_stride whose element 0 is global sample a.
+int response_chunk(lr_handle* hp_, lr_handle* ht_, const TdiShape& ts, const double* hp, const double* hc,
+                   int64_t h_a, int64_t h_b, int64_t h_stride, const double* basis_dev, int64_t nb, int64_t n,
+                   int64_t a, int64_t b, int64_t ly, double* out_chunk, int64_t o_stride, void* stream) {
+  const int64_t ya = a - ts.halo_lo > 0 ? a - ts.halo_lo : 0;
+  const int64_t yb = b + ts.halo_hi < n ? b + ts.halo_hi : n;
+  const Window wp{n, ya, yb - ya, h_a, h_b, h_stride, ly};
+  int rc = project_window(hp_, hp + (ya - h_a), hc + (ya - h_a), basis_dev, nb, wp, hp_->y_scr, stream);
+  if (rc != LR_OK) return rc;
+  const Window wt{n, a, b - a, ya, yb, ly, o_stride};
+  rc = tdi_window(ht_, hp_->y_scr + (a - ya), nb, wt, out_chunk, stream);
+  if (rc != LR_OK) hp_->last_cuda = ht_->last_cuda;
+  return rc;
+}
+
+int64_t round_up(int64_t v, int64_t u) { return (v + u - 1) / u * u; }
+
+}  // namespace
+
+extern "C" {
+
+int lr_response(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const double* h_cross, const double* beta,
+                const double* lam, const double* psi, int64_t batch, int64_t n, double* out, void* stream) {
+  lr_handle* h = hp_;
+  if (!h || !ht_ || !h_plus || !h_cross || !beta || !lam || !psi || !out) return LR_EINVAL;
+  int rc = check_project(h, batch, n);
+  if (rc == LR_OK) rc = check_tdi(ht_, batch, n);
+  if (rc != LR_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const TdiShape ts = tdi_shape(ht_);
+  const int nout = ht_->channels == LR_XYZ_AET ? 6 : 3;
+  // y of one chunk stays small enough to live in L2 (and bounds the footprint: no [batch][6][n] buffer)
+  const int64_t bc = batch < 8 ? batch : 8;
+  const int64_t budget = ((int64_t)40 << 20) / (bc * 6 * (int64_t)sizeof(double));
+  int64_t lc = budget / kChunkUnit * kChunkUnit;
+  if (lc < 4 * kChunkUnit) lc = 4 * kChunkUnit;
+  if (h->chunk_samples > 0) lc = round_up(h->chunk_samples, kChunkUnit);
+  if (lc > round_up(n, kChunkUnit)) lc = round_up(n, kChunkUnit);
+  const int64_t ly = round_up(lc + ts.halo_lo + ts.halo_hi, 2);
+  rc = ensure(h, &h->y_scr, &h->y_cap, (size_t)(bc * 6 * ly));
+  if (rc != LR_OK) return rc;
+  for (int64_t b0 = 0; b0 < batch; b0 += bc) {
+    const int64_t nb = batch - b0 < bc ? batch - b0 : bc;
+    Stage* S = nullptr;
+    rc = stage_basis(h, beta + b0, lam + b0, psi + b0, nb, st, &S);
+    if (rc != LR_OK) return rc;
+    for (int64_t a = 0; a < n; a += lc) {
+      const int64_t b = a + lc < n ? a + lc : n;
+      rc = response_chunk(h, ht_, ts, h_plus + b0 * n, h_cross + b0 * n, 0, n, n, S->dev, nb, n, a, b, ly,
+                          out + b0 * nout * n + a, n, stream);
+      if (rc != LR_OK) return rc;
+    }
+    LR_CUDA(h, cudaEventRecord(S->done, st));
+    S->pending = true;
   }
   return LR_OK;
 }
@@ -356,35 +515,81 @@ int lr_response_host(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const
                      const double* lam, const double* psi, int64_t batch, int64_t n, double* out, void* stream) {
   lr_handle* h = hp_;
   if (!h || !ht_ || !h_plus || !h_cross || !beta || !lam || !psi || !out) return LR_EINVAL;
-  if (!size_ok(batch, n)) return LR_EINVAL;
+  int rc = check_project(h, batch, n);
+  if (rc == LR_OK) rc = check_tdi(ht_, batch, n);
+  if (rc != LR_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
+  const TdiShape ts = tdi_shape(ht_);
   const int nout = ht_->channels == LR_XYZ_AET ? 6 : 3;
-  const size_t per = (size_t)n * sizeof(double) * (size_t)(2 + 6 + nout);  // device bytes per template
-  const size_t limit = (size_t)8 << 30;
-  int64_t chunk = (int64_t)(limit / per);
-  if (chunk < 1) chunk = 1;
-  if (chunk > batch) chunk = batch;
-  const size_t need = per * (size_t)chunk;
-  if (h->scratch_bytes < need) {
-    if (h->scratch) { cudaFree(h->scratch); h->scratch = nullptr; h->scratch_bytes = 0; }
-    LR_CUDA(h, cudaMalloc(&h->scratch, need));
-    h->scratch_bytes = need;
+  const int64_t mp = h->m_proj();
+  // three-stage pipeline over (template chunk, time chunk): H2D of the next chunk's h and D2H of the previous
+  // chunk's out run on the handle's copy streams while the kernels of the current chunk run on `stream`
+  const int64_t bc = batch < 8 ? batch : 8;
+  int64_t lc = round_up((n + 7) / 8, kChunkUnit);                       // about 8 chunks per template
+  const int64_t cap = ((int64_t)40 << 20) / (bc * 6 * (int64_t)sizeof(double)) / kChunkUnit * kChunkUnit;
+  if (lc > cap) lc = cap;
+  if (lc < 4 * kChunkUnit) lc = 4 * kChunkUnit;
+  if (h->chunk_samples > 0) lc = round_up(h->chunk_samples, kChunkUnit);
+  const int64_t ly = round_up(lc + ts.halo_lo + ts.halo_hi, 2);
+  const int64_t lh = ly + 2 * mp;
+  rc = ensure(h, &h->y_scr, &h->y_cap, (size_t)(bc * 6 * ly));
+  if (rc == LR_OK) rc = ensure(h, &h->h_buf, &h->h_cap, (size_t)(2 * 2 * bc * lh));
+  if (rc == LR_OK) rc = ensure(h, &h->o_buf, &h->o_cap, (size_t)(2 * bc * nout * lc));
+  if (rc != LR_OK) return rc;
+  if (!h->s_in) {
+    LR_CUDA(h, cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking));
+    LR_CUDA(h, cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+      LR_CUDA(h, cudaEventCreateWithFlags(&h->ev_in[i], cudaEventDisableTiming));
+      LR_CUDA(h, cudaEventCreateWithFlags(&h->ev_comp[i], cudaEventDisableTiming));
+      LR_CUDA(h, cudaEventCreateWithFlags(&h->ev_out[i], cudaEventDisableTiming));
+    }
   }
-  for (int64_t b0 = 0; b0 < batch; b0 += chunk) {
-    const int64_t nb = (batch - b0 < chunk) ? batch - b0 : chunk;
-    double* d_hp = h->scratch;
-    double* d_hc = d_hp + (size_t)nb * n;
-    double* d_y = d_hc + (size_t)nb * n;
-    double* d_out = d_y + (size_t)nb * 6 * n;
-    LR_CUDA(h, cudaMemcpyAsync(d_hp, h_plus + (size_t)b0 * n, (size_t)nb * n * sizeof(double), cudaMemcpyHostToDevice, st));
-    LR_CUDA(h, cudaMemcpyAsync(d_hc, h_cross + (size_t)b0 * n, (size_t)nb * n * sizeof(double), cudaMemcpyHostToDevice, st));
-    int rc = lr_project(h, d_hp, d_hc, beta + b0, lam + b0, psi + b0, nb, n, d_y, stream);
+  // the copy streams start after whatever the caller enqueued on `stream` before this call
+  LR_CUDA(h, cudaEventRecord(h->ev_comp[0], st));
+  LR_CUDA(h, cudaStreamWaitEvent(h->s_in, h->ev_comp[0], 0));
+  LR_CUDA(h, cudaStreamWaitEvent(h->s_out, h->ev_comp[0], 0));
+  int64_t c = 0;
+  const size_t dsz = sizeof(double);
+  for (int64_t b0 = 0; b0 < batch; b0 += bc) {
+    const int64_t nb = batch - b0 < bc ? batch - b0 : bc;
+    Stage* S = nullptr;
+    rc = stage_basis(h, beta + b0, lam + b0, psi + b0, nb, st, &S);
     if (rc != LR_OK) return rc;
-    rc = lr_tdi(ht_, d_y, nb, n, d_out, stream);
-    if (rc != LR_OK) { h->last_cuda = ht_->last_cuda; return rc; }
-    LR_CUDA(h, cudaMemcpyAsync(out + (size_t)b0 * nout * n, d_out, (size_t)nb * nout * n * sizeof(double),
-                               cudaMemcpyDeviceToHost, st));
+    for (int64_t a = 0; a < n; a += lc, ++c) {
+      const int slot = (int)(c & 1);
+      const int64_t b = a + lc < n ? a + lc : n;
+      const int64_t ya = a - ts.halo_lo > 0 ? a - ts.halo_lo : 0, yb = b + ts.halo_hi < n ? b + ts.halo_hi : n;
+      const int64_t ha = ya - mp > 0 ? ya - mp : 0, hb = yb + mp < n ? yb + mp : n;
+      double* hp_d = h->h_buf + (size_t)slot * 2 * bc * lh;
+      double* hc_d = hp_d + (size_t)bc * lh;
+      double* o_d = h->o_buf + (size_t)slot * bc * nout * lc;
+      // stage 1: H2D (the kernels of chunk c-2 must be done with this slot's h buffer)
+      if (c >= 2) LR_CUDA(h, cudaStreamWaitEvent(h->s_in, h->ev_comp[slot], 0));
+      LR_CUDA(h, cudaMemcpy2DAsync(hp_d, lh * dsz, h_plus + b0 * n + ha, n * dsz, (hb - ha) * dsz, nb,
+                                   cudaMemcpyHostToDevice, h->s_in));
+      LR_CUDA(h, cudaMemcpy2DAsync(hc_d, lh * dsz, h_cross + b0 * n + ha, n * dsz, (hb - ha) * dsz, nb,
+                                   cudaMemcpyHostToDevice, h->s_in));
+      LR_CUDA(h, cudaEventRecord(h->ev_in[slot], h->s_in));
+      // stage 2: kernels (the D2H of chunk c-2 must be done with this slot's out buffer)
+      LR_CUDA(h, cudaStreamWaitEvent(st, h->ev_in[slot], 0));
+      if (c >= 2) LR_CUDA(h, cudaStreamWaitEvent(st, h->ev_out[slot], 0));
+      rc = response_chunk(h, ht_, ts, hp_d, hc_d, ha, hb, lh, S->dev, nb, n, a, b, ly, o_d, lc, stream);
+      if (rc != LR_OK) return rc;
+      LR_CUDA(h, cudaEventRecord(h->ev_comp[slot], st));
+      // stage 3: D2H
+      LR_CUDA(h, cudaStreamWaitEvent(h->s_out, h->ev_comp[slot], 0));
+      for (int ch = 0; ch < nout; ++ch)   // rows [template][channel]: one 2-D copy per channel
+        LR_CUDA(h, cudaMemcpy2DAsync(out + (b0 * nout + ch) * n + a, (size_t)nout * n * dsz, o_d + (size_t)ch * lc,
+                                     (size_t)nout * lc * dsz, (b - a) * dsz, nb, cudaMemcpyDeviceToHost, h->s_out));
+      LR_CUDA(h, cudaEventRecord(h->ev_out[slot], h->s_out));
+    }
+    LR_CUDA(h, cudaEventRecord(S->done, st));
+    S->pending = true;
   }
+  // join: `stream` waits for the last copies, then the call waits for `stream`
+  LR_CUDA(h, cudaStreamWaitEvent(st, h->ev_out[0], 0));
+  if (c >= 2) LR_CUDA(h, cudaStreamWaitEvent(st, h->ev_out[1], 0));
   LR_CUDA(h, cudaStreamSynchronize(st));
   return LR_OK;
 }

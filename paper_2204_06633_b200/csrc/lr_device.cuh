@@ -56,7 +56,12 @@ struct Params {
   double inv_h;        // 1 / knot_dt
   double inv_dt;       // 1 / dt
   double inv_cdt;      // 1 / (c dt)
-  int n;               // samples per template
+  int n;               // samples this launch processes: local indices [0, n)
+  int n_off;           // global sample index of local sample 0 (time and margins are global)
+  int n_glob;          // samples of the whole series
+  int rd_lo, rd_hi;    // local index range [rd_lo, rd_hi) in which the input rows may be read (0 outside)
+  int64_t in_stride;   // elements between rows (and templates: rows x in_stride) of the input arrays
+  int64_t out_stride;  // same for the output array
   int m_proj, m_front, m_back;
   int halo_lo, halo_hi;  // staged window = [n0 - halo_lo, n0 + B + halo_hi)
   int ntiles;

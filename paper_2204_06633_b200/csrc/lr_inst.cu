@@ -57,8 +57,10 @@ static int launch_tdi_fir(const Params& prm, int channels, const double* y, doub
                         (size_t)FirTile<GEN, NN>::NT * NN * (2 * P - 1) * sizeof(double);
     if ((e = prepare(tdi_fir_setup_kernel<PT, GEN, NN>, smem)) != cudaSuccess) return (int)e;
     if ((e = cudaMemsetAsync(plan.list, 0, sizeof(int), st)) != cudaSuccess) return (int)e;
-    tdi_fir_setup_kernel<PT, GEN, NN><<<(unsigned)prm.ntiles, kFirSetupThreads, smem, st>>>(prm, plan.coef, plan.flags,
-                                                                                        plan.list);
+    Params full = prm;   // the plan covers the whole series, whatever window this launch filters
+    full.n = prm.n_glob; full.n_off = 0;
+    tdi_fir_setup_kernel<PT, GEN, NN><<<(unsigned)plan.plan_tiles, kFirSetupThreads, smem, st>>>(full, plan.coef,
+                                                                                             plan.flags, plan.list);
     g_launches.fetch_add(1);
     if ((e = cudaGetLastError()) != cudaSuccess) return (int)e;
   }

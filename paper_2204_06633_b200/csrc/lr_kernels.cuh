@@ -37,13 +37,13 @@ project_kernel(const Params prm, const double* __restrict__ hp, const double* __
   const int64_t b = blockIdx.x / prm.ntiles;
   const int n0 = tile * kProjThreads;
   const int g0 = n0 - prm.halo_lo;  // global sample index of staged index 0
-  const double* hpb = hp + b * (int64_t)prm.n;
-  const double* hcb = hc + b * (int64_t)prm.n;
+  const double* hpb = hp + b * prm.in_stride;
+  const double* hcb = hc + b * prm.in_stride;
 
   for (int m = threadIdx.x; m < W; m += kProjThreads) {
     const int g = g0 + m;
     D2 v{0.0, 0.0};
-    if (g >= 0 && g < prm.n) { v.x = __ldg(hpb + g); v.y = __ldg(hcb + g); }
+    if (g >= prm.rd_lo && g < prm.rd_hi) { v.x = __ldg(hpb + g); v.y = __ldg(hcb + g); }
     raw[m] = v;
   }
   __syncthreads();
@@ -54,10 +54,11 @@ project_kernel(const Params prm, const double* __restrict__ hp, const double* __
 
   const int n = n0 + (int)threadIdx.x;
   if (n >= prm.n) return;
-  double* yb = y + b * 6 * (int64_t)prm.n + n;
-  if (n < prm.m_proj || n >= prm.n - prm.m_proj) {
+  double* yb = y + b * 6 * prm.out_stride + n;
+  const int ng = prm.n_off + n;   // global sample index
+  if (ng < prm.m_proj || ng >= prm.n_glob - prm.m_proj) {
 #pragma unroll
-    for (int s = 0; s < 6; ++s) yb[(int64_t)s * prm.n] = 0.0;
+    for (int s = 0; s < 6; ++s) yb[s * prm.out_stride] = 0.0;
     return;
   }
 
@@ -65,9 +66,9 @@ project_kernel(const Params prm, const double* __restrict__ hp, const double* __
 #pragma unroll
   for (int a = 0; a < 9; ++a) bs[a] = __ldg(basis + b * 9 + a);
   double y6[6];
-  project_sample<PT>(prm, raw, dif, W, n - g0, sample_trel(prm, n), bs, y6);
+  project_sample<PT>(prm, raw, dif, W, n - g0, sample_trel(prm, ng), bs, y6);
 #pragma unroll
-  for (int s = 0; s < 6; ++s) yb[(int64_t)s * prm.n] = y6[s];
+  for (int s = 0; s < 6; ++s) yb[s * prm.out_stride] = y6[s];
 }
 
 // ---------------------------------------------------------------------------------------------- stage 2
@@ -85,11 +86,11 @@ tdi_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ 
   const int64_t b = blockIdx.x / prm.ntiles;
   const int n0 = tile * kTdiThreads;
   const int g0 = n0 - prm.halo_lo;
-  const double* yb = y + b * 6 * (int64_t)prm.n;
+  const double* yb = y + b * 6 * prm.in_stride;
 
   for (int m = threadIdx.x; m < 6 * W; m += kTdiThreads) {
     const int s = m / W, g = g0 + (m - s * W);
-    raw[m] = (g >= 0 && g < prm.n) ? __ldg(yb + (int64_t)s * prm.n + g) : 0.0;
+    raw[m] = (g >= prm.rd_lo && g < prm.rd_hi) ? __ldg(yb + s * prm.in_stride + g) : 0.0;
   }
   __syncthreads();
   for (int m = threadIdx.x; m < 6 * W; m += kTdiThreads) {
@@ -101,16 +102,17 @@ tdi_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ 
   const int n = n0 + (int)threadIdx.x;
   if (n >= prm.n) return;
   const int nout = channels == 2 ? 6 : 3;
-  double* ob = out + b * nout * (int64_t)prm.n + n;
-  if (n < prm.m_front || n >= prm.n - prm.m_back) {
-    for (int c = 0; c < nout; ++c) ob[(int64_t)c * prm.n] = 0.0;
+  double* ob = out + b * nout * prm.out_stride + n;
+  const int ng = prm.n_off + n;   // global sample index
+  if (ng < prm.m_front || ng >= prm.n_glob - prm.m_back) {
+    for (int c = 0; c < nout; ++c) ob[c * prm.out_stride] = 0.0;
     return;
   }
 
   double xyz[3];
-  tdi_sample<PT, GEN>(prm, raw, dif, W, n - g0, sample_trel(prm, n), xyz);
+  tdi_sample<PT, GEN>(prm, raw, dif, W, n - g0, sample_trel(prm, ng), xyz);
 
-  const int64_t N = prm.n;
+  const int64_t N = prm.out_stride;
   if (channels != 1) { ob[0] = xyz[0]; ob[N] = xyz[1]; ob[2 * N] = xyz[2]; }
   if (channels != 0) {  // eq. 21
     const double A = (xyz[2] - xyz[0]) * 0.70710678118654752440;
@@ -137,6 +139,7 @@ struct FirPlanArgs {
   double* coef;   // DEVICE [ntiles][12][Wc][kFirKStride]
   int* flags;     // DEVICE [ntiles]: != 0 marks a tile that needs per-sample weights
   int* list;      // DEVICE [1 + ntiles]: count, then the flagged tiles
+  int plan_tiles; // tiles of the plan (the whole series)
   int fixup_grid; // CTAs of the fix-up kernel (2 per SM)
   void* side;     // cudaStream_t owned by the handle: the fix-up kernel runs there, beside the apply kernel
   void* fork;     // cudaEvent_t: the caller's stream reached the plan

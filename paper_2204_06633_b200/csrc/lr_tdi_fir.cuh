@@ -278,7 +278,8 @@ tdi_fir_setup_kernel(const Params prm, double* __restrict__ plan, int* __restric
   const int tile = blockIdx.x;
   const int n0 = tile * B;
   const int Wc = prm.fir_wc;
-  if (n0 + B <= prm.m_front || n0 >= prm.n - prm.m_back) {   // tile entirely inside a margin: never applied
+  // (the plan is always built for the whole series: prm.n_off = 0, tiles are global)
+  if (n0 + B <= prm.m_front || n0 >= prm.n_glob - prm.m_back) {   // tile entirely inside a margin: never applied
     if (tid == 0) flags[tile] = 0;
     return;
   }
@@ -330,33 +331,35 @@ tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __r
   double* res = K + fir_plan_doubles_per_tile(Wc);
 
   const int tid = threadIdx.x;
-  const int tile = blockIdx.x / batch;
+  const int tile = blockIdx.x / batch;                       // local tile: local samples [n0, n0 + B)
   const int64_t b = blockIdx.x - (int64_t)tile * batch;
   const int n0 = tile * B;
   const int g0 = n0 - prm.halo_lo;
-  const int64_t N = prm.n;
+  const int tile_g = tile + prm.n_off / B;                   // global tile (prm.n_off is a multiple of B)
+  const int n0g = prm.n_off + n0;
+  const int64_t N = prm.out_stride;
   const int nout = channels == 2 ? 6 : 3;
   double* ob = out + b * nout * N;
 
-  const int v_lo = prm.m_front, v_hi = prm.n - prm.m_back;   // valid samples [v_lo, v_hi)
-  if (n0 + B <= v_lo || n0 >= v_hi) {                        // tile entirely inside a margin
+  const int v_lo = prm.m_front, v_hi = prm.n_glob - prm.m_back;   // valid global samples [v_lo, v_hi)
+  if (n0g + B <= v_lo || n0g >= v_hi) {                      // tile entirely inside a margin
     for (int i = tid; i < B; i += kFirThreads)
       if (n0 + i < prm.n)
         for (int c = 0; c < nout; ++c) ob[(int64_t)c * N + n0 + i] = 0.0;
     return;
   }
-  if (flags[tile] != 0) return;                              // exact per-sample tile: the fix-up kernel's
+  if (flags[tile_g] != 0) return;                            // exact per-sample tile: the fix-up kernel's
 
   // first differences straight from global memory (the second load of each pair hits L1)
-  const double* yb = y + b * 6 * N;
+  const double* yb = y + b * 6 * prm.in_stride;
   for (int m = tid; m < 6 * W; m += kFirThreads) {
     const int s = m / W, g = g0 + (m - s * W);
-    const double* ys = yb + (int64_t)s * N;
-    const double a = (g >= 0 && g < prm.n) ? __ldg(ys + g) : 0.0;
-    const double c = (g + 1 >= 0 && g + 1 < prm.n) ? __ldg(ys + g + 1) : 0.0;
+    const double* ys = yb + s * prm.in_stride;
+    const double a = (g >= prm.rd_lo && g < prm.rd_hi) ? __ldg(ys + g) : 0.0;
+    const double c = (g + 1 >= prm.rd_lo && g + 1 < prm.rd_hi) ? __ldg(ys + g + 1) : 0.0;
     dif[m] = c - a;
   }
-  const double2* src = reinterpret_cast<const double2*>(plan + (size_t)tile * fir_plan_doubles_per_tile(Wc));
+  const double2* src = reinterpret_cast<const double2*>(plan + (size_t)tile_g * fir_plan_doubles_per_tile(Wc));
   double2* dst = reinterpret_cast<double2*>(K);
   const int cnt = (int)(fir_plan_doubles_per_tile(Wc) / 2);
   for (int m = tid; m < cnt; m += kFirThreads) dst[m] = __ldg(src + m);
@@ -366,7 +369,7 @@ tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __r
   for (int i = tid; i < B; i += kFirThreads) {
     const int n = n0 + i;
     if (n >= prm.n) break;
-    const bool valid = n >= v_lo && n < v_hi;
+    const bool valid = n0g + i >= v_lo && n0g + i < v_hi;
     fir_store(ob, N, n, channels, valid ? res[i] : 0.0, valid ? res[B + i] : 0.0, valid ? res[2 * B + i] : 0.0);
   }
 }
@@ -385,19 +388,21 @@ tdi_fir_fixup_kernel(const Params prm, const double* __restrict__ y, double* __r
   double* raw = reinterpret_cast<double*>(smem_raw);
   double* dif = raw + 6 * W;
   const int tid = threadIdx.x;
-  const int64_t N = prm.n;
+  const int64_t N = prm.out_stride;
   const int nout = channels == 2 ? 6 : 3;
-  const int v_lo = prm.m_front, v_hi = prm.n - prm.m_back;
+  const int v_lo = prm.m_front, v_hi = prm.n_glob - prm.m_back;
+  const int tile_lo = prm.n_off / B, ntl = (prm.n + B - 1) / B;   // this launch covers global tiles [tile_lo, tile_lo + ntl)
   const int64_t items = (int64_t)list[0] * batch;
   for (int64_t w = blockIdx.x; w < items; w += gridDim.x) {
-    const int tile = list[1 + (int)(w / batch)];
+    const int tile = list[1 + (int)(w / batch)] - tile_lo;      // local tile
+    if (tile < 0 || tile >= ntl) continue;                      // (block-uniform)
     const int64_t b = w % batch;
     const int n0 = tile * B, g0 = n0 - prm.halo_lo;
-    const double* yb = y + b * 6 * N;
+    const double* yb = y + b * 6 * prm.in_stride;
     __syncthreads();
     for (int m = tid; m < 6 * W; m += B) {
       const int s = m / W, g = g0 + (m - s * W);
-      raw[m] = (g >= 0 && g < prm.n) ? __ldg(yb + (int64_t)s * N + g) : 0.0;
+      raw[m] = (g >= prm.rd_lo && g < prm.rd_hi) ? __ldg(yb + s * prm.in_stride + g) : 0.0;
     }
     __syncthreads();
     for (int m = tid; m < 6 * W; m += B) {
@@ -405,10 +410,10 @@ tdi_fir_fixup_kernel(const Params prm, const double* __restrict__ y, double* __r
       dif[m] = (ww < W - 1) ? raw[m + 1] - raw[m] : 0.0;
     }
     __syncthreads();
-    const int n = n0 + tid;
+    const int n = n0 + tid, ng = prm.n_off + n;
     if (n < prm.n) {
       double xyz[3] = {0.0, 0.0, 0.0};
-      if (n >= v_lo && n < v_hi) tdi_sample<PT, GEN>(prm, raw, dif, W, prm.halo_lo + tid, sample_trel(prm, n), xyz);
+      if (ng >= v_lo && ng < v_hi) tdi_sample<PT, GEN>(prm, raw, dif, W, prm.halo_lo + tid, sample_trel(prm, ng), xyz);
       fir_store(out + b * nout * N, N, n, channels, xyz[0], xyz[1], xyz[2]);
     }
   }

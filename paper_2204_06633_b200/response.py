@@ -74,6 +74,16 @@ class Response:
             out = torch.empty((b, self.n_out, n), dtype=torch.float64, device=y.device)
         return B.lr_tdi(self._h, y, out, b, stream)
 
+    def response(self, h_plus, h_cross, beta, lam, psi, out=None, tdi=None, stream=None):
+        """h -> out on the device without a [B,6,N] array (lr_response)."""
+        import torch
+        h_plus = h_plus.reshape(-1, h_plus.shape[-1])
+        b, n = h_plus.shape
+        t = tdi or self
+        if out is None:
+            out = torch.empty((b, t.n_out, n), dtype=torch.float64, device=h_plus.device)
+        return B.lr_response(self._h, t._h, h_plus, h_cross, beta, lam, psi, out, stream)
+
     def response_host(self, h_plus, h_cross, beta, lam, psi, out, tdi=None, stream=None):
         return B.lr_response_host(self._h, (tdi or self)._h, h_plus, h_cross, beta, lam, psi, out, stream)
 

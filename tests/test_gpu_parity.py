@@ -282,6 +282,39 @@ def test_gpu_hybrid_same_handle_bitwise(lr):
     assert np.array_equal(out, a)
 
 
+@pytest.mark.parametrize("tdi_path", ["auto", "per_sample", "fir4"])
+def test_gpu_response_chunked_bitwise(lr, tdi_path):
+    """lr_response (device, chunked through the small y scratch) and lr_response_host (pipelined copies) equal
+    lr_project + lr_tdi bit for bit: 11 templates (two template chunks), 30,011 samples in chunks of 7,168
+    (ragged last chunk), and the automatic single-chunk case; hybrid second handle included."""
+    import torch
+    w = inputs.config(3, batch=11, n=30011)
+    tab = w.table()
+    hp, hc = _stack(w, range(11))
+    beta, lam, psi = ([getattr(s, k) for s in w.sources] for k in ("beta", "lam", "psi"))
+    eq = inputs.orbit_table("eq", w.t0, w.t0 + w.n * w.dt, const_ltt=inputs.ARM / inputs.C_LIGHT)
+    R = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="XYZ_AET", tdi_path=tdi_path)
+    R1 = lr.Response(eq, w.dt, w.order, 1, t0=w.t0, channels="AET", tdi_path=tdi_path)
+    hpd, hcd = to_dev(hp), to_dev(hc)
+    y = R.project(hpd, hcd, beta, lam, psi)
+    for Rt in (R, R1):
+        ref = Rt.tdi(y).cpu().numpy()
+        for chunk in (0, 7168, 1792):
+            lr.lr_set_option(R.handle, lr.LR_OPT_CHUNK_SAMPLES, chunk)
+            got = R.response(hpd, hcd, beta, lam, psi, tdi=Rt)
+            torch.cuda.synchronize()
+            assert np.array_equal(got.cpu().numpy(), ref), (tdi_path, chunk)
+            out = torch.empty(ref.shape, dtype=torch.float64).pin_memory()
+            R.response_host(torch.from_numpy(hp).pin_memory(), torch.from_numpy(hc).pin_memory(), beta, lam, psi, out,
+                            tdi=Rt)
+            assert np.array_equal(out.numpy(), ref), (tdi_path, chunk, "host")
+    # pageable host buffers work too
+    lr.lr_set_option(R.handle, lr.LR_OPT_CHUNK_SAMPLES, 7168)
+    out = np.empty((11, 6, w.n))
+    R.response_host(hp.copy(), hc.copy(), beta, lam, psi, out)
+    assert np.array_equal(out, R.tdi(y).cpu().numpy())
+
+
 def test_gpu_orbit_spline_matches_oracle(lr):
     """Orbit ingestion (lr_create's device spline) against the oracle's spline and scipy's not-a-knot
     CubicSpline at random times: positions to 1e-15 relative, light times to 1e-15 s."""
