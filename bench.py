@@ -300,6 +300,23 @@ def run_gpu(args, rank, world, local_rank):
     wall = time.perf_counter() - wall0
     launches = lr.lr_launch_count() - launches0
     ms_proj, ms_tdi = float(np.mean(tps)), float(np.mean(tts))
+    # lr_response: the same step as ONE call, in time chunks through the small L2-resident y scratch
+    ms_resp = None
+    if batch == 1:
+        hp1, hc1 = chunk_inputs(0, 1)
+        be1, la1, ps1 = angles(0, 1)
+        for _ in range(2):
+            R.response(hp1, hc1, be1, la1, ps1, out=out[:1])
+        tr = []
+        for _ in range(max(3, min(args.steps, 20))):
+            flush.zero_()
+            e0, e1 = ev(), ev()
+            e0.record(stream)
+            R.response(hp1, hc1, be1, la1, ps1, out=out[:1])
+            e1.record(stream)
+            e1.synchronize()
+            tr.append(e0.elapsed_time(e1))
+        ms_resp = float(np.mean(tr))
     # the same steps with the FIR plan rebuilt by every lr_tdi call (plan kernel inside the timed region)
     R.set_plan_cache(False)
     cold = [step(True) for _ in range(max(3, min(args.steps, 10)))]
@@ -369,6 +386,7 @@ def run_gpu(args, rank, world, local_rank):
                                    "frac_fp64": ach_proj / peak, "alg_GBps": BYTES_PROJECT * batch * n / (ms_proj * 1e6)},
                     "lr_tdi": {"ms": ms_tdi, "alg_ops_per_sample": ops_t, "gops": ach_tdi / 1e9,
                                "frac_fp64": ach_tdi / peak, "alg_GBps": bytes_tdi(nout) * batch * n / (ms_tdi * 1e6)}},
+        "lr_response": {"ms_per_step": ms_resp, "note": "one call, h -> out, y only in a <= 40 MB scratch"},
         "tdi_plan": {"cached_between_calls": True, "ms_tdi_with_plan_rebuilt_every_call": ms_tdi_cold,
                      "value_with_plan_rebuilt_every_call": units / (max_over_ranks(ms_proj + ms_tdi_cold) * 1e-3)
                      if world == 1 else None},

@@ -72,6 +72,7 @@ struct lr_handle {
   double* o_buf = nullptr; size_t o_cap = 0;
   cudaStream_t s_in = nullptr, s_out = nullptr;
   cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
+  cudaEvent_t ev_fix[2] = {nullptr, nullptr};       // fix-up kernel of the chunk in y slot 0 / 1 finished
   int last_cuda = 0;
 
   int64_t m_proj() const {
@@ -236,6 +237,7 @@ void lr_destroy(lr_handle* h) {
     if (h->ev_in[i]) cudaEventDestroy(h->ev_in[i]);
     if (h->ev_comp[i]) cudaEventDestroy(h->ev_comp[i]);
     if (h->ev_out[i]) cudaEventDestroy(h->ev_out[i]);
+    if (h->ev_fix[i]) cudaEventDestroy(h->ev_fix[i]);
   }
   if (h->s_in) cudaStreamDestroy(h->s_in);
   if (h->s_out) cudaStreamDestroy(h->s_out);
@@ -334,12 +336,15 @@ TdiShape tdi_shape(const lr_handle* h) {
   return t;
 }
 
-int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, double* out, void* stream) {
+// join_later: if non-null and the FIR path runs, the fix-up kernel's completion is recorded there and the
+// caller's stream does NOT wait for it (set to nullptr by the per-sample path, which has no fix-up kernel).
+int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, double* out, void* stream,
+               cudaEvent_t* join_later = nullptr) {
   lr::Params P = make_params(h, w.n_glob);
   const TdiShape ts = tdi_shape(h);
   const int path = ts.path;
   cudaStream_t st = (cudaStream_t)stream;
-  lr::FirPlanArgs pa{nullptr, nullptr, nullptr, 0, 0, nullptr, nullptr, nullptr, false};
+  lr::FirPlanArgs pa{nullptr, nullptr, nullptr, 0, 0, nullptr, nullptr, nullptr, true, false};
   P.halo_lo = ts.halo_lo; P.halo_hi = ts.halo_hi; P.fir_wc = ts.wc;
   if (path != LR_TDI_PER_SAMPLE) {
     if (w.off % lr::kFirTile != 0) return LR_EINVAL;   // windows of the FIR path start on a tile
@@ -379,9 +384,11 @@ int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, do
       LR_CUDA(h, cudaEventCreateWithFlags(&pl.join, cudaEventDisableTiming));
     }
     pa.side = pl.side; pa.fork = pl.fork; pa.join = pl.join;
+    if (join_later) { pa.join = *join_later; pa.wait_join = false; }
     apply_window(P, w);
     P.ntiles = (int)((w.n + lr::kFirTile - 1) / lr::kFirTile);
   } else {
+    if (join_later) *join_later = nullptr;
     apply_window(P, w);
     P.ntiles = (int)((w.n + lr::kTdiThreads - 1) / lr::kTdiThreads);
   }
@@ -456,16 +463,24 @@ int ensure(lr_handle* h, double** buf, size_t* cap, size_t need) {
 // out_chunk: DEVICE rows of stride o_stride whose element 0 is global sample a.
 int response_chunk(lr_handle* hp_, lr_handle* ht_, const TdiShape& ts, const double* hp, const double* hc,
                    int64_t h_a, int64_t h_b, int64_t h_stride, const double* basis_dev, int64_t nb, int64_t n,
-                   int64_t a, int64_t b, int64_t ly, double* out_chunk, int64_t o_stride, void* stream) {
+                   int64_t a, int64_t b, int64_t ly, double* out_chunk, int64_t o_stride, void* stream,
+                   double* y_slot, cudaEvent_t* fix_done) {
   const int64_t ya = a - ts.halo_lo > 0 ? a - ts.halo_lo : 0;
   const int64_t yb = b + ts.halo_hi < n ? b + ts.halo_hi : n;
   const Window wp{n, ya, yb - ya, h_a, h_b, h_stride, ly};
-  int rc = project_window(hp_, hp + (ya - h_a), hc + (ya - h_a), basis_dev, nb, wp, hp_->y_scr, stream);
+  int rc = project_window(hp_, hp + (ya - h_a), hc + (ya - h_a), basis_dev, nb, wp, y_slot, stream);
   if (rc != LR_OK) return rc;
   const Window wt{n, a, b - a, ya, yb, ly, o_stride};
-  rc = tdi_window(ht_, hp_->y_scr + (a - ya), nb, wt, out_chunk, stream);
+  rc = tdi_window(ht_, y_slot + (a - ya), nb, wt, out_chunk, stream, fix_done);
   if (rc != LR_OK) hp_->last_cuda = ht_->last_cuda;
   return rc;
+}
+
+// the two y slots alternate between chunks; a slot is rewritten only after the fix-up kernel that read it
+int ensure_fix_events(lr_handle* h) {
+  for (int i = 0; i < 2; ++i)
+    if (!h->ev_fix[i]) LR_CUDA(h, cudaEventCreateWithFlags(&h->ev_fix[i], cudaEventDisableTiming));
+  return LR_OK;
 }
 
 int64_t round_up(int64_t v, int64_t u) { return (v + u - 1) / u * u; }
@@ -492,22 +507,30 @@ int lr_response(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const doub
   if (h->chunk_samples > 0) lc = round_up(h->chunk_samples, kChunkUnit);
   if (lc > round_up(n, kChunkUnit)) lc = round_up(n, kChunkUnit);
   const int64_t ly = round_up(lc + ts.halo_lo + ts.halo_hi, 2);
-  rc = ensure(h, &h->y_scr, &h->y_cap, (size_t)(bc * 6 * ly));
+  rc = ensure(h, &h->y_scr, &h->y_cap, (size_t)(2 * bc * 6 * ly));
+  if (rc == LR_OK) rc = ensure_fix_events(h);
   if (rc != LR_OK) return rc;
+  cudaEvent_t pending[2] = {nullptr, nullptr};   // fix-up kernels still reading y slot 0 / 1
+  int64_t c = 0;
   for (int64_t b0 = 0; b0 < batch; b0 += bc) {
     const int64_t nb = batch - b0 < bc ? batch - b0 : bc;
     Stage* S = nullptr;
     rc = stage_basis(h, beta + b0, lam + b0, psi + b0, nb, st, &S);
     if (rc != LR_OK) return rc;
-    for (int64_t a = 0; a < n; a += lc) {
+    for (int64_t a = 0; a < n; a += lc, ++c) {
+      const int slot = (int)(c & 1);
       const int64_t b = a + lc < n ? a + lc : n;
+      if (pending[slot]) LR_CUDA(h, cudaStreamWaitEvent(st, pending[slot], 0));
+      pending[slot] = h->ev_fix[slot];
       rc = response_chunk(h, ht_, ts, h_plus + b0 * n, h_cross + b0 * n, 0, n, n, S->dev, nb, n, a, b, ly,
-                          out + b0 * nout * n + a, n, stream);
+                          out + b0 * nout * n + a, n, stream, h->y_scr + (size_t)slot * bc * 6 * ly, &pending[slot]);
       if (rc != LR_OK) return rc;
     }
     LR_CUDA(h, cudaEventRecord(S->done, st));
     S->pending = true;
   }
+  for (int i = 0; i < 2; ++i)   // join the last fix-up kernels
+    if (pending[i]) LR_CUDA(h, cudaStreamWaitEvent(st, pending[i], 0));
   return LR_OK;
 }
 
@@ -532,7 +555,8 @@ int lr_response_host(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const
   if (h->chunk_samples > 0) lc = round_up(h->chunk_samples, kChunkUnit);
   const int64_t ly = round_up(lc + ts.halo_lo + ts.halo_hi, 2);
   const int64_t lh = ly + 2 * mp;
-  rc = ensure(h, &h->y_scr, &h->y_cap, (size_t)(bc * 6 * ly));
+  rc = ensure(h, &h->y_scr, &h->y_cap, (size_t)(2 * bc * 6 * ly));
+  if (rc == LR_OK) rc = ensure_fix_events(h);
   if (rc == LR_OK) rc = ensure(h, &h->h_buf, &h->h_cap, (size_t)(2 * 2 * bc * lh));
   if (rc == LR_OK) rc = ensure(h, &h->o_buf, &h->o_cap, (size_t)(2 * bc * nout * lc));
   if (rc != LR_OK) return rc;
@@ -550,6 +574,7 @@ int lr_response_host(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const
   LR_CUDA(h, cudaStreamWaitEvent(h->s_in, h->ev_comp[0], 0));
   LR_CUDA(h, cudaStreamWaitEvent(h->s_out, h->ev_comp[0], 0));
   int64_t c = 0;
+  cudaEvent_t pending[2] = {nullptr, nullptr};   // fix-up kernels still reading y slot 0 / 1
   const size_t dsz = sizeof(double);
   for (int64_t b0 = 0; b0 < batch; b0 += bc) {
     const int64_t nb = batch - b0 < bc ? batch - b0 : bc;
@@ -574,11 +599,15 @@ int lr_response_host(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const
       // stage 2: kernels (the D2H of chunk c-2 must be done with this slot's out buffer)
       LR_CUDA(h, cudaStreamWaitEvent(st, h->ev_in[slot], 0));
       if (c >= 2) LR_CUDA(h, cudaStreamWaitEvent(st, h->ev_out[slot], 0));
-      rc = response_chunk(h, ht_, ts, hp_d, hc_d, ha, hb, lh, S->dev, nb, n, a, b, ly, o_d, lc, stream);
+      if (pending[slot]) LR_CUDA(h, cudaStreamWaitEvent(st, pending[slot], 0));
+      pending[slot] = h->ev_fix[slot];
+      rc = response_chunk(h, ht_, ts, hp_d, hc_d, ha, hb, lh, S->dev, nb, n, a, b, ly, o_d, lc, stream,
+                          h->y_scr + (size_t)slot * bc * 6 * ly, &pending[slot]);
       if (rc != LR_OK) return rc;
       LR_CUDA(h, cudaEventRecord(h->ev_comp[slot], st));
-      // stage 3: D2H
+      // stage 3: D2H (after the chunk's kernels, the fix-up kernel on its side stream included)
       LR_CUDA(h, cudaStreamWaitEvent(h->s_out, h->ev_comp[slot], 0));
+      if (pending[slot]) LR_CUDA(h, cudaStreamWaitEvent(h->s_out, pending[slot], 0));
       for (int ch = 0; ch < nout; ++ch)   // rows [template][channel]: one 2-D copy per channel
         LR_CUDA(h, cudaMemcpy2DAsync(out + (b0 * nout + ch) * n + a, (size_t)nout * n * dsz, o_d + (size_t)ch * lc,
                                      (size_t)nout * lc * dsz, (b - a) * dsz, nb, cudaMemcpyDeviceToHost, h->s_out));

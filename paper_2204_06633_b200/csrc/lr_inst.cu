@@ -85,7 +85,7 @@ static int launch_tdi_fir(const Params& prm, int channels, const double* y, doub
                                                                     (int)batch);
   g_launches.fetch_add(1);
   if ((e = cudaGetLastError()) != cudaSuccess) return (int)e;
-  return (int)cudaStreamWaitEvent(st, (cudaEvent_t)plan.join, 0);   // join
+  return plan.wait_join ? (int)cudaStreamWaitEvent(st, (cudaEvent_t)plan.join, 0) : 0;   // join
 }
 
 template <int PT>

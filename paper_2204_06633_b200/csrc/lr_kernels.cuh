@@ -144,6 +144,8 @@ struct FirPlanArgs {
   void* side;     // cudaStream_t owned by the handle: the fix-up kernel runs there, beside the apply kernel
   void* fork;     // cudaEvent_t: the caller's stream reached the plan
   void* join;     // cudaEvent_t: the fix-up kernel finished
+  bool wait_join; // true: the caller's stream waits for `join` before the launcher returns; false: the caller
+                  // orders later work after `join` itself (chunked response: the next chunk overlaps the fix-up)
   bool build;
 };
 
