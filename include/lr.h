@@ -21,6 +21,8 @@
  *     and return without synchronising.  lr_response_host is synchronous.
  *   - all entry points return 0 on success or a negative LR_E* code; they never abort, throw or print.
  *     Inputs are not scanned for NaN (NaN propagates).
+ *   - a handle keeps per-call staging state (and lr_tdi's plan): use one handle from one host thread and one
+ *     stream at a time; different handles are independent.
  *   - there is no CPU fallback: every call that computes needs a CUDA device and fails with LR_ECUDA
  *     otherwise.
  */

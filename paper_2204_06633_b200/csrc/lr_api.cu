@@ -310,10 +310,10 @@ int project_window(lr_handle* h, const double* hp, const double* hc, const doubl
 }
 
 // which lr_tdi path this handle takes, and the staged halo of that path's kernels
-struct TdiShape { int path, wc, halo_lo, halo_hi; };
+struct TdiShape { int path, wc, taps, halo_lo, halo_hi; };
 
 TdiShape tdi_shape(const lr_handle* h) {
-  TdiShape t{h->tdi_path, 0, 0, 0};
+  TdiShape t{h->tdi_path, 0, 0, 0, 0};
   const int64_t mf = h->m_front(h->gen);
   // per-tile polynomial FIR when the delays drift slowly enough, else exact per-sample weights
   const int nlinks = h->gen == 1 ? 3 : 7;  // links in the longest delayed term
@@ -321,7 +321,8 @@ TdiShape tdi_shape(const lr_handle* h) {
   if (t.path == LR_TDI_AUTO) t.path = de <= 6e-6 ? LR_TDI_FIR3 : de <= 1.5e-4 ? LR_TDI_FIR4 : LR_TDI_PER_SAMPLE;
   if (t.path != LR_TDI_PER_SAMPLE) {
     const int imax = (int)h->tdi_reach(h->gen);
-    t.wc = ((imax + 2 * h->p - 2 + lr::kFirR - 1) / lr::kFirR) * lr::kFirR;
+    t.taps = imax + 2 * h->p - 2;
+    t.wc = ((t.taps + lr::kFirR - 1) / lr::kFirR) * lr::kFirR;
     const int back = t.wc - (h->p - 1);
     t.halo_lo = back > (int)(mf - h->m_proj()) ? back : (int)(mf - h->m_proj());
     t.halo_hi = h->p + lr::kFirR;
@@ -345,7 +346,7 @@ int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, do
   const int path = ts.path;
   cudaStream_t st = (cudaStream_t)stream;
   lr::FirPlanArgs pa{nullptr, nullptr, nullptr, 0, 0, nullptr, nullptr, nullptr, true, false};
-  P.halo_lo = ts.halo_lo; P.halo_hi = ts.halo_hi; P.fir_wc = ts.wc;
+  P.halo_lo = ts.halo_lo; P.halo_hi = ts.halo_hi; P.fir_wc = ts.wc; P.fir_taps = ts.taps;
   if (path != LR_TDI_PER_SAMPLE) {
     if (w.off % lr::kFirTile != 0) return LR_EINVAL;   // windows of the FIR path start on a tile
     // the plan always covers the whole series (global tiles)

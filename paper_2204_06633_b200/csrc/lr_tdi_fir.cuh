@@ -203,11 +203,12 @@ LR_HD void fir_merge(const Params& prm, const FirTile<GEN, NN>& T, const double*
 }
 
 // E: apply.  One work item = kFirR consecutive samples of one channel.  dif: [6][W]; res: [3][B] (tile
-// staging of X, Y, Z).  nl0 = staged index of the tile's first sample; Wc is a multiple of kFirR.
+// staging of X, Y, Z).  nl0 = staged index of the tile's first sample; Wc is a multiple of kFirR and the
+// first `pad` taps of every series are zero padding.
 // Per tap the coefficient is evaluated at each sample's own tau (Horner over the NN powers) and applied to
 // the sliding window of first differences: NN FMAs per (tap, sample), one accumulator per sample.
 template <int NN>
-LR_HD void fir_apply(const double* dif, int W, const double* K, int Wc, int P, int nl0, int B, double* res,
+LR_HD void fir_apply(const double* dif, int W, const double* K, int Wc, int pad, int P, int nl0, int B, double* res,
                      int tid, int nthreads) {
   constexpr int R = kFirR;
   const int groups = (B + R - 1) / R;
@@ -230,8 +231,10 @@ LR_HD void fir_apply(const double* dif, int W, const double* K, int Wc, int P, i
       for (int m0 = 0; m0 < Wc; m0 += R) {
 #pragma unroll
         for (int r = 0; r < R; ++r) win[R + r] = d[m0 + R + r];
+        const int skip = m0 == 0 ? pad : 0;   // the first `pad` stored taps are padding (all zero)
 #pragma unroll
         for (int mm = 0; mm < R; ++mm) {
+          if (mm < skip) continue;
           double kc[NN];
 #pragma unroll
           for (int p = 0; p < NN; ++p) kc[p] = kk[(m0 + mm) * kFirKStride + p];
@@ -364,7 +367,7 @@ tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __r
   const int cnt = (int)(fir_plan_doubles_per_tile(Wc) / 2);
   for (int m = tid; m < cnt; m += kFirThreads) dst[m] = __ldg(src + m);
   __syncthreads();
-  fir_apply<NN>(dif, W, K, Wc, prm.p, prm.halo_lo, B, res, tid, kFirThreads);
+  fir_apply<NN>(dif, W, K, Wc, Wc - prm.fir_taps, prm.p, prm.halo_lo, B, res, tid, kFirThreads);
   __syncthreads();
   for (int i = tid; i < B; i += kFirThreads) {
     const int n = n0 + i;
