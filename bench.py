@@ -148,7 +148,7 @@ def _make_workload(kind, rank):
         return inputs.config(1), 1
     if kind == "4yr":
         return inputs.config(4), 1
-    if kind == "chirp":
+    if kind in ("chirp", "hybrid"):   # hybrid: config 5 run (i), TDI-1 on equal-arm constant delays
         return inputs.config(5), 1
     raise ValueError(kind)
 
@@ -218,8 +218,9 @@ def run_reference(args, rank, world):
 
 
 def workload_config(w, batch, args):
-    return {"workload": f"BASELINE.json configs[{ {'tiny': 0, 'year': 1, 'batch': 2, '4yr': 3, 'chirp': 4}[args.workload] }] ({w.name})",
-            "batch": batch, "n": w.n, "dt": w.dt, "lagrange_order": w.order, "tdi_gen": w.tdi_gen,
+    return {"workload": f"BASELINE.json configs[{ {'tiny': 0, 'year': 1, 'batch': 2, '4yr': 3, 'chirp': 4, 'hybrid': 4}[args.workload] }] ({w.name})",
+            "batch": batch, "n": w.n, "dt": w.dt, "lagrange_order": w.order,
+            "tdi_gen": 1 if args.workload == "hybrid" else w.tdi_gen,
             "chain": "nested", "channels": w.channels, "orbits": w.orbit_kind, "tdi_path": args.tdi_path,
             "l2": "flushed between steps (256 MiB memset outside the per-step event pairs)"}
 
@@ -237,6 +238,12 @@ def run_gpu(args, rank, world, local_rank):
     nout = 6 if w.channels == "XYZ_AET" else 3
     R = lr.Response(w.table(), w.dt, w.order, w.tdi_gen, t0=w.t0, chain="nested", channels=w.channels,
                     tdi_path=args.tdi_path)
+    Rt, tdi_gen = R, w.tdi_gen
+    if args.workload == "hybrid":
+        from paper_2204_06633_b200 import inputs as _inp
+        eq = _inp.orbit_table("eq", w.t0, w.t0 + w.n * w.dt, const_ltt=_inp.ARM / _inp.C_LIGHT)
+        tdi_gen = 1
+        Rt = lr.Response(eq, w.dt, w.order, 1, t0=w.t0, chain="nested", channels=w.channels, tdi_path=args.tdi_path)
     stream = torch.cuda.current_stream()
 
     y = torch.empty((chunk, 6, n), dtype=torch.float64, device=dev)
@@ -273,7 +280,7 @@ def run_gpu(args, rank, world, local_rank):
             e0.record(stream)
             R.project(hp, hc, be, la, ps, y_out=y[:hi - lo])
             e1.record(stream)
-            R.tdi(y[:hi - lo], out=out[:hi - lo])
+            Rt.tdi(y[:hi - lo], out=out[:hi - lo])
             e2.record(stream)
             if timed:
                 e2.synchronize()
@@ -310,7 +317,7 @@ def run_gpu(args, rank, world, local_rank):
             flush.zero_()
             e0, e1 = ev(), ev()
             e0.record(stream)
-            R.response(hp, hc, be, la, ps, out=out[:hi - lo])
+            R.response(hp, hc, be, la, ps, out=out[:hi - lo], tdi=Rt)
             e1.record(stream)
             e1.synchronize()
             t += e0.elapsed_time(e1)
@@ -319,9 +326,9 @@ def run_gpu(args, rank, world, local_rank):
     step_response()
     ms_resp = float(np.mean([step_response() for _ in range(max(2, min(args.steps, 20)))]))
     # the same steps with the FIR plan rebuilt by every lr_tdi call (plan kernel inside the timed region)
-    R.set_plan_cache(False)
+    Rt.set_plan_cache(False)
     cold = [step(True) for _ in range(max(3, min(args.steps, 10)))]
-    R.set_plan_cache(True)
+    Rt.set_plan_cache(True)
     step(False)
     torch.cuda.synchronize()
     ms_tdi_cold = float(np.mean([b for _, b in cold]))
@@ -340,7 +347,7 @@ def run_gpu(args, rank, world, local_rank):
     hc_h.copy_(hc_d[:eb].cpu())
     be, la, ps = angles(0, eb)
     for _ in range(max(1, min(args.warmup, 3))):
-        R.response_host(hp_h, hc_h, be, la, ps, out_h)
+        R.response_host(hp_h, hc_h, be, la, ps, out_h, tdi=Rt)
     torch.cuda.synchronize()
     barrier()
     e2e_ms = []
@@ -349,7 +356,7 @@ def run_gpu(args, rank, world, local_rank):
         torch.cuda.synchronize()
         e0, e1 = ev(), ev()
         e0.record(stream)
-        R.response_host(hp_h, hc_h, be, la, ps, out_h)
+        R.response_host(hp_h, hc_h, be, la, ps, out_h, tdi=Rt)
         e1.record(stream)
         e1.synchronize()
         e2e_ms.append(e0.elapsed_time(e1))
@@ -358,7 +365,7 @@ def run_gpu(args, rank, world, local_rank):
 
     if rank != 0:
         return
-    ops_t, ops_p = ops_tdi(T, w.tdi_gen), ops_project(T)
+    ops_t, ops_p = ops_tdi(T, tdi_gen), ops_project(T)
     ach_tdi = ops_t * batch * n / (ms_tdi * 1e-3)
     ach_proj = ops_p * batch * n / (ms_proj * 1e-3)
     dom = "lr_tdi" if ms_tdi >= ms_proj else "lr_project"
@@ -414,7 +421,7 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="year", choices=["year", "batch", "tiny", "4yr", "chirp"])
+    ap.add_argument("--workload", default="year", choices=["year", "batch", "tiny", "4yr", "chirp", "hybrid"])
     ap.add_argument("--order", type=int, default=None, help="override the Lagrange order (order sweep)")
     ap.add_argument("--chunk", type=int, default=64, help="templates per launch (batch workload)")
     ap.add_argument("--e2e-templates", type=int, default=4)

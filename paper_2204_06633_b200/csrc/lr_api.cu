@@ -55,6 +55,7 @@ struct lr_handle {
   int order = 0, p = 0, gen = 2, chain = LR_CHAIN_NESTED, channels = LR_XYZ;
   double r_max = 0, l_max = 0;
   double max_ldot = 0;   // max |dL_ij/dt| over the table (dimensionless), from the spline
+  bool const_ltt = false; // every light-time table is constant: lr_tdi's plan is one tile (NEXT-4)
   int tdi_path = -1;     // LR_OPT_TDI_PATH: -1 auto | 0 generic | 3 | 4
   int plan_cache = 1;    // LR_OPT_TDI_PLAN_CACHE
   int sm_count = 0;
@@ -182,6 +183,10 @@ int lr_create(const lr_orbits* orb, double dt, int order, int tdi_gen, lr_handle
     if (orb->ltt[k] > h->l_max) h->l_max = orb->ltt[k];
 
   lr::pair_constants(h->p, h->bk);
+  h->const_ltt = true;
+  for (int s = 0; s < 6 && h->const_ltt; ++s)
+    for (int64_t k = 1; k < nk; ++k)
+      if (orb->ltt[s * nk + k] != orb->ltt[s * nk]) { h->const_ltt = false; break; }
 
   std::vector<lr::D4> coef;
   try { coef.resize((size_t)15 * (nk - 1)); } catch (...) { delete h; return LR_ENOMEM; }
@@ -349,8 +354,12 @@ int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, do
   P.halo_lo = ts.halo_lo; P.halo_hi = ts.halo_hi; P.fir_wc = ts.wc; P.fir_taps = ts.taps;
   if (path != LR_TDI_PER_SAMPLE) {
     if (w.off % lr::kFirTile != 0) return LR_EINVAL;   // windows of the FIR path start on a tile
-    // the plan always covers the whole series (global tiles)
-    P.ntiles = (int)((w.n_glob + lr::kFirTile - 1) / lr::kFirTile);
+    // the plan covers the whole series (global tiles); with constant light times every tile has the same
+    // filters, so the plan is ONE tile (the constant-delay fast path of SURVEY.md §8(f) NEXT-4)
+    const bool uniform = h->const_ltt;
+    P.fir_uniform = uniform ? 1 : 0;
+    P.fir_tile0 = uniform ? (int)(h->m_front(h->gen) / lr::kFirTile) : 0;
+    P.ntiles = uniform ? 1 : (int)((w.n_glob + lr::kFirTile - 1) / lr::kFirTile);
     Plan& pl = h->plan;
     const bool reuse = h->plan_cache && pl.valid && pl.n == w.n_glob && pl.t0 == h->t0 && pl.gen == h->gen &&
                        pl.chain == h->chain && pl.path == path;

@@ -66,6 +66,8 @@ struct Params {
   int halo_lo, halo_hi;  // staged window = [n0 - halo_lo, n0 + B + halo_hi)
   int ntiles;
   int fir_wc;            // FIR path: taps per series as stored (padded to a multiple of kFirR)
+  int fir_uniform;       // FIR path: 1 = all light times are constant: ONE plan tile (slot 0) serves every tile
+  int fir_tile0;         // FIR path: global tile whose geometry plan slot 0 is built from
   int fir_taps;          // FIR path: taps per series that can be non-zero (<= fir_wc; the padding is at the front)
   int chain_sum;         // 0: nested delays (default), 1: eq. 20 sums of the L at t
   double bk[kPMax + 1];  // bk[k] = 1 / prod_{m != k} (k - m), m = -P+1..P, for k = 1..P

@@ -278,12 +278,13 @@ tdi_fir_setup_kernel(const Params prm, double* __restrict__ plan, int* __restric
   FirTile<GEN, NN>& T = *reinterpret_cast<FirTile<GEN, NN>*>(smem_raw);
   double* cnode = reinterpret_cast<double*>(smem_raw + ((sizeof(FirTile<GEN, NN>) + 15) / 16) * 16);
   const int tid = threadIdx.x;
-  const int tile = blockIdx.x;
+  const int slot = blockIdx.x;                      // plan slot; = the global tile unless the plan is uniform
+  const int tile = prm.fir_tile0 + slot;
   const int n0 = tile * B;
   const int Wc = prm.fir_wc;
   // (the plan is always built for the whole series: prm.n_off = 0, tiles are global)
   if (n0 + B <= prm.m_front || n0 >= prm.n_glob - prm.m_back) {   // tile entirely inside a margin: never applied
-    if (tid == 0) flags[tile] = 0;
+    if (tid == 0) flags[slot] = 0;
     return;
   }
   if (tid == 0) T.generic = 0;
@@ -292,13 +293,13 @@ tdi_fir_setup_kernel(const Params prm, double* __restrict__ plan, int* __restric
   fir_split_terms<GEN, NN>(prm, T, tid, kFirSetupThreads);
   __syncthreads();
   if (tid == 0) {
-    flags[tile] = T.generic;
+    flags[slot] = T.generic;
     if (T.generic) list[1 + atomicAdd(list, 1)] = tile;
   }
   if (T.generic) return;
   fir_node_coeffs<PT, GEN, NN>(prm, T, cnode, tid, kFirSetupThreads);
   __syncthreads();
-  fir_merge<PT, GEN, NN>(prm, T, cnode, plan + (size_t)tile * fir_plan_doubles_per_tile(Wc), Wc, tid,
+  fir_merge<PT, GEN, NN>(prm, T, cnode, plan + (size_t)slot * fir_plan_doubles_per_tile(Wc), Wc, tid,
                          kFirSetupThreads);
 }
 
@@ -351,7 +352,8 @@ tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __r
         for (int c = 0; c < nout; ++c) ob[(int64_t)c * N + n0 + i] = 0.0;
     return;
   }
-  if (flags[tile_g] != 0) return;                            // exact per-sample tile: the fix-up kernel's
+  const int slot = prm.fir_uniform ? 0 : tile_g;             // constant light times: one plan for every tile
+  if (flags[slot] != 0) return;                              // exact per-sample tile: the fix-up kernel's
 
   // first differences straight from global memory (the second load of each pair hits L1)
   const double* yb = y + b * 6 * prm.in_stride;
@@ -362,7 +364,7 @@ tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __r
     const double c = (g + 1 >= prm.rd_lo && g + 1 < prm.rd_hi) ? __ldg(ys + g + 1) : 0.0;
     dif[m] = c - a;
   }
-  const double2* src = reinterpret_cast<const double2*>(plan + (size_t)tile_g * fir_plan_doubles_per_tile(Wc));
+  const double2* src = reinterpret_cast<const double2*>(plan + (size_t)slot * fir_plan_doubles_per_tile(Wc));
   double2* dst = reinterpret_cast<double2*>(K);
   const int cnt = (int)(fir_plan_doubles_per_tile(Wc) / 2);
   for (int m = tid; m < cnt; m += kFirThreads) dst[m] = __ldg(src + m);
