@@ -458,7 +458,10 @@ int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out,
 
 namespace {
 
-constexpr int64_t kChunkUnit = 1792;   // lcm of the kernels' tile sizes (128, 224, 256)
+constexpr int64_t gcd_(int64_t a, int64_t b) { return b == 0 ? a : gcd_(b, a % b); }
+constexpr int64_t lcm_(int64_t a, int64_t b) { return a / gcd_(a, b) * b; }
+// chunks of the one-call response start on a tile of every kernel: lcm of the tile sizes (128, 224, 256) = 1792
+constexpr int64_t kChunkUnit = lcm_(lcm_(lr::kProjThreads, lr::kTdiThreads), lr::kFirTile);
 
 int ensure(lr_handle* h, double** buf, size_t* cap, size_t need) {
   if (*cap >= need) return LR_OK;

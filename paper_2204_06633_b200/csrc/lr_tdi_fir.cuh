@@ -23,7 +23,10 @@
 
 namespace lr {
 
-constexpr int kFirR = 7;          // consecutive samples per thread (odd: conflict-free 64-bit smem reads)
+#ifndef LR_FIR_R
+#define LR_FIR_R 7
+#endif
+constexpr int kFirR = LR_FIR_R;          // consecutive samples per thread (odd: conflict-free 64-bit smem reads)
 constexpr int kFirKStride = 4;    // doubles per (series, m) coefficient record (NN <= 4)
 
 // series used by channel X, in "local" order 13, 31, 12, 21; Y and Z rotate the slots
