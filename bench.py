@@ -415,6 +415,69 @@ def run_gpu(args, rank, world, local_rank):
     print(json.dumps(line), flush=True)
 
 
+def run_gpu_time_sharded(args, rank, world, local_rank):
+    """N > 1, one template split along time: every rank holds its span of h plus the halo and computes its span
+    of out with lr_response_span; no collective on the data path.  Strong scaling: value = n / max-over-ranks time."""
+    import torch
+    import paper_2204_06633_b200 as lr
+    lr.binding.lib()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    w, batch = make_workload(args.workload, 0, args.order)
+    if batch != 1:
+        raise SystemExit("--shard time needs a single-template workload")
+    s = w.sources[0]
+    R = lr.Response(w.table(), w.dt, w.order, w.tdi_gen, t0=w.t0, chain="nested", channels=w.channels,
+                    tdi_path=args.tdi_path)
+    lo, hi, unit = R.span_halo()
+    first, count, h_first, h_len = lr.shard_time(w.n, rank, world, unit, lo, hi)
+    hp, hc = w.waveform(0)
+    hps = torch.from_numpy(hp[h_first:h_first + h_len].copy()).to(dev)[None]
+    hcs = torch.from_numpy(hc[h_first:h_first + h_len].copy()).to(dev)[None]
+    out = torch.empty((1, R.n_out, max(count, 1)), dtype=torch.float64, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        if count:
+            R.response_span(hps, hcs, h_first, [s.beta], [s.lam], [s.psi], w.n, first, count, out=out[:, :, :count])
+        e1.record(stream)
+        e1.synchronize()
+        return e0.elapsed_time(e1)
+
+    for _ in range(args.warmup):
+        step()
+    peak = lr.lr_measure_fp64_peak(args.peak_seconds)
+    barrier()
+    torch.cuda.synchronize()
+    launches0 = lr.lr_launch_count()
+    with ClockSampler(local_rank) as clk:
+        ms = [step() for _ in range(args.steps)]
+        torch.cuda.synchronize()
+    barrier()
+    launches = lr.lr_launch_count() - launches0
+    ms_step = max_over_ranks(float(np.mean(ms)))
+    if rank != 0:
+        return
+    T = w.order + 1
+    ach = (ops_tdi(T, w.tdi_gen) + ops_project(T)) * w.n / (ms_step * 1e-3)
+    print(json.dumps({
+        "metric": "response samples/s (6-link proj + TDI-2, fp64)", "value": w.n / (ms_step * 1e-3),
+        "unit": "samples/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": dict(workload_config(w, 1, args), parallelism=f"{world} ranks, one template split along time "
+                       "(lr_response_span, halos recomputed, no collective)"),
+        "gpu_launches": launches, "e2e": None,
+        "roofline": {"bound": "alu", "kernel": "whole path (lr_response_span)", "achieved": ach / 1e9,
+                     "peak": world * peak / 1e9, "unit": "Gop/s (FP64 thread-instruction slots, DFMA = 1)",
+                     "frac": ach / (world * peak), "traffic": None,
+                     "peak_source": "lr_measure_fp64_peak on rank 0 x ranks"},
+        "clocks": clk.summary()}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -429,6 +492,9 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--tdi-path", default="auto", choices=["auto", "per_sample", "fir3", "fir4"])
+    ap.add_argument("--shard", default="templates", choices=["templates", "time"],
+                    help="N > 1: 'templates' = every rank its own template(s) (weak scaling, default); 'time' = ONE "
+                         "template split along time with lr_response_span (strong scaling, 'year'/'4yr'/'chirp')")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -445,7 +511,10 @@ def main():
         torch.cuda.set_device(local_rank)
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     try:
-        run_gpu(args, rank, world, local_rank)
+        if args.shard == "time" and world > 1:
+            run_gpu_time_sharded(args, rank, world, local_rank)
+        else:
+            run_gpu(args, rank, world, local_rank)
     finally:
         if world > 1:
             import torch.distributed as dist

@@ -141,6 +141,22 @@ int lr_response(lr_handle* h_proj, lr_handle* h_tdi, const double* h_plus, const
                 const double* beta, const double* lambda, const double* psi, int64_t batch, int64_t n, double* out,
                 void* cuda_stream);
 
+/* The same for a SPAN of the time axis (one long template split over several GPUs, each rank
+ * recomputing its halo instead of exchanging it — no collective).  Computes out for the global samples
+ * [first, first+count) of a series of n samples; time, margins and results are those of the whole-series
+ * call, bit for bit.  h_plus, h_cross: DEVICE [batch][h_len] holding the global samples
+ * [h_first, h_first+h_len), which must include [first - lo, first+count+hi) clipped to [0, n) with (lo, hi)
+ * from lr_get_span_halo; out: DEVICE [batch][3|6][count].  `first` must be a multiple of the span unit
+ * (lr_get_span_halo's `unit`, 1792 samples).  Errors: LR_EINVAL for a bad span or a too-short h slice, else as
+ * lr_response. */
+int lr_response_span(lr_handle* h_proj, lr_handle* h_tdi, const double* h_plus, const double* h_cross,
+                     int64_t h_first, int64_t h_len, const double* beta, const double* lambda, const double* psi,
+                     int64_t batch, int64_t n, int64_t first, int64_t count, double* out, void* cuda_stream);
+
+/* Samples of h a span needs before (lo) and after (hi) itself, and the alignment unit of `first`.  Any pointer
+ * may be NULL. */
+int lr_get_span_halo(const lr_handle* h_proj, const lr_handle* h_tdi, int64_t* lo, int64_t* hi, int64_t* unit);
+
 /* Both stages with HOST buffers: copies h_plus/h_cross [batch][n] to the device, runs lr_project on
  * `h_proj` and lr_tdi on `h_tdi` (may be the same handle), copies out [batch][3|6][n] back and waits.
  * The call is a three-stage pipeline over chunks of time: the H2D copy of the next chunk and the D2H copy of

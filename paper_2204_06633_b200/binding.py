@@ -26,7 +26,7 @@ LR_MAX_ORDER = 65
 
 # every symbol include/lr.h declares
 SYMBOLS = ("lr_create", "lr_destroy", "lr_set_option", "lr_get_margins", "lr_project", "lr_tdi",
-           "lr_response", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count",
+           "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count",
            "lr_last_cuda_error", "lr_strerror")
 
 
@@ -73,6 +73,8 @@ def lib():
     L.lr_project.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
     L.lr_tdi.argtypes = [vp, vp, i64, i64, vp, vp]
     L.lr_response.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
+    L.lr_response_span.argtypes = [vp, vp, vp, vp, i64, i64, vp, vp, vp, i64, i64, i64, i64, vp, vp]
+    L.lr_get_span_halo.argtypes = [vp, vp, pi64, pi64, pi64]
     L.lr_response_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
     L.lr_eval_orbit.argtypes = [vp, ci, vp, i64, vp, vp]
     L.lr_measure_fp64_peak.argtypes = [dbl, ctypes.POINTER(dbl)]
@@ -178,6 +180,31 @@ def lr_response(h_proj, h_tdi, h_plus, h_cross, beta, lam, psi, out, stream=None
     _check(lib().lr_response(h_proj, h_tdi, _dev_ptr(h_plus, "h_plus"), _dev_ptr(h_cross, "h_cross", B * n),
                              beta.ctypes.data, lam.ctypes.data, psi.ctypes.data, B, n, _dev_ptr(out, "out"),
                              _stream(stream)), "lr_response", h_proj)
+    return out
+
+
+def lr_get_span_halo(h_proj, h_tdi):
+    """(lo, hi, unit): h samples a span needs before / after itself, and the alignment of a span's start."""
+    a, b, c = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
+    _check(lib().lr_get_span_halo(h_proj, h_tdi, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)),
+           "lr_get_span_halo", h_proj)
+    return a.value, b.value, c.value
+
+
+def lr_response_span(h_proj, h_tdi, h_plus, h_cross, h_first, beta, lam, psi, n, first, count, out, stream=None):
+    """lr_response_span: h_plus, h_cross CUDA [B, h_len] = global samples [h_first, h_first+h_len) of a series
+    of n samples; out CUDA [B, 3|6, count] receives the global samples [first, first+count)."""
+    beta, lam, psi = _host(beta), _host(lam), _host(psi)
+    B = beta.size
+    if h_plus.numel() % B:
+        raise ValueError("h_plus size is not a multiple of the batch")
+    h_len = h_plus.numel() // B
+    if out.numel() not in (3 * B * count, 6 * B * count):
+        raise ValueError("out must be [batch,3,count] or [batch,6,count]")
+    _check(lib().lr_response_span(h_proj, h_tdi, _dev_ptr(h_plus, "h_plus"), _dev_ptr(h_cross, "h_cross", B * h_len),
+                                  int(h_first), h_len, beta.ctypes.data, lam.ctypes.data, psi.ctypes.data, B, int(n),
+                                  int(first), int(count), _dev_ptr(out, "out"), _stream(stream)),
+           "lr_response_span", h_proj)
     return out
 
 

@@ -502,15 +502,32 @@ int64_t round_up(int64_t v, int64_t u) { return (v + u - 1) / u * u; }
 
 extern "C" {
 
-int lr_response(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const double* h_cross, const double* beta,
-                const double* lam, const double* psi, int64_t batch, int64_t n, double* out, void* stream) {
+int lr_get_span_halo(const lr_handle* hp_, const lr_handle* ht_, int64_t* lo, int64_t* hi, int64_t* unit) {
+  if (!hp_ || !ht_) return LR_EINVAL;
+  const TdiShape ts = tdi_shape(ht_);
+  if (lo) *lo = ts.halo_lo + hp_->m_proj();
+  if (hi) *hi = ts.halo_hi + hp_->m_proj();
+  if (unit) *unit = kChunkUnit;
+  return LR_OK;
+}
+
+int lr_response_span(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const double* h_cross, int64_t h_first,
+                     int64_t h_len, const double* beta, const double* lam, const double* psi, int64_t batch,
+                     int64_t n, int64_t first, int64_t count, double* out, void* stream) {
   lr_handle* h = hp_;
   if (!h || !ht_ || !h_plus || !h_cross || !beta || !lam || !psi || !out) return LR_EINVAL;
   int rc = check_project(h, batch, n);
   if (rc == LR_OK) rc = check_tdi(ht_, batch, n);
   if (rc != LR_OK) return rc;
-  cudaStream_t st = (cudaStream_t)stream;
   const TdiShape ts = tdi_shape(ht_);
+  const int64_t mp = h->m_proj();
+  if (first < 0 || count < 1 || first + count > n || first % kChunkUnit != 0) return LR_EINVAL;
+  if (h_first < 0 || h_len < 1 || h_first + h_len > n) return LR_EINVAL;
+  // the h slice must hold every sample the span's kernels read: [first - halo_lo - m_proj, first+count+halo_hi+m_proj)
+  const int64_t need_a = first - ts.halo_lo - mp > 0 ? first - ts.halo_lo - mp : 0;
+  const int64_t need_b = first + count + ts.halo_hi + mp < n ? first + count + ts.halo_hi + mp : n;
+  if (h_first > need_a || h_first + h_len < need_b) return LR_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
   const int nout = ht_->channels == LR_XYZ_AET ? 6 : 3;
   // y of one chunk stays small enough to live in L2 (and bounds the footprint: no [batch][6][n] buffer)
   const int64_t bc = batch < 8 ? batch : 8;
@@ -518,7 +535,7 @@ int lr_response(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const doub
   int64_t lc = budget / kChunkUnit * kChunkUnit;
   if (lc < 4 * kChunkUnit) lc = 4 * kChunkUnit;
   if (h->chunk_samples > 0) lc = round_up(h->chunk_samples, kChunkUnit);
-  if (lc > round_up(n, kChunkUnit)) lc = round_up(n, kChunkUnit);
+  if (lc > round_up(count, kChunkUnit)) lc = round_up(count, kChunkUnit);
   const int64_t ly = round_up(lc + ts.halo_lo + ts.halo_hi, 2);
   rc = ensure(h, &h->y_scr, &h->y_cap, (size_t)(2 * bc * 6 * ly));
   if (rc == LR_OK) rc = ensure_fix_events(h);
@@ -530,13 +547,14 @@ int lr_response(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const doub
     Stage* S = nullptr;
     rc = stage_basis(h, beta + b0, lam + b0, psi + b0, nb, st, &S);
     if (rc != LR_OK) return rc;
-    for (int64_t a = 0; a < n; a += lc, ++c) {
+    for (int64_t a = first; a < first + count; a += lc, ++c) {
       const int slot = (int)(c & 1);
-      const int64_t b = a + lc < n ? a + lc : n;
+      const int64_t b = a + lc < first + count ? a + lc : first + count;
       if (pending[slot]) LR_CUDA(h, cudaStreamWaitEvent(st, pending[slot], 0));
       pending[slot] = h->ev_fix[slot];
-      rc = response_chunk(h, ht_, ts, h_plus + b0 * n, h_cross + b0 * n, 0, n, n, S->dev, nb, n, a, b, ly,
-                          out + b0 * nout * n + a, n, stream, h->y_scr + (size_t)slot * bc * 6 * ly, &pending[slot]);
+      rc = response_chunk(h, ht_, ts, h_plus + b0 * h_len, h_cross + b0 * h_len, h_first, h_first + h_len, h_len,
+                          S->dev, nb, n, a, b, ly, out + b0 * nout * count + (a - first), count, stream,
+                          h->y_scr + (size_t)slot * bc * 6 * ly, &pending[slot]);
       if (rc != LR_OK) return rc;
     }
     LR_CUDA(h, cudaEventRecord(S->done, st));
@@ -545,6 +563,11 @@ int lr_response(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const doub
   for (int i = 0; i < 2; ++i)   // join the last fix-up kernels
     if (pending[i]) LR_CUDA(h, cudaStreamWaitEvent(st, pending[i], 0));
   return LR_OK;
+}
+
+int lr_response(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const double* h_cross, const double* beta,
+                const double* lam, const double* psi, int64_t batch, int64_t n, double* out, void* stream) {
+  return lr_response_span(hp_, ht_, h_plus, h_cross, 0, n, beta, lam, psi, batch, n, 0, n, out, stream);
 }
 
 int lr_response_host(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const double* h_cross, const double* beta,

@@ -19,6 +19,20 @@ def shard_templates(batch, rank, world):
     return lo, lo + base + (1 if rank < extra else 0)
 
 
+def shard_time(n, rank, world, unit, lo, hi):
+    """Span [first, first+count) of a series of n samples owned by `rank` of `world`, with starts on multiples of
+    `unit`, and the slice [h_first, h_first+h_len) of h that rank must hold (its span plus the halo (lo, hi) of
+    lr_get_span_halo, clipped to the series).  The spans partition [0, n); no collective is needed (SURVEY.md
+    §8(e): halos are recomputed, not exchanged).  Ranks beyond the number of units get count = 0."""
+    if world < 1 or not 0 <= rank < world or n < 1 or unit < 1:
+        raise ValueError("bad shard arguments")
+    units = -(-n // unit)
+    a, b = shard_templates(units, rank, world)
+    first, end = min(a * unit, n), min(b * unit, n)
+    h_first, h_end = max(0, first - lo), min(n, end + hi)
+    return first, end - first, h_first, (h_end - h_first if end > first else 0)
+
+
 class Response:
     """One orbit table + (dt, order, TDI generation): owns an lr_handle."""
 
@@ -83,6 +97,18 @@ class Response:
         if out is None:
             out = torch.empty((b, t.n_out, n), dtype=torch.float64, device=h_plus.device)
         return B.lr_response(self._h, t._h, h_plus, h_cross, beta, lam, psi, out, stream)
+
+    def span_halo(self, tdi=None):
+        return B.lr_get_span_halo(self._h, (tdi or self)._h)
+
+    def response_span(self, h_plus, h_cross, h_first, beta, lam, psi, n, first, count, out=None, tdi=None, stream=None):
+        """out[B, n_out, count] for the global samples [first, first+count) from the h slice starting at h_first."""
+        import torch
+        t = tdi or self
+        h_plus = h_plus.reshape(-1, h_plus.shape[-1])
+        if out is None:
+            out = torch.empty((h_plus.shape[0], t.n_out, count), dtype=torch.float64, device=h_plus.device)
+        return B.lr_response_span(self._h, t._h, h_plus, h_cross, h_first, beta, lam, psi, n, first, count, out, stream)
 
     def response_host(self, h_plus, h_cross, beta, lam, psi, out, tdi=None, stream=None):
         return B.lr_response_host(self._h, (tdi or self)._h, h_plus, h_cross, beta, lam, psi, out, stream)

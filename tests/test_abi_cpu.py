@@ -111,11 +111,30 @@ def test_shard_templates_is_a_partition():
         shard_templates(4, 2, 2)
 
 
+def test_shard_time_is_a_partition_with_halos():
+    from paper_2204_06633_b200 import shard_time
+    unit, lo, hi = 1792, 90, 87
+    for n in (1, 1791, 1792, 10640, 3153600):
+        for world in (1, 2, 3, 8):
+            spans = [shard_time(n, r, world, unit, lo, hi) for r in range(world)]
+            pos = 0
+            for first, count, h_first, h_len in spans:
+                if count == 0:
+                    assert h_len == 0
+                    continue
+                assert first == pos and first % unit == 0
+                assert h_first == max(0, first - lo) and h_first + h_len == min(n, first + count + hi)
+                pos = first + count
+            assert pos == n
+    with pytest.raises(ValueError):
+        shard_time(10, 3, 2, unit, lo, hi)
+
+
 _GLOO_WORKER = r'''
 import os, sys
 sys.path.insert(0, sys.argv[1])
 import torch, torch.distributed as dist
-from paper_2204_06633_b200 import shard_templates
+from paper_2204_06633_b200 import shard_templates, shard_time
 import bench
 dist.init_process_group("gloo")
 rank, world = dist.get_rank(), dist.get_world_size()
@@ -125,6 +144,12 @@ lo, hi = shard_templates(batch, rank, world)
 own = torch.zeros(batch, dtype=torch.int64); own[lo:hi] = 1
 dist.all_reduce(own)
 assert bool((own == 1).all()), own
+# time-axis sharding of one long template: the ranks' spans tile [0, n) (halos are recomputed, not exchanged)
+n = 100000
+first, count, h_first, h_len = shard_time(n, rank, world, 1792, 90, 87)
+cover = torch.zeros(n, dtype=torch.int64); cover[first:first + count] = 1
+dist.all_reduce(cover)
+assert bool((cover == 1).all())
 # max-over-ranks timing + whole-job aggregation used by bench.py
 ms = bench.max_over_ranks(10.0 * (rank + 1))
 assert ms == 10.0 * world, ms

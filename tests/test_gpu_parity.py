@@ -315,6 +315,38 @@ def test_gpu_response_chunked_bitwise(lr, tdi_path):
     assert np.array_equal(out, R.tdi(y).cpu().numpy())
 
 
+@pytest.mark.parametrize("world", [2, 3])
+def test_gpu_time_sharded_spans_bitwise(lr, world):
+    """Time-axis sharding: every "rank" gets only its slice of h (span + halo, its own device
+    tensors) and computes its span with lr_response_span; the concatenation equals the whole-series result bit
+    for bit.  The ranks are run one after the other on the one GPU (they never wait on each other)."""
+    import torch
+    w = inputs.config(2, n=50021, f0=2e-3, t0=3.0e7)
+    tab = w.table()
+    s = w.sources[0]
+    hp, hc = w.waveform(0)
+    R = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="XYZ_AET")
+    ref = R.tdi(R.project(to_dev(hp)[None], to_dev(hc)[None], [s.beta], [s.lam], [s.psi])).cpu().numpy()
+    lo, hi, unit = R.span_halo()
+    got = np.full_like(ref, np.nan)
+    for rank in range(world):
+        first, count, h_first, h_len = lr.shard_time(w.n, rank, world, unit, lo, hi)
+        Rk = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="XYZ_AET")     # the rank's own handle
+        hps = to_dev(hp[h_first:h_first + h_len].copy())[None]
+        hcs = to_dev(hc[h_first:h_first + h_len].copy())[None]
+        out = Rk.response_span(hps, hcs, h_first, [s.beta], [s.lam], [s.psi], w.n, first, count)
+        torch.cuda.synchronize()
+        got[:, :, first:first + count] = out.cpu().numpy()
+    assert np.array_equal(got, ref)
+    # a slice that is too short is refused, as is a span that does not start on a unit
+    first, count, h_first, h_len = lr.shard_time(w.n, 1, 2, unit, lo, hi)
+    with pytest.raises(lr.LrError):
+        R.response_span(to_dev(hp[first:first + count].copy())[None], to_dev(hc[first:first + count].copy())[None],
+                        first, [s.beta], [s.lam], [s.psi], w.n, first, count)
+    with pytest.raises(lr.LrError):
+        R.response_span(to_dev(hp)[None], to_dev(hc)[None], 0, [s.beta], [s.lam], [s.psi], w.n, 100, 1000)
+
+
 def test_gpu_orbit_spline_matches_oracle(lr):
     """Orbit ingestion (lr_create's device spline) against the oracle's spline and scipy's not-a-knot
     CubicSpline at random times: positions to 1e-15 relative, light times to 1e-15 s."""
