@@ -511,7 +511,7 @@ def main():
         torch.cuda.set_device(local_rank)
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     try:
-        if args.shard == "time" and world > 1:
+        if args.shard == "time":
             run_gpu_time_sharded(args, rank, world, local_rank)
         else:
             run_gpu(args, rank, world, local_rank)
