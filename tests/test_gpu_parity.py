@@ -238,6 +238,49 @@ def test_gpu_laser_noise_suppression(lr):
         assert res[key] > 1e-10, res
 
 
+def test_gpu_worked_example_golden(lr, golden_dir):
+    """The CUDA path against the printed worked example (tests/golden/worked_example_p2.json; SURVEY.md §8(c),
+    survey-computed from PAPER.md eqs. 10-18 with 40-digit arithmetic) WITHOUT the oracle in between: static
+    equal-arm triangle, monochromatic source, every series is Re[(re + i im) e^{i w t}].  The fixture prints
+    10 digits, and the fp64 input h limits the agreement to ~1e-11 at 2 mHz."""
+    import json
+    import os
+    g = json.load(open(os.path.join(golden_dir, "worked_example_p2.json")))
+    beta, lam, psi, iota, A, f = 0.2, 1.0, 0.3, 0.5, 1e-22, 2e-3
+    dt, n, t0, order = 10.0, 3000, 5.0, 25
+    tab = inputs.orbit_table("static", t0, t0 + n * dt, const_ltt=inputs.ARM / inputs.C_LIGHT)
+    t = t0 + dt * np.arange(n)
+    w = 2 * np.pi * f
+    hp = A * (1 + np.cos(iota) ** 2) * np.cos(w * t)
+    hc = -2 * A * np.cos(iota) * np.sin(w * t)
+    for path in ("per_sample", "fir3"):
+        outs = {}
+        for gen in (1, 2):
+            R = lr.Response(tab, dt, order, gen, t0=t0, channels="XYZ_AET", tdi_path=path)
+            mp, mf, mb = R.margins()
+            y = R.project(to_dev(hp)[None], to_dev(hc)[None], [beta], [lam], [psi])
+            outs[gen] = (R.tdi(y).cpu().numpy()[0], mf, mb)
+        yh = y.cpu().numpy()[0]
+        for s, (i, j) in enumerate(inputs.LINKS):
+            v = g["links"][f"{i}{j}"]
+            want = v["re"] * np.cos(w * t) - v["im"] * np.sin(w * t)
+            assert np.abs(yh[s, mp:n - mp] - want[mp:n - mp]).max() < 3e-9 * np.hypot(v["re"], v["im"]), (path, s)
+        for gen in (1, 2):
+            o, mf, mb = outs[gen]
+            for c, name in enumerate("XYZ"):
+                re, im = g["tdi"][name][f"gen{gen}"]
+                want = re * np.cos(w * t) - im * np.sin(w * t)
+                assert np.abs(o[c, mf:n - mb] - want[mf:n - mb]).max() < 3e-9 * np.hypot(re, im), (path, gen, name)
+            for c in range(2):   # |A|, |E| (T is 3e-5 of A here: a null channel)
+                basis = np.stack([np.cos(w * t[mf:n - mb]), np.sin(w * t[mf:n - mb])], axis=1)
+                amp = float(np.hypot(*np.linalg.lstsq(basis, o[3 + c, mf:n - mb] * 1e24, rcond=None)[0])) * 1e-24
+                assert abs(amp - g["aet_abs"][f"gen{gen}"][c]) < 1e-8 * amp
+        ns = 1234   # t = 12345 s
+        assert abs(yh[0, ns] - g["spot"]["y12"]) < 1e-9 * abs(g["spot"]["y12"])
+        assert abs(outs[1][0][0, ns] - g["spot"]["X1"]) < 1e-9 * abs(g["spot"]["X1"])
+        assert abs(outs[2][0][0, ns] - g["spot"]["X2"]) < 1e-9 * abs(g["spot"]["X2"])
+
+
 def test_gpu_relabelling(lr):
     """Pin P4 on the GPU: cyclic relabelling of the spacecraft permutes (X,Y,Z) -> (Z,X,Y) of the relabelled
     run back onto (X,Y,Z); the reflection 2<->3 flips the sign of X."""
