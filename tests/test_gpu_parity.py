@@ -149,6 +149,33 @@ def test_tdi_delay_crossing_whole_sample(lr):
                 assert_parity(out[:, mf:n - mb], oo[:, mf:n - mb], f"crossing gen{gen} {path}", CH_NAMES["XYZ"])
 
 
+@pytest.mark.parametrize("ldot", [1e-9, 3e-8, 1e-6, 1e-5])
+def test_tdi_auto_path_follows_the_light_time_rate(lr, ldot):
+    """LR_TDI_AUTO picks quadratic / cubic FIR / per-sample weights from the largest |dL/dt| of the table
+    (1e-9: Keplerian-like; 3e-8..1e-6: strongly perturbed orbits; 1e-5: beyond any orbit, a delay sweeps through
+    whole samples every few hundred samples).  Whatever it picks must match the oracle, and the automatic
+    choice must agree bit for bit with the explicitly selected path it is documented to take."""
+    dt, n, t0, order = 5.0, 12000, 4.0e7, 25
+    base = inputs.orbit_table("kepler", t0, t0 + n * dt)
+    tk = base.t_start + base.knot_dt * np.arange(base.n_knots)
+    rate = ldot * (1 + 0.1 * np.arange(6))[:, None] * np.array([1, -1, 1, -1, 1, -1])[:, None]
+    ltt = 8.3 + 0.01 * np.arange(6)[:, None] + rate * (tk - (t0 + 0.5 * n * dt))[None, :]
+    tab = inputs.OrbitTable(base.t_start, base.knot_dt, base.x, np.ascontiguousarray(ltt))
+    rng = np.random.default_rng(17)
+    t = t0 + dt * np.arange(n)
+    y = np.stack([np.sin(2 * np.pi * f * t + p) for f, p in zip(rng.uniform(2e-4, 2e-2, 6), rng.uniform(0, 6, 6))])
+    O = orc.Oracle(tab, dt, t0, order)
+    oo = O.tdi(y, 2, nested=True, channels=orc.CH_XYZ_AET)
+    R = lr.Response(tab, dt, order, 2, t0=t0, channels="XYZ_AET")
+    _, mf, mb = R.margins()
+    out = R.tdi(to_dev(y)[None]).cpu().numpy()[0]
+    assert_parity(out[:, mf:n - mb], oo[:, mf:n - mb], f"auto path, dL/dt = {ldot:g}", CH_NAMES["XYZ_AET"])
+    de = 7 * 1.6 * ldot * 224      # links x largest rate x tile
+    expect = "fir3" if de <= 6e-6 else "fir4" if de <= 1.5e-4 else "per_sample"
+    Re = lr.Response(tab, dt, order, 2, t0=t0, channels="XYZ_AET", tdi_path=expect)
+    assert np.array_equal(Re.tdi(to_dev(y)[None]).cpu().numpy()[0], out), expect
+
+
 # ------------------------------------------------------------------------------------------- config 2
 @pytest.mark.parametrize("f0", [None, 1e-4, 1e-3, 1e-2])
 @pytest.mark.parametrize("chain", ["nested", "sum"])
