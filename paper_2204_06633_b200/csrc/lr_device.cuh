@@ -150,17 +150,38 @@ LR_HD void interp_sbp(const Params& prm, double eps, int a, Dif dif, double (&S)
 // ---------------------------------------------------------------------------------------------- stage 1
 // One time sample of eqs. 10-16 for all six links.  raw/dif: staged (h+, hx) pairs and their first
 // differences, W entries; nl = this sample's staged index; bs = k(3), u(3), v(3).  y6[slot] receives y_ij.
-template <int PT>
+template <int PT, class Store>
 LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W, int nl, double trel,
-                          const double* bs, double (&y6)[6]) {
-  const double k0 = bs[0], k1 = bs[1], k2 = bs[2];
-  const double u0 = bs[3], u1 = bs[4], u2 = bs[5];
-  const double v0 = bs[6], v1 = bs[7], v2 = bs[8];
-  double x[3][3];
+                          const double* bs, Store store) {
+  // geometry first (everything that needs the positions and the basis), so that only 12 doubles stay live
+  // across the nine interpolations: Dr[3] and, per arm, xi+, xix, k.n
+  double Dr[3], xip[3], xic[3], kn[3];
+  {
+    const double k0 = bs[0], k1 = bs[1], k2 = bs[2];
+    const double u0 = bs[3], u1 = bs[4], u2 = bs[5];
+    const double v0 = bs[6], v1 = bs[7], v2 = bs[8];
+    double x[3][3];
 #pragma unroll
-  for (int i = 0; i < 3; ++i)
+    for (int i = 0; i < 3; ++i) {
 #pragma unroll
-    for (int a = 0; a < 3; ++a) x[i][a] = spline_eval(prm, i * 3 + a, trel);
+      for (int a = 0; a < 3; ++a) x[i][a] = spline_eval(prm, i * 3 + a, trel);
+      Dr[i] = (k0 * x[i][0] + k1 * x[i][1] + k2 * x[i][2]) * prm.inv_cdt;   // reception delay k.x_i/c [samples]
+    }
+    // three arms: arm a joins receiver i = a and emitter j = (a+1)%3 (links 12, 23, 31); the reverse links
+    // 21, 32, 13 share xi+ and xix and flip the sign of k.n
+#pragma unroll
+    for (int arm = 0; arm < 3; ++arm) {
+      const int i = arm, j = (arm + 1) % 3;
+      const double d0 = x[i][0] - x[j][0], d1 = x[i][1] - x[j][1], d2 = x[i][2] - x[j][2];
+      const double inv = 1.0 / sqrt(d0 * d0 + d1 * d1 + d2 * d2);
+      const double n0v = d0 * inv, n1v = d1 * inv, n2v = d2 * inv;  // emitter j -> receiver i
+      const double un = u0 * n0v + u1 * n1v + u2 * n2v;
+      const double vn = v0 * n0v + v1 * n1v + v2 * n2v;
+      kn[arm] = k0 * n0v + k1 * n1v + k2 * n2v;
+      xip[arm] = un * un - vn * vn;   // eq. 12
+      xic[arm] = 2.0 * un * vn;
+    }
+  }
 
   auto fetch = [&](int m, double (&d)[2]) {
     const D2 v = dif[m];
@@ -170,34 +191,24 @@ LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W
   auto clampi = [](int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); };
 
   // reception: h at t - k.x_i/c for the three receivers (each shared by the two links it receives)
-  double Dr[3], Sr[3][2];
+  double Sr[3][2];
   int ar[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    Dr[i] = (k0 * x[i][0] + k1 * x[i][1] + k2 * x[i][2]) * prm.inv_cdt;
     double eps;
     split_delay(Dr[i], nl, ar[i], eps);
     ar[i] = clampi(ar[i], a_min, a_max);
     interp_sbp<PT, 2>(prm, eps, ar[i], fetch, Sr[i]);
   }
 
-  // three arms: arm a joins receiver i = a and emitter j = (a+1)%3 (links 12, 23, 31); the reverse links
-  // 21, 32, 13 share xi+ and xix and flip the sign of k.n
 #pragma unroll
   for (int arm = 0; arm < 3; ++arm) {
     const int i = arm, j = (arm + 1) % 3;
-    const double d0 = x[i][0] - x[j][0], d1 = x[i][1] - x[j][1], d2 = x[i][2] - x[j][2];
-    const double inv = 1.0 / sqrt(d0 * d0 + d1 * d1 + d2 * d2);
-    const double n0v = d0 * inv, n1v = d1 * inv, n2v = d2 * inv;  // emitter j -> receiver i
-    const double un = u0 * n0v + u1 * n1v + u2 * n2v;
-    const double vn = v0 * n0v + v1 * n1v + v2 * n2v;
-    const double kn = k0 * n0v + k1 * n1v + k2 * n2v;
-    const double xip = un * un - vn * vn, xic = 2.0 * un * vn;  // eq. 12
 #pragma unroll
     for (int dir = 0; dir < 2; ++dir) {
       const int rx = dir == 0 ? i : j, tx = dir == 0 ? j : i;
       const int slot = link_slot(rx, tx);
-      const double kappa = dir == 0 ? kn : -kn;
+      const double kappa = dir == 0 ? kn[arm] : -kn[arm];
       // emission: t - L_rx,tx(t) - k.x_tx(t)/c
       const double De = fma(spline_eval(prm, 9 + slot, trel), prm.inv_dt, Dr[tx]);
       int ae;
@@ -208,7 +219,7 @@ LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W
       const D2 re = raw[ae], rr = raw[ar[rx]];
       const double dhp = (re.x - rr.x) - Se[0] + Sr[rx][0];
       const double dhc = (re.y - rr.y) - Se[1] + Sr[rx][1];
-      y6[slot] = (xip * dhp + xic * dhc) / (2.0 * (1.0 - kappa));  // eq. 16
+      store(slot, (xip[arm] * dhp + xic[arm] * dhc) / (2.0 * (1.0 - kappa)));  // eq. 16
     }
   }
 }

@@ -18,7 +18,10 @@ namespace lr {
 // throughput.  The caps below keep the order-25 kernels spill-free.
 constexpr int kProjThreads = 128;
 constexpr int kTdiThreads = 256;
-__host__ __device__ constexpr int proj_min_blocks(int PT) { return PT == 0 ? 2 : PT <= 13 ? 4 : 3; }
+#ifndef LR_PROJ_MINB
+#define LR_PROJ_MINB 4
+#endif
+__host__ __device__ constexpr int proj_min_blocks(int PT) { return PT == 0 ? 2 : PT <= 13 ? LR_PROJ_MINB : 3; }
 __host__ __device__ constexpr int tdi_min_blocks(int PT) { return PT == 0 ? 2 : PT <= 13 ? 3 : 2; }
 
 // ---------------------------------------------------------------------------------------------- stage 1
@@ -65,10 +68,9 @@ project_kernel(const Params prm, const double* __restrict__ hp, const double* __
   double bs[9];
 #pragma unroll
   for (int a = 0; a < 9; ++a) bs[a] = __ldg(basis + b * 9 + a);
-  double y6[6];
-  project_sample<PT>(prm, raw, dif, W, n - g0, sample_trel(prm, ng), bs, y6);
-#pragma unroll
-  for (int s = 0; s < 6; ++s) yb[s * prm.out_stride] = y6[s];
+  const int64_t os = prm.out_stride;
+  project_sample<PT>(prm, raw, dif, W, n - g0, sample_trel(prm, ng), bs,
+                     [&](int slot, double v) { yb[slot * os] = v; });
 }
 
 // ---------------------------------------------------------------------------------------------- stage 2
