@@ -167,6 +167,23 @@ int lr_response_host(lr_handle* h_proj, lr_handle* h_tdi, const double* h_plus, 
                      const double* beta, const double* lambda, const double* psi, int64_t batch, int64_t n,
                      double* out, void* cuda_stream);
 
+/* Noise-weighted inner product of frequency-domain channels (eqs. 2-3, 22):
+ *   LR_IP_CROSS : out[b] = scale * sum_{ch,k} Re( conj(fa[b][ch][k]) fb[b'][ch][k] ) * inv_psd[ch][k]
+ *   LR_IP_DIFF  : out[b] = scale * sum_{ch,k} | fa[b][ch][k] - fb[b'][ch][k] |^2   * inv_psd[ch][k]
+ * with b' = b (batch_b == batch) or 0 (batch_b == 1: one data set d against every template).  With
+ * a~ = dt * rfft(a), df = 1/(n dt) and inv_psd = 1/S_n (0 in the DC bin), scale = 4 df gives <a|b> of eq. 2
+ * summed over the channels (eq. 22) and, in LR_IP_DIFF mode, scale = -2 df gives log L = -<d-h|d-h>/2 of eq. 3.
+ * The Fourier transforms are the caller's (a library FFT).  fa: DEVICE [batch][nch][nf] complex128 (re, im
+ * interleaved), fb: DEVICE [batch_b][nch][nf], inv_psd: DEVICE [nch][nf], work: DEVICE scratch of
+ * batch * LR_IP_BLOCKS doubles, out: DEVICE [batch].  Deterministic (fixed reduction tree).  batch <= 65535.
+ * Enqueues on `cuda_stream`.  Errors: LR_EINVAL, LR_ECUDA. */
+#define LR_IP_CROSS 0
+#define LR_IP_DIFF 1
+#define LR_IP_BLOCKS 256
+int lr_inner_product(const double* fa, const double* fb, const double* inv_psd, double scale, int mode,
+                     int64_t batch, int64_t batch_b, int nch, int64_t nf, double* work, double* out,
+                     void* cuda_stream);
+
 /* Evaluate the device spline of one orbit channel (0..8 = x[i][a] as i*3+a, 9..14 = L link slots) at
  * `m` times t (DEVICE [m]) into out (DEVICE [m]); used by the tests to pin the orbit ingestion. */
 int lr_eval_orbit(lr_handle* h, int channel, const double* t, int64_t m, double* out, void* cuda_stream);

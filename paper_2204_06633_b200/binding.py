@@ -19,6 +19,7 @@ LR_OK, LR_EINVAL, LR_ERANGE, LR_ECUDA, LR_ENOMEM = 0, -1, -2, -3, -4
 LR_OPT_T0, LR_OPT_CHAIN, LR_OPT_CHANNELS, LR_OPT_TDI_GEN, LR_OPT_TDI_PATH = 1, 2, 3, 4, 5
 LR_OPT_TDI_PLAN_CACHE = 6
 LR_OPT_CHUNK_SAMPLES = 7
+LR_IP_CROSS, LR_IP_DIFF, LR_IP_BLOCKS = 0, 1, 256
 LR_TDI_AUTO, LR_TDI_PER_SAMPLE, LR_TDI_FIR3, LR_TDI_FIR4 = -1, 0, 3, 4
 LR_CHAIN_NESTED, LR_CHAIN_SUM = 0, 1
 LR_XYZ, LR_AET, LR_XYZ_AET = 0, 1, 2
@@ -26,7 +27,7 @@ LR_MAX_ORDER = 65
 
 # every symbol include/lr.h declares
 SYMBOLS = ("lr_create", "lr_destroy", "lr_set_option", "lr_get_margins", "lr_project", "lr_tdi",
-           "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count",
+           "lr_inner_product", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count",
            "lr_last_cuda_error", "lr_strerror")
 
 
@@ -76,6 +77,7 @@ def lib():
     L.lr_response_span.argtypes = [vp, vp, vp, vp, i64, i64, vp, vp, vp, i64, i64, i64, i64, vp, vp]
     L.lr_get_span_halo.argtypes = [vp, vp, pi64, pi64, pi64]
     L.lr_response_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
+    L.lr_inner_product.argtypes = [vp, vp, vp, dbl, ci, i64, i64, ci, i64, vp, vp, vp]
     L.lr_eval_orbit.argtypes = [vp, ci, vp, i64, vp, vp]
     L.lr_measure_fp64_peak.argtypes = [dbl, ctypes.POINTER(dbl)]
     L.lr_launch_count.argtypes = []
@@ -230,6 +232,26 @@ def _as_host_f64(a):
     if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]):
         raise TypeError("host buffers must be C-contiguous float64")
     return a
+
+
+def lr_inner_product(fa, fb, inv_psd, scale, mode=LR_IP_CROSS, out=None, stream=None):
+    """lr_inner_product: fa CUDA complex128 [B, nch, nf], fb [B or 1, nch, nf], inv_psd CUDA float64 [nch, nf];
+    returns out CUDA float64 [B]."""
+    import torch
+    for name, t in (("fa", fa), ("fb", fb)):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.complex128 and t.is_contiguous()
+                and t.dim() == 3):
+            raise TypeError(f"{name} must be a contiguous complex128 CUDA tensor [batch, nch, nf]")
+    B, nch, nf = fa.shape
+    if fb.shape[1:] != fa.shape[1:] or fb.shape[0] not in (1, B):
+        raise ValueError("fb must be [batch or 1, nch, nf]")
+    if out is None:
+        out = torch.empty(B, dtype=torch.float64, device=fa.device)
+    work = torch.empty(B * LR_IP_BLOCKS, dtype=torch.float64, device=fa.device)
+    _check(lib().lr_inner_product(fa.data_ptr(), fb.data_ptr(), _dev_ptr(inv_psd, "inv_psd", nch * nf), float(scale),
+                                  int(mode), B, fb.shape[0], nch, nf, work.data_ptr(), _dev_ptr(out, "out", B),
+                                  _stream(stream)), "lr_inner_product")
+    return out
 
 
 def lr_eval_orbit(h, channel, t, out, stream=None):

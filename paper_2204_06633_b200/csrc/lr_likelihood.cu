@@ -1,0 +1,84 @@
+// lr_likelihood.cu — noise-weighted inner product of frequency-domain TDI channels (lr_inner_product):
+// PAPER.md eqs. 2-3 and 22, SURVEY.md §8(f) NEXT-2.  The Fourier transforms are a
+// library step of the caller (cuFFT through torch.fft.rfft); this file is the weighted reduction, which is
+// bound by HBM (40 B per frequency bin and channel) and deterministic (fixed two-stage tree, no atomics).
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <atomic>
+
+#include "../../include/lr.h"
+
+namespace lr {
+extern std::atomic<int64_t> g_launches;
+
+constexpr int kIpThreads = 256;
+
+__device__ __forceinline__ double block_sum(double v, double* sm) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) sm[warp] = v;
+  __syncthreads();
+  double t = 0.0;
+  if (warp == 0) {
+    t = lane < kIpThreads / 32 ? sm[lane] : 0.0;
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) t += __shfl_down_sync(0xffffffffu, t, o);
+  }
+  __syncthreads();
+  return t;   // valid in thread 0
+}
+
+// stage 1: grid (LR_IP_BLOCKS, batch); block bx of template b sums its contiguous slice of the M = nch*nf bins
+__global__ void __launch_bounds__(kIpThreads)
+ip_partial_kernel(const double2* __restrict__ fa, const double2* __restrict__ fb, const double* __restrict__ inv_psd,
+                  int64_t M, int64_t batch_b, int mode, double* __restrict__ work) {
+  __shared__ double sm[kIpThreads / 32];
+  const int64_t b = blockIdx.y;
+  const double2* a = fa + b * M;
+  const double2* c = fb + (batch_b == 1 ? 0 : b) * M;
+  const int64_t lo = M * blockIdx.x / gridDim.x, hi = M * (blockIdx.x + 1) / gridDim.x;
+  double acc = 0.0;
+  for (int64_t e = lo + threadIdx.x; e < hi; e += kIpThreads) {
+    const double2 x = __ldg(a + e), y = __ldg(c + e);
+    const double w = __ldg(inv_psd + e);
+    if (mode == 0) {
+      acc = fma(fma(x.x, y.x, x.y * y.y), w, acc);            // Re(conj(a) b) / S_n
+    } else {
+      const double dr = x.x - y.x, di = x.y - y.y;            // |a - b|^2 / S_n
+      acc = fma(fma(dr, dr, di * di), w, acc);
+    }
+  }
+  const double t = block_sum(acc, sm);
+  if (threadIdx.x == 0) work[b * gridDim.x + blockIdx.x] = t;
+}
+
+// stage 2: one block per template adds the LR_IP_BLOCKS partial sums in a fixed order
+__global__ void __launch_bounds__(kIpThreads)
+ip_final_kernel(const double* __restrict__ work, int nblk, double scale, double* __restrict__ out) {
+  __shared__ double sm[kIpThreads / 32];
+  const int64_t b = blockIdx.x;
+  double acc = 0.0;
+  for (int i = threadIdx.x; i < nblk; i += kIpThreads) acc += work[b * nblk + i];
+  const double t = block_sum(acc, sm);
+  if (threadIdx.x == 0) out[b] = scale * t;
+}
+}  // namespace lr
+
+extern "C" int lr_inner_product(const double* fa, const double* fb, const double* inv_psd, double scale, int mode,
+                                int64_t batch, int64_t batch_b, int nch, int64_t nf, double* work, double* out,
+                                void* stream) {
+  if (!fa || !fb || !inv_psd || !work || !out) return LR_EINVAL;
+  if (batch < 1 || batch > 65535 || (batch_b != 1 && batch_b != batch) || nch < 1 || nf < 1) return LR_EINVAL;
+  if (mode != LR_IP_CROSS && mode != LR_IP_DIFF) return LR_EINVAL;
+  const int64_t M = (int64_t)nch * nf;
+  cudaStream_t st = (cudaStream_t)stream;
+  dim3 grid(LR_IP_BLOCKS, (unsigned)batch);
+  lr::ip_partial_kernel<<<grid, lr::kIpThreads, 0, st>>>(reinterpret_cast<const double2*>(fa),
+                                                         reinterpret_cast<const double2*>(fb), inv_psd, M, batch_b,
+                                                         mode, work);
+  lr::ip_final_kernel<<<(unsigned)batch, lr::kIpThreads, 0, st>>>(work, LR_IP_BLOCKS, scale, out);
+  lr::g_launches.fetch_add(2);
+  return cudaGetLastError() == cudaSuccess ? LR_OK : LR_ECUDA;
+}

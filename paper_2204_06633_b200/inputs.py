@@ -346,3 +346,27 @@ def eval_tones(par, k, t):
     for f, a, p in zip(freq[k], amp[k], ph[k]):
         out = out + t.dtype.type(a) * np.sin(two_pi * t.dtype.type(f) * t + t.dtype.type(p))
     return out
+
+
+# ------------------------------------------------------------------------------- noise PSD (stand-in)
+def psd_standin(f, tdi_gen=2, arm_s=ARM / C_LIGHT):
+    """One-sided noise PSD S_n(f) of the TDI channels A, E, T as [3, len(f)] — a smooth analytic STAND-IN for
+    the "SciRDv1" curve of the LDC `tdi` package, which is not in the container.  Shape: test-mass
+    acceleration noise (3e-15 m/s^2/rtHz, reddened below 0.4 mHz) and optical-metrology noise (15 pm/rtHz,
+    reddened below 2 mHz) in relative-frequency units, through the equal-arm Michelson transfer
+    16 sin^2(w L) [S_oms + (3 + cos 2wL) S_acc] (x 4 sin^2(2 w L) for generation 2), with T less sensitive
+    than A, E at low frequency.  Only its smoothness and dynamic range matter for the tests; entry f = 0 is inf."""
+    f = np.asarray(f, dtype=np.float64)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        w = 2.0 * np.pi * f
+        s_acc = (3e-15 / (w * C_LIGHT)) ** 2 * (1.0 + (0.4e-3 / f) ** 2) * (1.0 + (f / 8e-3) ** 4)
+        s_oms = (15e-12 * w / C_LIGHT) ** 2 * (1.0 + (2e-3 / f) ** 4)
+        x = w * arm_s
+        gen = 4.0 * np.sin(2.0 * x) ** 2 if tdi_gen == 2 else 1.0
+        floor = 1e-6   # keeps the zeros of the transfer function (f = k / 2L) finite
+        tr = 16.0 * (np.sin(x) ** 2 + floor) * (gen + floor if tdi_gen == 2 else 1.0)
+        ae = tr * (s_oms + (3.0 + np.cos(2.0 * x)) * s_acc)
+        tt = tr * (s_oms + 8.0 * (np.sin(0.5 * x) ** 2 + floor) * s_acc) * (2.0 + np.cos(x))
+    out = np.stack([ae, ae, tt])
+    out[:, f == 0] = np.inf
+    return out

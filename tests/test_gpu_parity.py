@@ -471,6 +471,50 @@ def test_tdi_plan_cache(lr):
     assert np.array_equal(both[1:], fresh(yb, 5000, w.t0 + 12345.0, "nested"))
 
 
+# ------------------------------------------------------------------------------- likelihood (NEXT-2)
+def test_gpu_inner_product_parity(lr):
+    """lr_inner_product against the likelihood oracle on the SAME frequency-domain arrays (numpy FFT of real
+    A, E, T series of 9 templates), both modes, batch_b = batch and = 1, odd nf: relative error <= 1e-13; and
+    end to end from the GPU's own TDI output through torch.fft.rfft (cuFFT) against oracle TDI + numpy FFT."""
+    import torch
+    from oracle import likelihood as lk
+    w = inputs.config(3, batch=9, n=40001)
+    tab = w.table()
+    hp, hc = _stack(w, range(9))
+    beta, lam, psi = ([getattr(s, k) for s in w.sources] for k in ("beta", "lam", "psi"))
+    R = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="AET")
+    aet = R.response(to_dev(hp), to_dev(hc), beta, lam, psi)
+    torch.cuda.synchronize()
+    aet_h = aet.cpu().numpy()
+    n, dt = w.n, w.dt
+    f = np.fft.rfftfreq(n, dt)
+    psd = inputs.psd_standin(f)
+    inv = np.zeros_like(psd)
+    inv[:, 1:] = 1.0 / psd[:, 1:]
+    fh = lk.to_frequency(aet_h, dt)                       # [9, 3, nf]
+    fd = fh[4:5]                                          # "data" = template 4 (noiseless injection, PAPER.md:64)
+    df = 1.0 / (n * dt)
+    fh_d, fd_d, inv_d = (torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (fh, fd, inv))
+    want = lk.inner_product(fh, fd, psd, dt, n)           # <h_b|d> for every template
+    got = lr.lr_inner_product(fh_d, fd_d, inv_d, 4 * df).cpu().numpy()
+    assert np.abs(got - want.astype(np.float64)).max() <= 1e-13 * np.abs(want).max()
+    want = lk.inner_product(fh, fh, psd, dt, n)
+    got = lr.lr_inner_product(fh_d, fh_d, inv_d, 4 * df).cpu().numpy()
+    assert np.abs(got - want.astype(np.float64)).max() <= 1e-13 * np.abs(want).max()
+    ll = np.array([lk.log_likelihood(fd[0], fh[b], psd, dt, n) for b in range(9)], dtype=np.float64)
+    got = lr.lr_inner_product(fh_d, fd_d, inv_d, -2 * df, mode=lr.LR_IP_DIFF).cpu().numpy()
+    assert got[4] == 0.0 and np.all(got[np.arange(9) != 4] < 0)
+    assert np.abs(got - ll).max() <= 1e-12 * np.abs(ll).max()
+    # deterministic: the same call twice gives the same bits
+    assert np.array_equal(got, lr.lr_inner_product(fh_d, fd_d, inv_d, -2 * df, mode=lr.LR_IP_DIFF).cpu().numpy())
+    # end to end with the library FFT on the device
+    fh_gpu = (dt * torch.fft.rfft(aet, dim=-1)).contiguous()
+    got = lr.lr_inner_product(fh_gpu, fh_gpu, inv_d, 4 * df).cpu().numpy()
+    assert np.abs(got - want.astype(np.float64)).max() <= 1e-11 * np.abs(want).max()
+    with pytest.raises(lr.LrError):
+        lr.lr_inner_product(fh_d, fh_d, inv_d, 1.0, mode=7)
+
+
 # ---------------------------------------------------------------------------------------- edge cases
 def test_edge_cases_and_errors(lr):
     import torch
