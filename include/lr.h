@@ -179,7 +179,7 @@ int lr_response_host(lr_handle* h_proj, lr_handle* h_tdi, const double* h_plus, 
  * Enqueues on `cuda_stream`.  Errors: LR_EINVAL, LR_ECUDA. */
 #define LR_IP_CROSS 0
 #define LR_IP_DIFF 1
-#define LR_IP_BLOCKS 256
+#define LR_IP_BLOCKS 1024
 int lr_inner_product(const double* fa, const double* fb, const double* inv_psd, double scale, int mode,
                      int64_t batch, int64_t batch_b, int nch, int64_t nf, double* work, double* out,
                      void* cuda_stream);

@@ -19,7 +19,7 @@ LR_OK, LR_EINVAL, LR_ERANGE, LR_ECUDA, LR_ENOMEM = 0, -1, -2, -3, -4
 LR_OPT_T0, LR_OPT_CHAIN, LR_OPT_CHANNELS, LR_OPT_TDI_GEN, LR_OPT_TDI_PATH = 1, 2, 3, 4, 5
 LR_OPT_TDI_PLAN_CACHE = 6
 LR_OPT_CHUNK_SAMPLES = 7
-LR_IP_CROSS, LR_IP_DIFF, LR_IP_BLOCKS = 0, 1, 256
+LR_IP_CROSS, LR_IP_DIFF, LR_IP_BLOCKS = 0, 1, 1024
 LR_TDI_AUTO, LR_TDI_PER_SAMPLE, LR_TDI_FIR3, LR_TDI_FIR4 = -1, 0, 3, 4
 LR_CHAIN_NESTED, LR_CHAIN_SUM = 0, 1
 LR_XYZ, LR_AET, LR_XYZ_AET = 0, 1, 2

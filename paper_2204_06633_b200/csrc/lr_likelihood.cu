@@ -40,16 +40,26 @@ ip_partial_kernel(const double2* __restrict__ fa, const double2* __restrict__ fb
   const double2* c = fb + (batch_b == 1 ? 0 : b) * M;
   const int64_t lo = M * blockIdx.x / gridDim.x, hi = M * (blockIdx.x + 1) / gridDim.x;
   double acc = 0.0;
-  for (int64_t e = lo + threadIdx.x; e < hi; e += kIpThreads) {
-    const double2 x = __ldg(a + e), y = __ldg(c + e);
-    const double w = __ldg(inv_psd + e);
+  auto term = [&](const double2 x, const double2 y, const double w) {
     if (mode == 0) {
       acc = fma(fma(x.x, y.x, x.y * y.y), w, acc);            // Re(conj(a) b) / S_n
     } else {
       const double dr = x.x - y.x, di = x.y - y.y;            // |a - b|^2 / S_n
       acc = fma(fma(dr, dr, di * di), w, acc);
     }
+  };
+  int64_t e = lo + threadIdx.x;
+  for (; e + 3 * kIpThreads < hi; e += 4 * kIpThreads) {      // four independent loads in flight per thread
+    double2 x[4], y[4];
+    double w[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      x[u] = __ldg(a + e + u * kIpThreads); y[u] = __ldg(c + e + u * kIpThreads); w[u] = __ldg(inv_psd + e + u * kIpThreads);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) term(x[u], y[u], w[u]);
   }
+  for (; e < hi; e += kIpThreads) term(__ldg(a + e), __ldg(c + e), __ldg(inv_psd + e));
   const double t = block_sum(acc, sm);
   if (threadIdx.x == 0) work[b * gridDim.x + blockIdx.x] = t;
 }
