@@ -9,7 +9,8 @@ Contract: `python bench.py --gpus N --steps K --warmup W` pr
   * N > 1: every rank runs the same-sized workload on its own seeded template(s) (the path shards over
     templates with no collective: "scaling": "weak"); time = max over ranks, value = all ranks' samples / time;
   * `value` has the inputs resident in HBM; `e2e` goes through lr_response_host with pinned HOST buffers;
-  * `roofline`: the dominant kernel (TDI) against the FP64 issue rate measured live by lr_measure_fp64_peak;
+  * `roofline`: the dominant kernel (the slower of lr_project / lr_tdi) against the FP64 issue rate measured
+    live by lr_measure_fp64_peak; `kernels` has both; `lr_response`, `likelihood`, `tdi_plan` are extra legs;
   * `cpu_baseline` / `--impl reference`: the oracle (fp64 arithmetic, all host cores) on a bounded sample.
 """
 from __future__ import annotations
