@@ -230,6 +230,8 @@ def workload_config(w, batch, args):
 def run_gpu(args, rank, world, local_rank):
     import torch
     import paper_2204_06633_b200 as lr
+    from paper_2204_06633_b200 import build as lrbuild
+    lrbuild.ensure_built(local_rank)   # fresh checkout: compile the (git-ignored) library once
     lr.binding.lib()  # no CUDA extension -> fail loudly, there is no fallback
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)

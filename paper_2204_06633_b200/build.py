@@ -67,6 +67,23 @@ def build(force=False, verbose=False):
     return LIB
 
 
+def ensure_built(local_rank=0, timeout_s=900.0):
+    """Build liblr.so if it is MISSING (a fresh checkout: the .so is git-ignored).  Under torchrun only local
+    rank 0 compiles; the other ranks wait for the file.  Building the product is not a fallback: without nvcc
+    this raises."""
+    import time
+    if os.path.exists(LIB):
+        return LIB
+    if local_rank == 0:
+        return build(force=True)
+    t0 = time.time()
+    while not os.path.exists(LIB):
+        if time.time() - t0 > timeout_s:
+            raise RuntimeError("timed out waiting for local rank 0 to build liblr.so")
+        time.sleep(1.0)
+    return LIB
+
+
 if __name__ == "__main__":
     import sys
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

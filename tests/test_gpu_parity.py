@@ -23,7 +23,9 @@ def lr():
     if not torch.cuda.is_available():
         pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
     import paper_2204_06633_b200 as pkg
-    pkg.binding.lib()  # fail loudly if liblr.so is missing
+    from paper_2204_06633_b200 import build
+    build.ensure_built()   # fresh checkout: the .so is git-ignored; compiling it needs nvcc (no CPU fallback)
+    pkg.binding.lib()      # fail loudly if liblr.so cannot be loaded
     return pkg
 
 
