@@ -459,6 +459,8 @@ def run_gpu_time_sharded(args, rank, world, local_rank):
     of out with lr_response_span; no collective on the data path.  Strong scaling: value = n / max-over-ranks time."""
     import torch
     import paper_2204_06633_b200 as lr
+    from paper_2204_06633_b200 import build as lrbuild
+    lrbuild.ensure_built(local_rank)
     lr.binding.lib()
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
