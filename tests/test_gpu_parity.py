@@ -419,6 +419,32 @@ def test_gpu_time_sharded_spans_bitwise(lr, world):
         R.response_span(to_dev(hp)[None], to_dev(hc)[None], 0, [s.beta], [s.lam], [s.psi], w.n, 100, 1000)
 
 
+def test_gpu_non_default_stream(lr):
+    """Every call enqueues on the stream it is given: the same results on a side stream (torch.cuda.Stream) as on
+    the default stream, for the two-call path, the one-call paths and the host-buffer pipeline; a plan built on
+    one stream is reused safely from another."""
+    import torch
+    w = inputs.config(2, n=30011, f0=5e-3, t0=2.0e7)
+    tab = w.table()
+    s = w.sources[0]
+    hp, hc = w.waveform(0)
+    R = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="XYZ_AET")
+    hpd, hcd = to_dev(hp)[None], to_dev(hc)[None]
+    ref = R.tdi(R.project(hpd, hcd, [s.beta], [s.lam], [s.psi])).cpu().numpy()      # default stream, builds the plan
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        y = R.project(hpd, hcd, [s.beta], [s.lam], [s.psi], stream=side)
+        a = R.tdi(y, stream=side)
+        b = R.response(hpd, hcd, [s.beta], [s.lam], [s.psi], stream=side)
+        out = torch.empty(ref.shape, dtype=torch.float64).pin_memory()
+        R.response_host(torch.from_numpy(hp).pin_memory(), torch.from_numpy(hc).pin_memory(), [s.beta], [s.lam],
+                        [s.psi], out, stream=side)
+    side.synchronize()
+    assert np.array_equal(a.cpu().numpy(), ref) and np.array_equal(b.cpu().numpy(), ref)
+    assert np.array_equal(out.numpy(), ref)
+
+
 def test_gpu_orbit_spline_matches_oracle(lr):
     """Orbit ingestion (lr_create's device spline) against the oracle's spline and scipy's not-a-knot
     CubicSpline at random times: positions to 1e-15 relative, light times to 1e-15 s."""
