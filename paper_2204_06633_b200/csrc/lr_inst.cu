@@ -79,10 +79,16 @@ static int launch_tdi_fir(const Params& prm, int channels, const double* y, doub
   if ((e = cudaEventRecord((cudaEvent_t)plan.join, side)) != cudaSuccess) return (int)e;
 
   const size_t smem = fir_apply_smem_bytes(W, prm.fir_wc);
-  if ((e = prepare(tdi_fir_apply_kernel<NN>, smem)) != cudaSuccess) return (int)e;
   const int64_t grid = (int64_t)prm.ntiles * batch;
-  tdi_fir_apply_kernel<NN><<<(unsigned)grid, kFirThreads, smem, st>>>(prm, y, out, channels, plan.coef, plan.flags,
-                                                                    (int)batch);
+  if (prm.fir_uniform) {   // constant light times: the weights do not depend on tile time, k0 alone
+    if ((e = prepare(tdi_fir_apply_kernel<1>, smem)) != cudaSuccess) return (int)e;
+    tdi_fir_apply_kernel<1><<<(unsigned)grid, kFirThreads, smem, st>>>(prm, y, out, channels, plan.coef, plan.flags,
+                                                                     (int)batch);
+  } else {
+    if ((e = prepare(tdi_fir_apply_kernel<NN>, smem)) != cudaSuccess) return (int)e;
+    tdi_fir_apply_kernel<NN><<<(unsigned)grid, kFirThreads, smem, st>>>(prm, y, out, channels, plan.coef, plan.flags,
+                                                                      (int)batch);
+  }
   g_launches.fetch_add(1);
   if ((e = cudaGetLastError()) != cudaSuccess) return (int)e;
   return plan.wait_join ? (int)cudaStreamWaitEvent(st, (cudaEvent_t)plan.join, 0) : 0;   // join

@@ -23,6 +23,12 @@
 
 namespace lr {
 
+#ifndef LR_FIR_MINB
+#define LR_FIR_MINB 7                    // resident apply CTAs per SM the register budget is set for
+#endif
+#ifndef LR_FIR_LOADS
+#define LR_FIR_LOADS 9
+#endif
 #ifndef LR_FIR_R
 #define LR_FIR_R 7
 #endif
@@ -210,7 +216,10 @@ LR_HD void fir_merge(const Params& prm, const FirTile<GEN, NN>& T, const double*
 // first `pad` taps of every series are zero padding.
 // Per tap the coefficient is evaluated at each sample's own tau (Horner over the NN powers) and applied to
 // the sliding window of first differences: NN FMAs per (tap, sample), one accumulator per sample.
-template <int NN>
+// NN = 1 (constant light times): k0 alone.
+// ALIAS: `res` overlays `dif`; every thread then runs the loop body exactly once (nthreads == 3 * groups) and
+// the block synchronises between the last read of dif and the first write of res.
+template <int NN, bool ALIAS = false>
 LR_HD void fir_apply(const double* dif, int W, const double* K, int Wc, int pad, int P, int nl0, int B, double* res,
                      int tid, int nthreads) {
   constexpr int R = kFirR;
@@ -226,39 +235,49 @@ LR_HD void fir_apply(const double* dif, int W, const double* K, int Wc, int pad,
 #pragma unroll 1
     for (int sl = 0; sl < 4; ++sl) {
       const double* d = dif + rot_slot_rt(fir_base_slot(sl), ch) * W + (nl0 + i0 - back);
-      const double* kk = K + (size_t)((ch * 4 + sl) * Wc) * kFirKStride;
-      double win[2 * R];
+      int koff = (ch * 4 + sl) * Wc * kFirKStride;
+#if defined(__CUDA_ARCH__) && !defined(LR_FIR_NO_PIN)
+      asm volatile("" : "+r"(koff));   // keep the tap offset in a register (ptxas otherwise rebuilds it per tap)
+#endif
+      const double* kk = K + koff;
+      // circular window: tap t = m0 + mm needs d[t .. t+R), kept at positions (t + r) % R; after the tap the
+      // slot of d[t] takes d[t + R] (indices are compile-time constants: m0 is a multiple of R)
+      double win[R];
 #pragma unroll
       for (int r = 0; r < R; ++r) win[r] = d[r];
 #pragma unroll 1
       for (int m0 = 0; m0 < Wc; m0 += R) {
-#pragma unroll
-        for (int r = 0; r < R; ++r) win[R + r] = d[m0 + R + r];
         const int skip = m0 == 0 ? pad : 0;   // the first `pad` stored taps are padding (all zero)
 #pragma unroll
         for (int mm = 0; mm < R; ++mm) {
-          if (mm < skip) continue;
-          double kc[NN];
+          if (mm >= skip) {
+            double kc[NN];
 #pragma unroll
-          for (int p = 0; p < NN; ++p) kc[p] = kk[(m0 + mm) * kFirKStride + p];
+            for (int p = 0; p < NN; ++p) kc[p] = kk[(m0 + mm) * kFirKStride + p];
+            double c[R];
 #pragma unroll
-          for (int r = 0; r < R; ++r) {
-            double c = kc[NN - 1];
+            for (int r = 0; r < R; ++r) c[r] = kc[NN - 1];
 #pragma unroll
-            for (int p = NN - 2; p >= 0; --p) c = fma(c, tau[r], kc[p]);
-            acc[r] = fma(c, win[mm + r], acc[r]);
+            for (int p = NN - 2; p >= 0; --p)
+#pragma unroll
+              for (int r = 0; r < R; ++r) c[r] = fma(c[r], tau[r], kc[p]);
+#pragma unroll
+            for (int r = 0; r < R; ++r) acc[r] = fma(c[r], win[(mm + r) % R], acc[r]);
           }
+          win[mm] = d[m0 + mm + R];
         }
-#pragma unroll
-        for (int r = 0; r < R; ++r) win[r] = win[R + r];
       }
     }
+#ifdef __CUDA_ARCH__
+    if (ALIAS) __syncthreads();
+#endif
 #pragma unroll
     for (int r = 0; r < R; ++r)
       if (i0 + r < B) res[ch * B + i0 + r] = acc[r];
   }
 }
 
+constexpr int kFirLoads = LR_FIR_LOADS;           // loads of y a thread of the apply kernel keeps in flight
 constexpr int kFirGroups = 32;                    // groups of kFirR samples per channel and tile
 constexpr int kFirTile = kFirGroups * kFirR;      // 224 samples per tile
 constexpr int kFirThreads = 3 * kFirGroups;       // apply kernel: one warp per channel
@@ -309,9 +328,9 @@ tdi_fir_setup_kernel(const Params prm, double* __restrict__ plan, int* __restric
 // ----------------------------------------------------------------------------------------- apply kernel
 // grid.x = ntiles * batch, template index fastest (the tiles of one time span share their plan through L2).
 // Tiles flagged by the plan are left to tdi_fir_fixup_kernel.
-// dynamic smem: dif[6][W] | K[12][Wc][4] | res[3][B]
+// dynamic smem: dif[6][W] | K[12][Wc][4]; the results res[3][B] overlay dif once every read of it is done
 LR_HD size_t fir_apply_smem_bytes(int W, int Wc) {
-  return ((size_t)6 * W + fir_plan_doubles_per_tile(Wc) + 3 * (size_t)kFirTile) * sizeof(double);
+  return ((size_t)6 * W + fir_plan_doubles_per_tile(Wc)) * sizeof(double);
 }
 
 // eq. 21 and the coalesced store of one sample (shared by the apply and fix-up kernels)
@@ -326,7 +345,7 @@ __device__ __forceinline__ void fir_store(double* ob, int64_t N, int n, int chan
 }
 
 template <int NN>
-__global__ void __launch_bounds__(kFirThreads, 7)
+__global__ void __launch_bounds__(kFirThreads, LR_FIR_MINB)
 tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ out, int channels,
                      const double* __restrict__ plan, const int* __restrict__ flags, int batch) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -335,7 +354,8 @@ tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __r
   const int Wc = prm.fir_wc;
   double* dif = reinterpret_cast<double*>(smem_raw);
   double* K = dif + 6 * W;
-  double* res = K + fir_plan_doubles_per_tile(Wc);
+  double* res = dif;
+  static_assert(kFirThreads == 3 * kFirGroups && kFirGroups * kFirR == kFirTile, "one work item per thread");
 
   const int tid = threadIdx.x;
   const int tile = blockIdx.x / batch;                       // local tile: local samples [n0, n0 + B)
@@ -358,21 +378,51 @@ tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __r
   const int slot = prm.fir_uniform ? 0 : tile_g;             // constant light times: one plan for every tile
   if (flags[slot] != 0) return;                              // exact per-sample tile: the fix-up kernel's
 
-  // first differences straight from global memory (the second load of each pair hits L1)
-  const double* yb = y + b * 6 * prm.in_stride;
-  for (int m = tid; m < 6 * W; m += kFirThreads) {
-    const int s = m / W, g = g0 + (m - s * W);
-    const double* ys = yb + s * prm.in_stride;
-    const double a = (g >= prm.rd_lo && g < prm.rd_hi) ? __ldg(ys + g) : 0.0;
-    const double c = (g + 1 >= prm.rd_lo && g + 1 < prm.rd_hi) ? __ldg(ys + g + 1) : 0.0;
-    dif[m] = c - a;
+  // the tile's plan: global -> shared without passing through registers, in flight under the loads of y
+  {
+    const double2* src = reinterpret_cast<const double2*>(plan + (size_t)slot * fir_plan_doubles_per_tile(Wc));
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(K);
+    const int cnt = (int)(fir_plan_doubles_per_tile(Wc) / 2);
+    for (int m = tid; m < cnt; m += kFirThreads)
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * m), "l"(src + m) : "memory");
+    asm volatile("cp.async.commit_group;" ::: "memory");
   }
-  const double2* src = reinterpret_cast<const double2*>(plan + (size_t)slot * fir_plan_doubles_per_tile(Wc));
-  double2* dst = reinterpret_cast<double2*>(K);
-  const int cnt = (int)(fir_plan_doubles_per_tile(Wc) / 2);
-  for (int m = tid; m < cnt; m += kFirThreads) dst[m] = __ldg(src + m);
+  // first differences straight from global memory.  A warp loads 32 consecutive samples of one series and
+  // forms 31 differences with a shuffle; all kFirLoads loads of a thread are issued before the first use, so
+  // the staging costs one memory round trip (the series are not in L2 when they come from another kernel
+  // launch: the filter loop of the other resident CTAs has to cover this wait).
+  {
+    const double* yb = y + b * 6 * prm.in_stride;
+    const int lane = tid & 31, warp = tid >> 5;
+    const int cps = (W + 30) / 31;                           // chunks of 31 differences per series (>= 8)
+    const int per_warp = 2 * cps;                            // 6 * cps chunks over 3 warps
+    for (int u0 = 0; u0 < per_warp; u0 += kFirLoads) {
+      double a[kFirLoads];
+      int sr = (warp + 3 * u0) / cps, chunk = (warp + 3 * u0) - sr * cps;
+      {
+        int s1 = sr, c1 = chunk;
+#pragma unroll
+        for (int u = 0; u < kFirLoads; ++u) {
+          const int g = g0 + c1 * 31 + lane;
+          const bool ok = u0 + u < per_warp && c1 * 31 + lane <= W && g >= prm.rd_lo && g < prm.rd_hi;
+          a[u] = ok ? __ldg(yb + (int64_t)s1 * prm.in_stride + g) : 0.0;
+          c1 += 3;
+          if (c1 >= cps) { c1 -= cps; ++s1; }
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < kFirLoads; ++u) {
+        const double c = __shfl_down_sync(0xffffffffu, a[u], 1);
+        const int w = chunk * 31 + lane;
+        if (u0 + u < per_warp && lane < 31 && w < W) dif[sr * W + w] = c - a[u];
+        chunk += 3;
+        if (chunk >= cps) { chunk -= cps; ++sr; }
+      }
+    }
+  }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
   __syncthreads();
-  fir_apply<NN>(dif, W, K, Wc, Wc - prm.fir_taps, prm.p, prm.halo_lo, B, res, tid, kFirThreads);
+  fir_apply<NN, true>(dif, W, K, Wc, Wc - prm.fir_taps, prm.p, prm.halo_lo, B, res, tid, kFirThreads);
   __syncthreads();
   for (int i = tid; i < B; i += kFirThreads) {
     const int n = n0 + i;
