@@ -87,14 +87,31 @@ LR_HD D4 load4(const D4* p) {
 LR_HD double sample_trel(const Params& P, int n) { return fma((double)n, P.dt, P.trel0); }
 
 // cubic spline channel `ch` at relative time trel (reading A9)
-LR_HD double spline_eval(const Params& P, int ch, double trel) {
+LR_HD int spline_interval(const Params& P, double trel, double& u) {
   const double s = trel * P.inv_h;
   int i = (int)floor(s);
   i = i < 0 ? 0 : (i > P.nint - 1 ? P.nint - 1 : i);
-  const double u = s - (double)i;
-  const D4 c = load4(P.coef + (int64_t)ch * P.nint + i);
+  u = s - (double)i;
+  return i;
+}
+// where the coefficients of interval i come from: the table in global memory, or the copy of the (at most
+// two) intervals of a tile that a kernel staged in shared memory
+struct CoefGlobal {
+  LR_HD D4 get(const Params& P, int ch, int i) const { return load4(P.coef + (int64_t)ch * P.nint + i); }
+};
+struct CoefTile {
+  const D4* sc;   // [15][2]
+  int i0;
+  LR_HD D4 get(const Params&, int ch, int i) const { return sc[ch * 2 + (i - i0)]; }
+};
+template <class Coef>
+LR_HD double spline_eval(const Params& P, const Coef& src, int ch, double trel) {
+  double u;
+  const int i = spline_interval(P, trel, u);
+  const D4 c = src.get(P, ch, i);
   return fma(fma(fma(c.w, u, c.z), u, c.y), u, c.x);
 }
+LR_HD double spline_eval(const Params& P, int ch, double trel) { return spline_eval(P, CoefGlobal{}, ch, trel); }
 
 // Split a delay of D samples: anchor index a = n - ceil(D) + 1 (the sample just above the target
 // n - D), eps = ceil(D) - D in [0,1).  Stencil taps are a-P .. a+P-1.
@@ -150,9 +167,9 @@ LR_HD void interp_sbp(const Params& prm, double eps, int a, Dif dif, double (&S)
 // ---------------------------------------------------------------------------------------------- stage 1
 // One time sample of eqs. 10-16 for all six links.  raw/dif: staged (h+, hx) pairs and their first
 // differences, W entries; nl = this sample's staged index; bs = k(3), u(3), v(3).  y6[slot] receives y_ij.
-template <int PT, class Store>
+template <int PT, class Store, class Coef = CoefGlobal>
 LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W, int nl, double trel,
-                          const double* bs, Store store) {
+                          const double* bs, Store store, const Coef& coef = Coef{}) {
   // geometry first (everything that needs the positions and the basis), so that only 12 doubles stay live
   // across the nine interpolations: Dr[3] and, per arm, xi+, xix, k.n
   double Dr[3], xip[3], xic[3], kn[3];
@@ -164,7 +181,7 @@ LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
 #pragma unroll
-      for (int a = 0; a < 3; ++a) x[i][a] = spline_eval(prm, i * 3 + a, trel);
+      for (int a = 0; a < 3; ++a) x[i][a] = spline_eval(prm, coef, i * 3 + a, trel);
       Dr[i] = (k0 * x[i][0] + k1 * x[i][1] + k2 * x[i][2]) * prm.inv_cdt;   // reception delay k.x_i/c [samples]
     }
     // three arms: arm a joins receiver i = a and emitter j = (a+1)%3 (links 12, 23, 31); the reverse links
@@ -210,7 +227,7 @@ LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W
       const int slot = link_slot(rx, tx);
       const double kappa = dir == 0 ? kn[arm] : -kn[arm];
       // emission: t - L_rx,tx(t) - k.x_tx(t)/c
-      const double De = fma(spline_eval(prm, 9 + slot, trel), prm.inv_dt, Dr[tx]);
+      const double De = fma(spline_eval(prm, coef, 9 + slot, trel), prm.inv_dt, Dr[tx]);
       int ae;
       double eps, Se[2];
       split_delay(De, nl, ae, eps);

@@ -43,6 +43,18 @@ project_kernel(const Params prm, const double* __restrict__ hp, const double* __
   const double* hpb = hp + b * prm.in_stride;
   const double* hcb = hc + b * prm.in_stride;
 
+  // the samples of a tile fall in one or two spline intervals (knots are hours apart): their coefficients
+  // go to shared memory, so that no evaluation in project_sample waits on a global load
+  __shared__ D4 sc[15 * 2];
+  double u_unused;
+  const int n_last = n0 + kProjThreads - 1 < prm.n - 1 ? n0 + kProjThreads - 1 : prm.n - 1;
+  const int i_lo = spline_interval(prm, sample_trel(prm, prm.n_off + n0), u_unused);
+  const int i_hi = spline_interval(prm, sample_trel(prm, prm.n_off + n_last), u_unused);
+  const bool tile_coef = i_hi - i_lo <= 1;   // (block-uniform)
+  if (tile_coef && threadIdx.x < 30) {
+    const int ch = threadIdx.x >> 1, i = i_lo + (threadIdx.x & 1);
+    sc[threadIdx.x] = load4(prm.coef + (int64_t)ch * prm.nint + (i < prm.nint ? i : prm.nint - 1));
+  }
   for (int m = threadIdx.x; m < W; m += kProjThreads) {
     const int g = g0 + m;
     D2 v{0.0, 0.0};
@@ -69,8 +81,11 @@ project_kernel(const Params prm, const double* __restrict__ hp, const double* __
 #pragma unroll
   for (int a = 0; a < 9; ++a) bs[a] = __ldg(basis + b * 9 + a);
   const int64_t os = prm.out_stride;
-  project_sample<PT>(prm, raw, dif, W, n - g0, sample_trel(prm, ng), bs,
-                     [&](int slot, double v) { yb[slot * os] = v; });
+  auto store = [&](int slot, double v) { yb[slot * os] = v; };
+  if (tile_coef)
+    project_sample<PT>(prm, raw, dif, W, n - g0, sample_trel(prm, ng), bs, store, CoefTile{sc, i_lo});
+  else
+    project_sample<PT>(prm, raw, dif, W, n - g0, sample_trel(prm, ng), bs, store, CoefGlobal{});
 }
 
 // ---------------------------------------------------------------------------------------------- stage 2
