@@ -26,9 +26,6 @@ namespace lr {
 #ifndef LR_FIR_MINB
 #define LR_FIR_MINB 7                    // resident apply CTAs per SM the register budget is set for
 #endif
-#ifndef LR_FIR_LOADS
-#define LR_FIR_LOADS 9
-#endif
 #ifndef LR_FIR_R
 #define LR_FIR_R 7
 #endif
@@ -214,8 +211,12 @@ LR_HD void fir_merge(const Params& prm, const FirTile<GEN, NN>& T, const double*
 // E: apply.  One work item = kFirR consecutive samples of one channel.  dif: [6][W]; res: [3][B] (tile
 // staging of X, Y, Z).  nl0 = staged index of the tile's first sample; Wc is a multiple of kFirR and the
 // first `pad` taps of every series are zero padding.
-// Per tap the coefficient is evaluated at each sample's own tau (Horner over the NN powers) and applied to
-// the sliding window of first differences: NN FMAs per (tap, sample), one accumulator per sample.
+// X(n) = sum_p tau_n^p A_p(n) with A_p(n) = sum_m K_p[m] dif[n + m]: NN accumulators per sample, NN FMAs per
+// (tap, sample), the powers of tau applied once at the end.  Every FMA of the loop is (k_p, dif, A_p): k_p is
+// common to the R samples of a tap and dif to the NN accumulators of a sample, so consecutive FMAs share a
+// source register.  That matters on sm_100: a DFMA with three register operands none of which the previous
+// instruction used issues every third cycle instead of every second (measured: 42 against 53-54 DFMA/clk/SM),
+// which is what the Horner form (coefficient evaluated at tau_n first, then one FMA into one accumulator) ran at.
 // NN = 1 (constant light times): k0 alone.
 // ALIAS: `res` overlays `dif`; every thread then runs the loop body exactly once (nthreads == 3 * groups) and
 // the block synchronises between the last read of dif and the first write of res.
@@ -229,9 +230,11 @@ LR_HD void fir_apply(const double* dif, int W, const double* K, int Wc, int pad,
   for (int w = tid; w < 3 * groups; w += nthreads) {
     const int ch = w / groups, g = w - ch * groups;
     const int i0 = g * R;                                  // first sample of the group inside the tile
-    double acc[R], tau[R];
+    double acc[NN][R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) { acc[r] = 0.0; tau[r] = ((double)(i0 + r) - half) * inv_half; }
+    for (int p = 0; p < NN; ++p)
+#pragma unroll
+      for (int r = 0; r < R; ++r) acc[p][r] = 0.0;
 #pragma unroll 1
     for (int sl = 0; sl < 4; ++sl) {
       const double* d = dif + rot_slot_rt(fir_base_slot(sl), ch) * W + (nl0 + i0 - back);
@@ -254,30 +257,30 @@ LR_HD void fir_apply(const double* dif, int W, const double* K, int Wc, int pad,
             double kc[NN];
 #pragma unroll
             for (int p = 0; p < NN; ++p) kc[p] = kk[(m0 + mm) * kFirKStride + p];
-            double c[R];
 #pragma unroll
-            for (int r = 0; r < R; ++r) c[r] = kc[NN - 1];
+            for (int p = 0; p < NN; ++p)
 #pragma unroll
-            for (int p = NN - 2; p >= 0; --p)
-#pragma unroll
-              for (int r = 0; r < R; ++r) c[r] = fma(c[r], tau[r], kc[p]);
-#pragma unroll
-            for (int r = 0; r < R; ++r) acc[r] = fma(c[r], win[(mm + r) % R], acc[r]);
+              for (int r = 0; r < R; ++r) acc[p][r] = fma(kc[p], win[(mm + r) % R], acc[p][r]);
           }
           win[mm] = d[m0 + mm + R];
         }
       }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      const double tau = ((double)(i0 + r) - half) * inv_half;
+#pragma unroll
+      for (int p = NN - 2; p >= 0; --p) acc[p][r] = fma(acc[p + 1][r], tau, acc[p][r]);
     }
 #ifdef __CUDA_ARCH__
     if (ALIAS) __syncthreads();
 #endif
 #pragma unroll
     for (int r = 0; r < R; ++r)
-      if (i0 + r < B) res[ch * B + i0 + r] = acc[r];
+      if (i0 + r < B) res[ch * B + i0 + r] = acc[0][r];
   }
 }
 
-constexpr int kFirLoads = LR_FIR_LOADS;           // loads of y a thread of the apply kernel keeps in flight
 constexpr int kFirGroups = 32;                    // groups of kFirR samples per channel and tile
 constexpr int kFirTile = kFirGroups * kFirR;      // 224 samples per tile
 constexpr int kFirThreads = 3 * kFirGroups;       // apply kernel: one warp per channel
@@ -345,7 +348,7 @@ __device__ __forceinline__ void fir_store(double* ob, int64_t N, int n, int chan
 }
 
 template <int NN>
-__global__ void __launch_bounds__(kFirThreads, LR_FIR_MINB)
+__global__ void __launch_bounds__(kFirThreads, NN > 3 ? 5 : LR_FIR_MINB)   // NN = 4: 28 accumulators
 tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ out, int channels,
                      const double* __restrict__ plan, const int* __restrict__ flags, int batch) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -387,36 +390,28 @@ tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __r
       asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * m), "l"(src + m) : "memory");
     asm volatile("cp.async.commit_group;" ::: "memory");
   }
-  // first differences straight from global memory.  A warp loads 32 consecutive samples of one series and
-  // forms 31 differences with a shuffle; all kFirLoads loads of a thread are issued before the first use, so
-  // the staging costs one memory round trip (the series are not in L2 when they come from another kernel
-  // launch: the filter loop of the other resident CTAs has to cover this wait).
+  // first differences straight from global memory (the second load of each pair hits L1).  Instructions
+  // count here: an FP64 instruction holds its scheduler's issue port for two cycles, so every other
+  // instruction of the kernel takes time from the filter loop of the co-resident CTAs.
   {
-    const double* yb = y + b * 6 * prm.in_stride;
-    const int lane = tid & 31, warp = tid >> 5;
-    const int cps = (W + 30) / 31;                           // chunks of 31 differences per series (>= 8)
-    const int per_warp = 2 * cps;                            // 6 * cps chunks over 3 warps
-    for (int u0 = 0; u0 < per_warp; u0 += kFirLoads) {
-      double a[kFirLoads];
-      int sr = (warp + 3 * u0) / cps, chunk = (warp + 3 * u0) - sr * cps;
-      {
-        int s1 = sr, c1 = chunk;
+    const double* yb = y + b * 6 * prm.in_stride + g0;
+    if (g0 >= prm.rd_lo && g0 + W < prm.rd_hi) {             // (block-uniform) the whole window is readable
 #pragma unroll
-        for (int u = 0; u < kFirLoads; ++u) {
-          const int g = g0 + c1 * 31 + lane;
-          const bool ok = u0 + u < per_warp && c1 * 31 + lane <= W && g >= prm.rd_lo && g < prm.rd_hi;
-          a[u] = ok ? __ldg(yb + (int64_t)s1 * prm.in_stride + g) : 0.0;
-          c1 += 3;
-          if (c1 >= cps) { c1 -= cps; ++s1; }
-        }
+      for (int sr = 0; sr < 6; ++sr) {
+        const double* ys = yb + sr * prm.in_stride;
+        double* ds = dif + sr * W;
+#pragma unroll 3
+        for (int w = tid; w < W; w += kFirThreads) ds[w] = __ldg(ys + w + 1) - __ldg(ys + w);
       }
-#pragma unroll
-      for (int u = 0; u < kFirLoads; ++u) {
-        const double c = __shfl_down_sync(0xffffffffu, a[u], 1);
-        const int w = chunk * 31 + lane;
-        if (u0 + u < per_warp && lane < 31 && w < W) dif[sr * W + w] = c - a[u];
-        chunk += 3;
-        if (chunk >= cps) { chunk -= cps; ++sr; }
+    } else {
+      for (int sr = 0; sr < 6; ++sr) {
+        const double* ys = yb + sr * prm.in_stride;
+        for (int w = tid; w < W; w += kFirThreads) {
+          const int g = g0 + w;
+          const double a = (g >= prm.rd_lo && g < prm.rd_hi) ? __ldg(ys + w) : 0.0;
+          const double c = (g + 1 >= prm.rd_lo && g + 1 < prm.rd_hi) ? __ldg(ys + w + 1) : 0.0;
+          dif[sr * W + w] = c - a;
+        }
       }
     }
   }
