@@ -46,6 +46,12 @@ LR_HD int rot_slot_rt(int s, int r) {
        : (i == 0 && j == 2) ? 3 : (i == 2 && j == 1) ? 4 : 5;
 }
 
+// the link slots of the four series of channel ch (X, Y, Z = rotation by ch), three bits each
+__host__ __device__ constexpr int fir_slot_word(int ch) {
+  return rot_slot(fir_base_slot(0), ch) | rot_slot(fir_base_slot(1), ch) << 3 | rot_slot(fir_base_slot(2), ch) << 6 |
+         rot_slot(fir_base_slot(3), ch) << 9;
+}
+
 template <int NN> LR_HD double fir_node(int i);
 template <> LR_HD double fir_node<3>(int i) { return i == 0 ? -1.0 : i == 1 ? 0.0 : 1.0; }
 template <> LR_HD double fir_node<4>(int i) { return i == 0 ? -1.0 : i == 1 ? -0.5 : i == 2 ? 0.5 : 1.0; }
@@ -230,6 +236,7 @@ LR_HD void fir_apply(const double* dif, int W, const double* K, int Wc, int pad,
   for (int w = tid; w < 3 * groups; w += nthreads) {
     const int ch = w / groups, g = w - ch * groups;
     const int i0 = g * R;                                  // first sample of the group inside the tile
+    const int slots = ch == 0 ? fir_slot_word(0) : ch == 1 ? fir_slot_word(1) : fir_slot_word(2);
     double acc[NN][R];
 #pragma unroll
     for (int p = 0; p < NN; ++p)
@@ -237,7 +244,7 @@ LR_HD void fir_apply(const double* dif, int W, const double* K, int Wc, int pad,
       for (int r = 0; r < R; ++r) acc[p][r] = 0.0;
 #pragma unroll 1
     for (int sl = 0; sl < 4; ++sl) {
-      const double* d = dif + rot_slot_rt(fir_base_slot(sl), ch) * W + (nl0 + i0 - back);
+      const double* d = dif + ((slots >> (3 * sl)) & 7) * W + (nl0 + i0 - back);
       int koff = (ch * 4 + sl) * Wc * kFirKStride;
 #if defined(__CUDA_ARCH__) && !defined(LR_FIR_NO_PIN)
       asm volatile("" : "+r"(koff));   // keep the tap offset in a register (ptxas otherwise rebuilds it per tap)
@@ -419,6 +426,10 @@ tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __r
   __syncthreads();
   fir_apply<NN, true>(dif, W, K, Wc, Wc - prm.fir_taps, prm.p, prm.halo_lo, B, res, tid, kFirThreads);
   __syncthreads();
+  if (n0 + B <= prm.n && n0g >= v_lo && n0g + B <= v_hi) {   // (block-uniform) a full tile of valid samples
+    for (int i = tid; i < B; i += kFirThreads) fir_store(ob, N, n0 + i, channels, res[i], res[B + i], res[2 * B + i]);
+    return;
+  }
   for (int i = tid; i < B; i += kFirThreads) {
     const int n = n0 + i;
     if (n >= prm.n) break;
