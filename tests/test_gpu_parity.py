@@ -238,6 +238,16 @@ def test_orders(lr, order):
 
 
 # ---------------------------------------------------------------------------------------------- pins
+@pytest.mark.parametrize("knot_dt", [400.0, 1000.0, 1290.0])
+def test_dense_orbit_knots(lr, knot_dt):
+    """Orbit knots closer than a projection tile (128 samples = 1280 s): at 400 s a tile spans four spline
+    intervals and the kernel reads the coefficients from the global table; at 1000 s and 1290 s it spans two and
+    uses its tile-local copy, with the interval boundary inside nearly every tile (reading A9)."""
+    w = inputs.config(2, n=4001, f0=3e-3, t0=2.0e7)
+    tab = inputs.orbit_table("kepler", w.t0, w.t0 + w.n * w.dt, knot_dt=knot_dt, pad=20000.0)
+    check_workload(lr, w, tab=tab)
+
+
 def test_gpu_laser_noise_suppression(lr):
     """Pin P3 run on the GPU TDI: three independent band-limited laser-noise series, y_ij = p_j(t - L_ij(t))
     - p_i(t) evaluated analytically; second-generation NESTED TDI must cancel them to interpolation level,
