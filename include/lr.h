@@ -167,6 +167,31 @@ int lr_response_host(lr_handle* h_proj, lr_handle* h_tdi, const double* h_plus, 
                      const double* beta, const double* lambda, const double* psi, int64_t batch, int64_t n,
                      double* out, void* cuda_stream);
 
+/* Template generator (eqs. 5-9; SURVEY.md §8(f) NEXT-1 "generate the GB waveform
+ * from the parameters").  One template is LR_GB_NPAR doubles
+ *   gb = { a_plus, a_cross, f0 [Hz], fdot [Hz/s], fddot [Hz/s^2], phi0 [rad] }
+ * and its polarisations at t_n = t0 + n dt (t0 = LR_OPT_T0 of the handle, dt = the handle's) are
+ *   h_plus[n]  = a_plus  cos( 2 pi (f0 t_n + fdot t_n^2 / 2 + fddot t_n^3 / 6) + phi0 )      eq. 5a
+ *   h_cross[n] = a_cross sin( same argument )                                                eq. 5b
+ * Eq. 9's inclination factors and signs are the caller's amplitudes (paper: a_plus = -A (1 + cos^2 iota),
+ * a_cross = -2 A cos iota; BASELINE.json's configs: a_plus = +A (1 + cos^2 iota)); eq. 9's rotation by 2 psi
+ * is applied by lr_project to the basis (reading A4); eq. 8 gives the paper's fddot = 11/3 fdot^2 / f0.
+ * The phase is reduced modulo one cycle in double-double arithmetic before it is rounded, so the samples are
+ * correct to a few ulp of the amplitude however many cycles have gone by.
+ * gb: HOST [batch][LR_GB_NPAR] (read before the call returns); h_plus, h_cross: DEVICE [batch][n].
+ * Errors: LR_EINVAL (null pointer, non-finite parameter, bad sizes), LR_ECUDA. */
+#define LR_GB_NPAR 6
+int lr_gb_waveform(lr_handle* h, const double* gb, int64_t batch, int64_t n, double* h_plus, double* h_cross,
+                   void* cuda_stream);
+
+/* Parameters -> TDI channels in one call: lr_gb_waveform, lr_project (on h_proj) and lr_tdi (on h_tdi, may be
+ * the same handle) chunk by chunk along time; neither h nor y exists as a whole array, both live in scratch
+ * of h_proj that stays in L2 between producer and consumer.  out: DEVICE [batch][3|6][n], bit-identical to
+ * lr_response on the output of lr_gb_waveform.  gb, beta, lambda, psi: HOST, read before the call returns.
+ * Errors: as lr_gb_waveform and lr_response. */
+int lr_response_gb(lr_handle* h_proj, lr_handle* h_tdi, const double* gb, const double* beta, const double* lambda,
+                   const double* psi, int64_t batch, int64_t n, double* out, void* cuda_stream);
+
 /* Noise-weighted inner product of frequency-domain channels (eqs. 2-3, 22):
  *   LR_IP_CROSS : out[b] = scale * sum_{ch,k} Re( conj(fa[b][ch][k]) fb[b'][ch][k] ) * inv_psd[ch][k]
  *   LR_IP_DIFF  : out[b] = scale * sum_{ch,k} | fa[b][ch][k] - fb[b'][ch][k] |^2   * inv_psd[ch][k]

@@ -20,6 +20,7 @@ LR_OPT_T0, LR_OPT_CHAIN, LR_OPT_CHANNELS, LR_OPT_TDI_GEN, LR_OPT_TDI_PATH = 1, 2
 LR_OPT_TDI_PLAN_CACHE = 6
 LR_OPT_CHUNK_SAMPLES = 7
 LR_IP_CROSS, LR_IP_DIFF, LR_IP_BLOCKS = 0, 1, 1024
+LR_GB_NPAR = 6
 LR_TDI_AUTO, LR_TDI_PER_SAMPLE, LR_TDI_FIR3, LR_TDI_FIR4 = -1, 0, 3, 4
 LR_CHAIN_NESTED, LR_CHAIN_SUM = 0, 1
 LR_XYZ, LR_AET, LR_XYZ_AET = 0, 1, 2
@@ -27,7 +28,7 @@ LR_MAX_ORDER = 65
 
 # every symbol include/lr.h declares
 SYMBOLS = ("lr_create", "lr_destroy", "lr_set_option", "lr_get_margins", "lr_project", "lr_tdi",
-           "lr_inner_product", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count",
+           "lr_inner_product", "lr_gb_waveform", "lr_response_gb", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count",
            "lr_last_cuda_error", "lr_strerror")
 
 
@@ -78,6 +79,8 @@ def lib():
     L.lr_get_span_halo.argtypes = [vp, vp, pi64, pi64, pi64]
     L.lr_response_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
     L.lr_inner_product.argtypes = [vp, vp, vp, dbl, ci, i64, i64, ci, i64, vp, vp, vp]
+    L.lr_gb_waveform.argtypes = [vp, vp, i64, i64, vp, vp, vp]
+    L.lr_response_gb.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
     L.lr_eval_orbit.argtypes = [vp, ci, vp, i64, vp, vp]
     L.lr_measure_fp64_peak.argtypes = [dbl, ctypes.POINTER(dbl)]
     L.lr_launch_count.argtypes = []
@@ -223,6 +226,38 @@ def lr_response_host(h_proj, h_tdi, h_plus, h_cross, beta, lam, psi, out, stream
                                   lam.ctypes.data, psi.ctypes.data, B, n, o.ctypes.data,
                                   _stream(stream) if stream is not None else _stream(None)),
            "lr_response_host", h_proj)
+    return out
+
+
+def _gb(gb):
+    g = np.ascontiguousarray(np.asarray(gb, dtype=np.float64))
+    if g.ndim == 1:
+        g = g[None]
+    if g.ndim != 2 or g.shape[1] != LR_GB_NPAR:
+        raise ValueError("gb must be [batch, 6] = a_plus, a_cross, f0, fdot, fddot, phi0")
+    return g
+
+
+def lr_gb_waveform(h, gb, n, h_plus, h_cross, stream=None):
+    """lr_gb_waveform: gb host [B, 6] -> h_plus, h_cross CUDA [B, n] (written)."""
+    g = _gb(gb)
+    B = g.shape[0]
+    _check(lib().lr_gb_waveform(h, g.ctypes.data, B, int(n), _dev_ptr(h_plus, "h_plus", B * n),
+                                _dev_ptr(h_cross, "h_cross", B * n), _stream(stream)), "lr_gb_waveform", h)
+    return h_plus, h_cross
+
+
+def lr_response_gb(h_proj, h_tdi, gb, beta, lam, psi, n, out, stream=None):
+    """lr_response_gb: waveform parameters host [B, 6] + sky angles -> out CUDA [B, 3|6, n]."""
+    g = _gb(gb)
+    beta, lam, psi = _host(beta), _host(lam), _host(psi)
+    B = g.shape[0]
+    if beta.size != B or lam.size != B or psi.size != B:
+        raise ValueError("beta, lambda, psi must have one entry per template")
+    if out.numel() not in (3 * B * n, 6 * B * n):
+        raise ValueError("out must be [batch,3,n] or [batch,6,n]")
+    _check(lib().lr_response_gb(h_proj, h_tdi, g.ctypes.data, beta.ctypes.data, lam.ctypes.data, psi.ctypes.data,
+                                B, int(n), _dev_ptr(out, "out"), _stream(stream)), "lr_response_gb", h_proj)
     return out
 
 

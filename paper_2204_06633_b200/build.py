@@ -9,7 +9,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "liblr.so")
-SOURCES = ("lr_api.cu", "lr_kernels.cu", "lr_peak.cu", "lr_likelihood.cu")
+SOURCES = ("lr_api.cu", "lr_kernels.cu", "lr_peak.cu", "lr_likelihood.cu", "lr_waveform.cu")
 INST_PT = (21, 16, 13, 0, 11, 8, 7, 6, 5, 4, 3, 2, 1)   # lr_inst.cu is compiled once per compile-time pair count (0 = run-time P)
 HEADERS = ("lr_inst.cu", "lr_device.cuh", "lr_kernels.cuh", "lr_tdi_fir.cuh", "lr_host.hpp", os.path.join("..", "..", "include", "lr.h"))
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

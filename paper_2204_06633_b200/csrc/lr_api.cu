@@ -9,6 +9,7 @@
 #include <string.h>
 
 #include <atomic>
+#include <cmath>
 #include <new>
 #include <vector>
 
@@ -18,6 +19,8 @@
 
 namespace lr {
 extern std::atomic<int64_t> g_launches;
+int launch_gb_waveform(const double* gb_dev, double t0, double dt, int64_t batch, int64_t first, int64_t count,
+                       int64_t stride, double* hp, double* hc, void* stream);   // lr_waveform.cu
 }
 
 namespace {
@@ -131,8 +134,10 @@ bool in_table(const lr_handle* h, int64_t n_first, int64_t n_last, double back_r
   return lo >= 0 && hi <= span;
 }
 
+// Stages the per-template constants of one launch: the source basis [batch][9] and, when `gb` is given, the
+// waveform parameters [batch][6] right behind it (device pointer returned in *gb_dev).
 int stage_basis(lr_handle* h, const double* beta, const double* lam, const double* psi, int64_t batch,
-                cudaStream_t st, Stage** used) {
+                cudaStream_t st, Stage** used, const double* gb = nullptr, const double** gb_dev = nullptr) {
   Stage& S = h->stage[h->next_slot];
   h->next_slot = (h->next_slot + 1) % kSlots;
   if (!S.done) LR_CUDA(h, cudaEventCreateWithFlags(&S.done, cudaEventDisableTiming));
@@ -141,12 +146,15 @@ int stage_basis(lr_handle* h, const double* beta, const double* lam, const doubl
     if (S.host) cudaFreeHost(S.host);
     if (S.dev) cudaFree(S.dev);
     S.host = nullptr; S.dev = nullptr; S.cap = 0;
-    LR_CUDA(h, cudaMallocHost(&S.host, (size_t)batch * 9 * sizeof(double)));
-    LR_CUDA(h, cudaMalloc(&S.dev, (size_t)batch * 9 * sizeof(double)));
+    LR_CUDA(h, cudaMallocHost(&S.host, (size_t)batch * 15 * sizeof(double)));
+    LR_CUDA(h, cudaMalloc(&S.dev, (size_t)batch * 15 * sizeof(double)));
     S.cap = batch;
   }
   for (int64_t b = 0; b < batch; ++b) lr::source_basis(beta[b], lam[b], psi[b], S.host + 9 * b);
-  LR_CUDA(h, cudaMemcpyAsync(S.dev, S.host, (size_t)batch * 9 * sizeof(double), cudaMemcpyHostToDevice, st));
+  if (gb) memcpy(S.host + 9 * batch, gb, (size_t)batch * 6 * sizeof(double));
+  LR_CUDA(h, cudaMemcpyAsync(S.dev, S.host, (size_t)batch * (gb ? 15 : 9) * sizeof(double), cudaMemcpyHostToDevice,
+                             st));
+  if (gb_dev) *gb_dev = S.dev + 9 * batch;
   *used = &S;
   return LR_OK;
 }
@@ -656,6 +664,84 @@ int lr_response_host(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const
   LR_CUDA(h, cudaStreamWaitEvent(st, h->ev_out[0], 0));
   if (c >= 2) LR_CUDA(h, cudaStreamWaitEvent(st, h->ev_out[1], 0));
   LR_CUDA(h, cudaStreamSynchronize(st));
+  return LR_OK;
+}
+
+int lr_gb_waveform(lr_handle* h, const double* gb, int64_t batch, int64_t n, double* h_plus, double* h_cross,
+                   void* stream) {
+  if (!h || !gb || !h_plus || !h_cross || !size_ok(batch, n)) return LR_EINVAL;
+  for (int64_t i = 0; i < batch * 6; ++i)
+    if (!std::isfinite(gb[i])) return LR_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  for (int64_t b0 = 0; b0 < batch; b0 += 32768) {   // grid.y limit
+    const int64_t nb = batch - b0 < 32768 ? batch - b0 : 32768;
+    std::vector<double> zero((size_t)nb, 0.0);
+    Stage* S = nullptr;
+    const double* gb_dev = nullptr;
+    int rc = stage_basis(h, zero.data(), zero.data(), zero.data(), nb, st, &S, gb + b0 * 6, &gb_dev);
+    if (rc != LR_OK) return rc;
+    LR_CUDA(h, (cudaError_t)lr::launch_gb_waveform(gb_dev, h->t0, h->dt, nb, 0, n, n, h_plus + b0 * n,
+                                                   h_cross + b0 * n, stream));
+    LR_CUDA(h, cudaEventRecord(S->done, st));
+    S->pending = true;
+  }
+  return LR_OK;
+}
+
+int lr_response_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const double* beta, const double* lam,
+                   const double* psi, int64_t batch, int64_t n, double* out, void* stream) {
+  lr_handle* h = hp_;
+  if (!h || !ht_ || !gb || !beta || !lam || !psi || !out) return LR_EINVAL;
+  int rc = check_project(h, batch, n);
+  if (rc == LR_OK) rc = check_tdi(ht_, batch, n);
+  if (rc != LR_OK) return rc;
+  for (int64_t i = 0; i < batch * 6; ++i)
+    if (!std::isfinite(gb[i])) return LR_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  const TdiShape ts = tdi_shape(ht_);
+  const int nout = ht_->channels == LR_XYZ_AET ? 6 : 3;
+  const int64_t mp = h->m_proj();
+  // the chunk loop of lr_response with one more kernel in front: the chunk's h (with the halos of both stages)
+  // is generated into a scratch that, like y, stays in L2 between its producer and its consumer
+  const int64_t bc = batch < 8 ? batch : 8;
+  const int64_t budget = ((int64_t)40 << 20) / (bc * 6 * (int64_t)sizeof(double));
+  int64_t lc = budget / kChunkUnit * kChunkUnit;
+  if (lc < 4 * kChunkUnit) lc = 4 * kChunkUnit;
+  if (h->chunk_samples > 0) lc = round_up(h->chunk_samples, kChunkUnit);
+  if (lc > round_up(n, kChunkUnit)) lc = round_up(n, kChunkUnit);
+  const int64_t ly = round_up(lc + ts.halo_lo + ts.halo_hi, 2);
+  const int64_t lh = ly + 2 * mp;
+  rc = ensure(h, &h->y_scr, &h->y_cap, (size_t)(2 * bc * 6 * ly));
+  if (rc == LR_OK) rc = ensure_fix_events(h);
+  if (rc == LR_OK) rc = ensure(h, &h->h_buf, &h->h_cap, (size_t)(2 * 2 * bc * lh));
+  if (rc != LR_OK) return rc;
+  cudaEvent_t pending[2] = {nullptr, nullptr};   // fix-up kernels still reading y slot 0 / 1
+  int64_t c = 0;
+  for (int64_t b0 = 0; b0 < batch; b0 += bc) {
+    const int64_t nb = batch - b0 < bc ? batch - b0 : bc;
+    Stage* S = nullptr;
+    const double* gb_dev = nullptr;
+    rc = stage_basis(h, beta + b0, lam + b0, psi + b0, nb, st, &S, gb + b0 * 6, &gb_dev);
+    if (rc != LR_OK) return rc;
+    for (int64_t a = 0; a < n; a += lc, ++c) {
+      const int slot = (int)(c & 1);
+      const int64_t b = a + lc < n ? a + lc : n;
+      const int64_t ya = a - ts.halo_lo > 0 ? a - ts.halo_lo : 0, yb = b + ts.halo_hi < n ? b + ts.halo_hi : n;
+      const int64_t ha = ya - mp > 0 ? ya - mp : 0, hb = yb + mp < n ? yb + mp : n;
+      double* hp_d = h->h_buf + (size_t)slot * 2 * bc * lh;
+      double* hc_d = hp_d + (size_t)bc * lh;
+      LR_CUDA(h, (cudaError_t)lr::launch_gb_waveform(gb_dev, h->t0, h->dt, nb, ha, hb - ha, lh, hp_d, hc_d, stream));
+      if (pending[slot]) LR_CUDA(h, cudaStreamWaitEvent(st, pending[slot], 0));
+      pending[slot] = h->ev_fix[slot];
+      rc = response_chunk(h, ht_, ts, hp_d, hc_d, ha, hb, lh, S->dev, nb, n, a, b, ly,
+                          out + b0 * nout * n + a, n, stream, h->y_scr + (size_t)slot * bc * 6 * ly, &pending[slot]);
+      if (rc != LR_OK) return rc;
+    }
+    LR_CUDA(h, cudaEventRecord(S->done, st));
+    S->pending = true;
+  }
+  for (int i = 0; i < 2; ++i)   // join the last fix-up kernels
+    if (pending[i]) LR_CUDA(h, cudaStreamWaitEvent(st, pending[i], 0));
   return LR_OK;
 }
 

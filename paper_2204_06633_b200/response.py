@@ -4,6 +4,8 @@ No arithmetic of the method lives here.
 """
 from __future__ import annotations
 
+import numpy as np
+
 from . import binding as B
 
 _CHANNELS = {"XYZ": B.LR_XYZ, "AET": B.LR_AET, "XYZ_AET": B.LR_XYZ_AET}
@@ -112,6 +114,24 @@ class Response:
 
     def response_host(self, h_plus, h_cross, beta, lam, psi, out, tdi=None, stream=None):
         return B.lr_response_host(self._h, (tdi or self)._h, h_plus, h_cross, beta, lam, psi, out, stream)
+
+    def gb_waveform(self, gb, n, stream=None):
+        """(h_plus, h_cross) CUDA [B, n] of the Galactic binaries gb [B, 6] (eqs. 5-9)."""
+        import torch
+        nb = np.asarray(gb, dtype=np.float64).reshape(-1, B.LR_GB_NPAR).shape[0]
+        hp = torch.empty((nb, n), dtype=torch.float64, device="cuda")
+        hc = torch.empty_like(hp)
+        B.lr_gb_waveform(self._h, gb, n, hp, hc, stream)
+        return hp, hc
+
+    def response_gb(self, gb, beta, lam, psi, n, out=None, tdi=None, stream=None):
+        """Parameters -> TDI channels (CUDA [B, 3|6, n]); h and y only exist chunk-wise in scratch."""
+        import torch
+        t = tdi or self
+        nb = np.asarray(gb, dtype=np.float64).reshape(-1, B.LR_GB_NPAR).shape[0]
+        if out is None:
+            out = torch.empty((nb, t.n_out, n), dtype=torch.float64, device="cuda")
+        return B.lr_response_gb(self._h, t._h, gb, beta, lam, psi, n, out, stream)
 
     def close(self):
         if self._h is not None:
