@@ -209,6 +209,22 @@ int lr_inner_product(const double* fa, const double* fb, const double* inv_psd, 
                      int64_t batch, int64_t batch_b, int nch, int64_t nf, double* work, double* out,
                      void* cuda_stream);
 
+/* One likelihood evaluation per template, parameters in, one scalar out ("only the scalar
+ * returns"; eqs. 2-3, 5-9, 10-22): lr_response_gb into scratch, the library's real-to-complex FFT (cuFFT, fp64)
+ * of the three TDI channels, lr_inner_product against one data set:
+ *   out[b] = scale * sum_{ch,k} inv_psd[ch][k] * ( mode LR_IP_DIFF ? |H_b[ch][k] - data_f[ch][k]|^2
+ *                                                                   : Re( conj(H_b[ch][k]) data_f[ch][k] ) )
+ * with H_b[ch][k] = sum_n out_b[ch][n] exp(-2 pi i k n / N), k = 0 .. N/2 — the UNNORMALISED forward DFT of the
+ * channels (margins are zeros); data_f must be in the same convention.  log L of eq. 3 with a~ = dt * DFT is
+ * scale = -2 dt / N, mode LR_IP_DIFF, inv_psd[ch][0] = 0.
+ * h_tdi must produce three channels (LR_XYZ or LR_AET).  gb, beta, lambda, psi: HOST [batch]...; data_f: DEVICE
+ * complex [3][N/2+1] (interleaved re, im); inv_psd: DEVICE [3][N/2+1]; out: DEVICE [batch].  Scratch (the
+ * channels and spectra of 8 templates, the FFT plan) is owned by h_proj and kept until lr_destroy.
+ * Errors: LR_EINVAL (as lr_response_gb, or six output channels), LR_ECUDA (CUDA or cuFFT failure). */
+int lr_loglike_gb(lr_handle* h_proj, lr_handle* h_tdi, const double* gb, const double* beta, const double* lambda,
+                  const double* psi, int64_t batch, int64_t n, const double* data_f, const double* inv_psd,
+                  double scale, int mode, double* out, void* cuda_stream);
+
 /* Evaluate the device spline of one orbit channel (0..8 = x[i][a] as i*3+a, 9..14 = L link slots) at
  * `m` times t (DEVICE [m]) into out (DEVICE [m]); used by the tests to pin the orbit ingestion. */
 int lr_eval_orbit(lr_handle* h, int channel, const double* t, int64_t m, double* out, void* cuda_stream);

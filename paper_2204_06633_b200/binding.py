@@ -28,7 +28,7 @@ LR_MAX_ORDER = 65
 
 # every symbol include/lr.h declares
 SYMBOLS = ("lr_create", "lr_destroy", "lr_set_option", "lr_get_margins", "lr_project", "lr_tdi",
-           "lr_inner_product", "lr_gb_waveform", "lr_response_gb", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count",
+           "lr_inner_product", "lr_gb_waveform", "lr_response_gb", "lr_loglike_gb", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count",
            "lr_last_cuda_error", "lr_strerror")
 
 
@@ -81,6 +81,7 @@ def lib():
     L.lr_inner_product.argtypes = [vp, vp, vp, dbl, ci, i64, i64, ci, i64, vp, vp, vp]
     L.lr_gb_waveform.argtypes = [vp, vp, i64, i64, vp, vp, vp]
     L.lr_response_gb.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
+    L.lr_loglike_gb.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, vp, vp, dbl, ci, vp, vp]
     L.lr_eval_orbit.argtypes = [vp, ci, vp, i64, vp, vp]
     L.lr_measure_fp64_peak.argtypes = [dbl, ctypes.POINTER(dbl)]
     L.lr_launch_count.argtypes = []
@@ -258,6 +259,28 @@ def lr_response_gb(h_proj, h_tdi, gb, beta, lam, psi, n, out, stream=None):
         raise ValueError("out must be [batch,3,n] or [batch,6,n]")
     _check(lib().lr_response_gb(h_proj, h_tdi, g.ctypes.data, beta.ctypes.data, lam.ctypes.data, psi.ctypes.data,
                                 B, int(n), _dev_ptr(out, "out"), _stream(stream)), "lr_response_gb", h_proj)
+    return out
+
+
+def lr_loglike_gb(h_proj, h_tdi, gb, beta, lam, psi, n, data_f, inv_psd, scale, mode=LR_IP_DIFF, out=None,
+                  stream=None):
+    """lr_loglike_gb: waveform parameters host [B, 6] + sky angles -> out CUDA float64 [B]; data_f CUDA
+    complex128 [3, n//2+1] (unnormalised DFT), inv_psd CUDA float64 [3, n//2+1]."""
+    import torch
+    g = _gb(gb)
+    beta, lam, psi = _host(beta), _host(lam), _host(psi)
+    B = g.shape[0]
+    nf = n // 2 + 1
+    if beta.size != B or lam.size != B or psi.size != B:
+        raise ValueError("beta, lambda, psi must have one entry per template")
+    if not (isinstance(data_f, torch.Tensor) and data_f.is_cuda and data_f.dtype == torch.complex128
+            and data_f.is_contiguous() and data_f.numel() == 3 * nf):
+        raise TypeError("data_f must be a contiguous CUDA complex128 tensor [3, n//2+1]")
+    if out is None:
+        out = torch.empty(B, dtype=torch.float64, device=data_f.device)
+    _check(lib().lr_loglike_gb(h_proj, h_tdi, g.ctypes.data, beta.ctypes.data, lam.ctypes.data, psi.ctypes.data, B,
+                               int(n), data_f.data_ptr(), _dev_ptr(inv_psd, "inv_psd", 3 * nf), float(scale),
+                               int(mode), _dev_ptr(out, "out", B), _stream(stream)), "lr_loglike_gb", h_proj)
     return out
 
 

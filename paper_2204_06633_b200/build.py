@@ -57,7 +57,10 @@ def build(force=False, verbose=False):
         results = list(ex.map(compile_one, jobs))
     objs = [o for o, _ in results]
     tmp = LIB + ".tmp"
-    r = subprocess.run([nvcc, "-shared", "-o", tmp, *objs, "-cudart", "static"], capture_output=True, text=True)
+    # cuFFT (the likelihood leg's real-to-complex transform) is the one library liblr links dynamically
+    cuda_lib = os.path.join(os.path.dirname(os.path.dirname(os.path.realpath(nvcc))), "lib64")
+    r = subprocess.run([nvcc, "-shared", "-o", tmp, *objs, "-cudart", "static", "-L" + cuda_lib, "-lcufft",
+                        "-Xlinker", "-rpath=" + cuda_lib], capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
     os.replace(tmp, LIB)

@@ -4,6 +4,7 @@
 // lr_project / lr_tdi marshal arguments and launch the kernels of lr_kernels.cuh on the caller's stream.
 // There is no CPU compute path: without a CUDA device every computing call returns LR_ECUDA.
 #include <cuda_runtime.h>
+#include <cufft.h>
 #include <math.h>
 #include <stdint.h>
 #include <string.h>
@@ -77,6 +78,10 @@ struct lr_handle {
   cudaStream_t s_in = nullptr, s_out = nullptr;
   cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
   cudaEvent_t ev_fix[2] = {nullptr, nullptr};       // fix-up kernel of the chunk in y slot 0 / 1 finished
+  // lr_loglike_gb: spectra of one template chunk, partial sums of the inner product, the cached FFT plan
+  double* f_buf = nullptr; size_t f_cap = 0;
+  double* ip_work = nullptr; size_t ip_cap = 0;
+  cufftHandle fft = 0; int64_t fft_n = 0;
   int last_cuda = 0;
 
   int64_t m_proj() const {
@@ -246,6 +251,9 @@ void lr_destroy(lr_handle* h) {
   if (h->y_scr) cudaFree(h->y_scr);
   if (h->h_buf) cudaFree(h->h_buf);
   if (h->o_buf) cudaFree(h->o_buf);
+  if (h->f_buf) cudaFree(h->f_buf);
+  if (h->ip_work) cudaFree(h->ip_work);
+  if (h->fft_n) cufftDestroy(h->fft);
   for (int i = 0; i < 2; ++i) {
     if (h->ev_in[i]) cudaEventDestroy(h->ev_in[i]);
     if (h->ev_comp[i]) cudaEventDestroy(h->ev_comp[i]);
@@ -688,8 +696,12 @@ int lr_gb_waveform(lr_handle* h, const double* gb, int64_t batch, int64_t n, dou
   return LR_OK;
 }
 
-int lr_response_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const double* beta, const double* lam,
-                   const double* psi, int64_t batch, int64_t n, double* out, void* stream) {
+}  // extern "C"
+
+namespace {
+// lr_response_gb with a row stride for out ([batch][3|6] rows of o_stride >= n doubles)
+int response_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const double* beta, const double* lam,
+                const double* psi, int64_t batch, int64_t n, double* out, int64_t o_stride, void* stream) {
   lr_handle* h = hp_;
   if (!h || !ht_ || !gb || !beta || !lam || !psi || !out) return LR_EINVAL;
   int rc = check_project(h, batch, n);
@@ -734,7 +746,8 @@ int lr_response_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const doubl
       if (pending[slot]) LR_CUDA(h, cudaStreamWaitEvent(st, pending[slot], 0));
       pending[slot] = h->ev_fix[slot];
       rc = response_chunk(h, ht_, ts, hp_d, hc_d, ha, hb, lh, S->dev, nb, n, a, b, ly,
-                          out + b0 * nout * n + a, n, stream, h->y_scr + (size_t)slot * bc * 6 * ly, &pending[slot]);
+                          out + b0 * nout * o_stride + a, o_stride, stream, h->y_scr + (size_t)slot * bc * 6 * ly,
+                          &pending[slot]);
       if (rc != LR_OK) return rc;
     }
     LR_CUDA(h, cudaEventRecord(S->done, st));
@@ -742,6 +755,60 @@ int lr_response_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const doubl
   }
   for (int i = 0; i < 2; ++i)   // join the last fix-up kernels
     if (pending[i]) LR_CUDA(h, cudaStreamWaitEvent(st, pending[i], 0));
+  return LR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lr_response_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const double* beta, const double* lam,
+                   const double* psi, int64_t batch, int64_t n, double* out, void* stream) {
+  return response_gb(hp_, ht_, gb, beta, lam, psi, batch, n, out, n, stream);
+}
+
+int lr_loglike_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const double* beta, const double* lam,
+                  const double* psi, int64_t batch, int64_t n, const double* data_f, const double* inv_psd,
+                  double scale, int mode, double* out, void* stream) {
+  lr_handle* h = hp_;
+  if (!h || !ht_ || !gb || !beta || !lam || !psi || !data_f || !inv_psd || !out) return LR_EINVAL;
+  if (ht_->channels == LR_XYZ_AET || n < 2 || n > 0x7fffffff) return LR_EINVAL;   // three channels per template
+  if (mode != LR_IP_CROSS && mode != LR_IP_DIFF) return LR_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t nf = n / 2 + 1;
+  const int64_t bc = batch < 8 ? batch : 8;
+  const int64_t np = n + (n & 1);   // row stride of the channels: cuFFT wants 16-byte aligned transforms
+  int rc = ensure(h, &h->o_buf, &h->o_cap, (size_t)(bc * 3 * np));
+  if (rc == LR_OK) rc = ensure(h, &h->f_buf, &h->f_cap, (size_t)(bc * 3 * nf * 2));
+  if (rc == LR_OK) rc = ensure(h, &h->ip_work, &h->ip_cap, (size_t)(bc * LR_IP_BLOCKS));
+  if (rc != LR_OK) return rc;
+  if (h->fft_n != n) {   // one plan of three real-to-complex transforms (the channels of one template), kept
+    if (h->fft_n) { cufftDestroy(h->fft); h->fft_n = 0; }
+    int len = (int)n;
+    int in_len = (int)np, out_len = (int)nf;
+    const cufftResult fr = cufftPlanMany(&h->fft, 1, &len, &in_len, 1, (int)np, &out_len, 1, (int)nf, CUFFT_D2Z, 3);
+    if (fr != CUFFT_SUCCESS) {
+      h->last_cuda = 10000 + (int)fr;   // cuFFT result codes are reported as 10000 + cufftResult
+      return LR_ECUDA;
+    }
+    h->fft_n = n;
+  }
+  if (cufftSetStream(h->fft, st) != CUFFT_SUCCESS) { h->last_cuda = 10000; return LR_ECUDA; }
+  for (int64_t b0 = 0; b0 < batch; b0 += bc) {
+    const int64_t nb = batch - b0 < bc ? batch - b0 : bc;
+    rc = response_gb(hp_, ht_, gb + b0 * 6, beta + b0, lam + b0, psi + b0, nb, n, h->o_buf, np, stream);
+    if (rc != LR_OK) return rc;
+    for (int64_t b = 0; b < nb; ++b) {
+      const cufftResult fr = cufftExecD2Z(h->fft, h->o_buf + b * 3 * np,
+                                          reinterpret_cast<cufftDoubleComplex*>(h->f_buf) + b * 3 * nf);
+      if (fr != CUFFT_SUCCESS) {
+        h->last_cuda = 20000 + (int)fr;   // 20000 + cufftResult: the transform itself
+        return LR_ECUDA;
+      }
+    }
+    rc = lr_inner_product(h->f_buf, data_f, inv_psd, scale, mode, nb, 1, 3, nf, h->ip_work, out + b0, stream);
+    if (rc != LR_OK) return rc;
+  }
   return LR_OK;
 }
 

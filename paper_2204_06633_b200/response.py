@@ -133,6 +133,12 @@ class Response:
             out = torch.empty((nb, t.n_out, n), dtype=torch.float64, device="cuda")
         return B.lr_response_gb(self._h, t._h, gb, beta, lam, psi, n, out, stream)
 
+    def loglike_gb(self, gb, beta, lam, psi, n, data_f, inv_psd, scale, mode=B.LR_IP_DIFF, out=None, tdi=None,
+                   stream=None):
+        """Parameters -> one scalar per template (CUDA [B]): waveform, response, FFT, noise-weighted inner product."""
+        return B.lr_loglike_gb(self._h, (tdi or self)._h, gb, beta, lam, psi, n, data_f, inv_psd, scale, mode, out,
+                               stream)
+
     def close(self):
         if self._h is not None:
             B.lr_destroy(self._h)

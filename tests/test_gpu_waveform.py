@@ -101,3 +101,58 @@ def test_response_gb_errors(lr):
         R.response_gb(bad, [0.1], [0.2], [0.3], w.n, out=out)
     with pytest.raises(ValueError):
         R.response_gb(np.zeros((1, 5)), [0.1], [0.2], [0.3], w.n, out=out)
+
+
+def test_loglike_gb_against_oracle_pipeline(lr):
+    """Parameters -> log L in one call against the oracle chain: exact-phase waveform, long-double
+    projection and TDI (A, E, T), numpy FFT, eq. 3 accumulated in long double.  Data = template 1 (noiseless
+    injection), analytic stand-in PSD.  11 templates (two chunks of 8), odd N."""
+    import torch
+    from oracle import likelihood as lk
+    w = inputs.config(2, n=12001, f0=3e-3, t0=2.0e7)
+    tab = w.table()
+    rng = np.random.default_rng(5)
+    nb = 11
+    gb = np.empty((nb, 6))
+    for b in range(nb):
+        a = owf.amplitudes_paper(1e-22 * (1 + 0.1 * b), 0.3 + 0.2 * b)
+        f0 = 3e-3 * (1 + 1e-4 * rng.standard_normal())
+        gb[b] = (a[0], a[1], f0, 1e-16, owf.fddot_eq8(f0, 1e-16), rng.uniform(0, 2 * math.pi))
+    gb[7] = gb[1]                                             # a copy of the data's parameters: log L = 0
+    beta, lam, psi = rng.uniform(-1, 1, nb), rng.uniform(0, 6, nb), rng.uniform(0, 3, nb)
+    beta[7], lam[7], psi[7] = beta[1], lam[1], psi[1]
+    n, dt = w.n, w.dt
+    O = orc.Oracle(tab, dt, w.t0, w.order)
+    mp, mf, mb = O.margins(2)
+    aet = np.zeros((nb, 3, n))
+    for b in range(nb):
+        op, oc = owf.gb_waveform(gb[b], w.t0, dt, n)
+        y = O.project(op, oc, beta[b], lam[b], psi[b], lo=mp, hi=n - mp)
+        aet[b] = O.tdi(y, 2, nested=True, channels=ORC_CH["AET"], lo=mf, hi=n - mb)
+    f = np.fft.rfftfreq(n, dt)
+    psd = inputs.psd_standin(f)
+    inv = np.zeros_like(psd)
+    inv[:, 1:] = 1.0 / psd[:, 1:]
+    fh = lk.to_frequency(aet, dt)
+    want = np.array([lk.log_likelihood(fh[1], fh[b], psd, dt, n) for b in range(nb)], dtype=np.float64)
+
+    R = lr.Response(tab, dt, w.order, 2, t0=w.t0, channels="AET")
+    data_f = torch.from_numpy(np.ascontiguousarray(np.fft.rfft(aet[1], axis=-1))).cuda()   # unnormalised DFT
+    inv_d = to_dev(inv)
+    got = R.loglike_gb(gb, beta, lam, psi, n, data_f, inv_d, -2.0 * dt / n)
+    torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    assert np.all(got <= 0)
+    # the data are the ORACLE's template 1; the GPU's own template 1 differs from it by the path's 1e-13
+    assert abs(got[1]) <= 1e-20 * np.abs(want).max() and abs(got[7]) <= 1e-20 * np.abs(want).max()
+    others = [b for b in range(nb) if b not in (1, 7)]
+    assert np.abs(got[others] - want[others]).max() <= 1e-10 * np.abs(want).max()
+    # <h|d> mode, and the same call twice gives the same bits
+    cross = R.loglike_gb(gb, beta, lam, psi, n, data_f, inv_d, 4.0 * dt / n, mode=lr.LR_IP_CROSS).cpu().numpy()
+    want_c = lk.inner_product(fh, fh[1:2], psd, dt, n).astype(np.float64)
+    assert np.abs(cross - want_c).max() <= 1e-10 * np.abs(want_c).max()
+    again = R.loglike_gb(gb, beta, lam, psi, n, data_f, inv_d, -2.0 * dt / n).cpu().numpy()
+    assert np.array_equal(got, again)
+    R6 = lr.Response(tab, dt, w.order, 2, t0=w.t0, channels="XYZ_AET")
+    with pytest.raises(lr.LrError):
+        R6.loglike_gb(gb, beta, lam, psi, n, data_f, inv_d, 1.0)
