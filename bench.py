@@ -363,6 +363,56 @@ def run_gpu(args, rank, world, local_rank):
         del fh, ch3, inv_psd
     except Exception as exc:   # never let the optional leg break the contract line
         lk = {"error": repr(exc)}
+    # parameters -> log L in ONE call (waveform, projection, TDI, FFT and inner product on the device,
+    # "only the scalar returns"): lr_loglike_gb on a 3-channel (A,E,T) handle of the same orbits.  Wall clock
+    # around the call and the read-back of the scalars: host traffic is 120 B in and 8 B out per template.
+    pl = None
+    try:
+        if args.workload not in ("year", "batch", "tiny") or not all(s.f0 > 0 for s in w.sources[:8]):
+            raise RuntimeError("no Galactic-binary parameters in this workload")
+        nb = min(chunk, 8)
+        Ra = lr.Response(w.table(), w.dt, w.order, w.tdi_gen, t0=w.t0, chain="nested", channels="AET")
+        gb = np.array([[s.A * (1.0 + np.cos(s.iota) ** 2), -2.0 * s.A * np.cos(s.iota), s.f0, s.fdot, 0.0, s.phi0]
+                       for s in w.sources[:nb]])
+        be, la, ps = angles(0, nb)
+        nf = n // 2 + 1
+        inv_psd = torch.ones((3, nf), dtype=torch.float64, device=dev)
+        inv_psd[:, 0] = 0.0
+        aet0 = Ra.response_gb(gb[:1], be[:1], la[:1], ps[:1], n)
+        data_f = torch.fft.rfft(aet0[0], dim=-1).contiguous()
+        del aet0
+        tw, td = [], []
+        for it in range(7):
+            torch.cuda.synchronize()
+            t0w = time.perf_counter()
+            e0, e1 = ev(), ev()
+            e0.record(stream)
+            ll = Ra.loglike_gb(gb, be, la, ps, n, data_f, inv_psd, -2.0 * w.dt / n)
+            e1.record(stream)
+            ll_h = ll.cpu()
+            t1w = time.perf_counter()
+            if it >= 2:
+                tw.append((t1w - t0w) * 1e3)
+                td.append(e0.elapsed_time(e1))
+        ms_w, ms_d = float(np.median(tw)), float(np.median(td))
+        pl = {"api": "lr_loglike_gb (host: 15 doubles in, 1 double out per template)", "templates": nb,
+              "ms_per_call_wall": ms_w, "ms_per_call_device": ms_d, "ms_lr_response_gb": None,
+              "value": nb * n / (ms_w * 1e-3), "unit": "samples/s", "loglike_per_s": nb / (ms_w * 1e-3),
+              "h2d_bytes_per_call": int(nb * 15 * 8), "d2h_bytes_per_call": int(nb * 8),
+              "log_l_of_the_data_template": float(ll_h[0])}
+        outg = torch.empty((nb, 3, n), dtype=torch.float64, device=dev)
+        tg = []
+        for it in range(5):
+            e0, e1 = ev(), ev()
+            e0.record(stream)
+            Ra.response_gb(gb, be, la, ps, n, out=outg)
+            e1.record(stream)
+            e1.synchronize()
+            tg.append(e0.elapsed_time(e1))
+        pl["ms_lr_response_gb"] = float(np.median(tg[1:]))
+        del outg, data_f, inv_psd, Ra
+    except Exception as exc:   # never let the optional leg break the contract line
+        pl = {"error": repr(exc)}
     # the same steps with the FIR plan rebuilt by every lr_tdi call (plan kernel inside the timed region)
     Rt.set_plan_cache(False)
     cold = [step(True) for _ in range(max(3, min(args.steps, 10)))]
@@ -433,6 +483,7 @@ def run_gpu(args, rank, world, local_rank):
                     "lr_tdi": {"ms": ms_tdi, "alg_ops_per_sample": ops_t, "gops": ach_tdi / 1e9,
                                "frac_fp64": ach_tdi / peak, "alg_GBps": bytes_tdi(nout) * batch * n / (ms_tdi * 1e6)}},
         "likelihood": lk,
+        "params_to_loglike": pl,
         "lr_response": {"ms_per_step": ms_resp, "note": "one call, h -> out, y only in a <= 40 MB scratch"},
         "tdi_plan": {"cached_between_calls": True, "ms_tdi_with_plan_rebuilt_every_call": ms_tdi_cold,
                      "value_with_plan_rebuilt_every_call": units / (max_over_ranks(ms_proj + ms_tdi_cold) * 1e-3)
