@@ -133,8 +133,8 @@ int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out,
 
 /* Both stages with DEVICE buffers and no [batch][6][n] array: h_plus, h_cross DEVICE [batch][n] -> out DEVICE
  * [batch][3|6][n], bit-identical to lr_project followed by lr_tdi.  The path runs in chunks of time (and of
- * 8 templates) through a y scratch of <= 40 MB owned by h_proj, which stays L2-resident, so the device footprint
- * is h + out (the paper's real call is waveform -> projection -> TDI with nothing
+ * 8 templates) through a y scratch of two slots of <= 256 MB owned by h_proj, so the device footprint
+ * is h + out + that scratch (the paper's real call is waveform -> projection -> TDI with nothing
  * in between leaving the GPU).  Enqueues on `cuda_stream` and returns without synchronising.
  * beta, lambda, psi: HOST [batch].  Errors: as lr_project / lr_tdi. */
 int lr_response(lr_handle* h_proj, lr_handle* h_tdi, const double* h_plus, const double* h_cross,
@@ -186,7 +186,7 @@ int lr_gb_waveform(lr_handle* h, const double* gb, int64_t batch, int64_t n, dou
 
 /* Parameters -> TDI channels in one call: lr_gb_waveform, lr_project (on h_proj) and lr_tdi (on h_tdi, may be
  * the same handle) chunk by chunk along time; neither h nor y exists as a whole array, both live in scratch
- * of h_proj that stays in L2 between producer and consumer.  out: DEVICE [batch][3|6][n], bit-identical to
+ * of h_proj.  out: DEVICE [batch][3|6][n], bit-identical to
  * lr_response on the output of lr_gb_waveform.  gb, beta, lambda, psi: HOST, read before the call returns.
  * Errors: as lr_gb_waveform and lr_response. */
 int lr_response_gb(lr_handle* h_proj, lr_handle* h_tdi, const double* gb, const double* beta, const double* lambda,
