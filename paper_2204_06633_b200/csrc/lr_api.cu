@@ -663,9 +663,9 @@ int lr_response_host(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const
       // stage 3: D2H (after the chunk's kernels, the fix-up kernel on its side stream included)
       LR_CUDA(h, cudaStreamWaitEvent(h->s_out, h->ev_comp[slot], 0));
       if (pending[slot]) LR_CUDA(h, cudaStreamWaitEvent(h->s_out, pending[slot], 0));
-      for (int ch = 0; ch < nout; ++ch)   // rows [template][channel]: one 2-D copy per channel
-        LR_CUDA(h, cudaMemcpy2DAsync(out + (b0 * nout + ch) * n + a, (size_t)nout * n * dsz, o_d + (size_t)ch * lc,
-                                     (size_t)nout * lc * dsz, (b - a) * dsz, nb, cudaMemcpyDeviceToHost, h->s_out));
+      // rows [template][channel] have one pitch on either side (n on the host, lc in the staging buffer): one copy
+      LR_CUDA(h, cudaMemcpy2DAsync(out + b0 * nout * n + a, (size_t)n * dsz, o_d, (size_t)lc * dsz, (b - a) * dsz,
+                                   (size_t)nb * nout, cudaMemcpyDeviceToHost, h->s_out));
       LR_CUDA(h, cudaEventRecord(h->ev_out[slot], h->s_out));
     }
     LR_CUDA(h, cudaEventRecord(S->done, st));
