@@ -9,4 +9,4 @@ from .binding import (LR_AET, LR_CHAIN_NESTED, LR_CHAIN_SUM, LR_ECUDA, LR_EINVAL
                       LR_XYZ_AET, LrError, LrUnavailable, lr_create, lr_destroy, lr_eval_orbit, lr_get_margins,
                       lr_launch_count, lr_measure_fp64_peak, lr_get_span_halo, lr_inner_product, lr_gb_waveform, lr_response_gb, lr_loglike_gb, LR_GB_NPAR, lr_project, lr_response, lr_response_host, lr_response_span, lr_set_option,
                       lr_strerror, lr_tdi)
-from .response import Response, shard_templates, shard_time  # noqa: F401
+from .response import Response, gather_scalars, shard_templates, shard_time  # noqa: F401

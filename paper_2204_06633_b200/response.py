@@ -35,6 +35,30 @@ def shard_time(n, rank, world, unit, lo, hi):
     return first, end - first, h_first, (h_end - h_first if end > first else 0)
 
 
+def gather_scalars(local, batch, rank, world, group=None):
+    """The one exchange step of the path: every rank has the log-likelihoods of ITS templates
+    (`shard_templates(batch, rank, world)`); afterwards every rank has all `batch` of them, in template order.
+    One all-gather of at most ceil(batch / world) doubles per rank (NCCL for CUDA tensors, gloo for CPU ones);
+    shards of unequal length are padded for the collective and trimmed afterwards."""
+    import torch
+    import torch.distributed as dist
+    lo, hi = shard_templates(batch, rank, world)
+    if local.numel() != hi - lo:
+        raise ValueError("local must hold this rank's shard of the batch")
+    if world == 1:
+        return local.clone()
+    width = -(-batch // world)
+    padded = torch.zeros(width, dtype=local.dtype, device=local.device)
+    padded[:hi - lo] = local
+    gathered = torch.empty(world * width, dtype=local.dtype, device=local.device)
+    dist.all_gather_into_tensor(gathered, padded, group=group)
+    parts = []
+    for r in range(world):
+        a, b = shard_templates(batch, r, world)
+        parts.append(gathered[r * width:r * width + (b - a)])
+    return torch.cat(parts)
+
+
 class Response:
     """One orbit table + (dt, order, TDI generation): owns an lr_handle."""
 

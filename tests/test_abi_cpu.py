@@ -134,7 +134,7 @@ _GLOO_WORKER = r'''
 import os, sys
 sys.path.insert(0, sys.argv[1])
 import torch, torch.distributed as dist
-from paper_2204_06633_b200 import shard_templates, shard_time
+from paper_2204_06633_b200 import gather_scalars, shard_templates, shard_time
 import bench
 dist.init_process_group("gloo")
 rank, world = dist.get_rank(), dist.get_world_size()
@@ -150,6 +150,10 @@ first, count, h_first, h_len = shard_time(n, rank, world, 1792, 90, 87)
 cover = torch.zeros(n, dtype=torch.int64); cover[first:first + count] = 1
 dist.all_reduce(cover)
 assert bool((cover == 1).all())
+# the likelihood stage's only exchange: all-gather of the per-template scalars, unequal shards (11 over 2 ranks)
+mine = torch.arange(lo, hi, dtype=torch.float64) * 1.5 - 7.0
+full = gather_scalars(mine, batch, rank, world)
+assert torch.equal(full, torch.arange(batch, dtype=torch.float64) * 1.5 - 7.0), full
 # max-over-ranks timing + whole-job aggregation used by bench.py
 ms = bench.max_over_ranks(10.0 * (rank + 1))
 assert ms == 10.0 * world, ms
