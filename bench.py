@@ -410,13 +410,15 @@ def run_gpu(args, rank, world, local_rank):
             e1.synchronize()
             tg.append(e0.elapsed_time(e1))
         pl["ms_lr_response_gb"] = float(np.median(tg[1:]))
-        if world > 1:   # the path's only exchange: all-gather of the scalars, nb per rank
-            full = lr.gather_scalars(ll, nb * world, rank, world)
-            torch.cuda.synchronize()
-            pl["gathered_scalars"] = int(full.numel())
+
         del outg, data_f, inv_psd, Ra
     except Exception as exc:   # never let the optional leg break the contract line
         pl = {"error": repr(exc)}
+    if world > 1:   # the path's only exchange: all-gather of the scalars; every rank takes part
+        if sum_over_ranks(0.0 if "error" in pl else 1.0) == world:
+            full = lr.gather_scalars(ll, pl["templates"] * world, rank, world)
+            torch.cuda.synchronize()
+            pl["gathered_scalars"] = int(full.numel())
     # the same steps with the FIR plan rebuilt by every lr_tdi call (plan kernel inside the timed region)
     Rt.set_plan_cache(False)
     cold = [step(True) for _ in range(max(3, min(args.steps, 10)))]
