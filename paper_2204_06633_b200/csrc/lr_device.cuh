@@ -83,6 +83,14 @@ LR_HD D4 load4(const D4* p) {
 #endif
 }
 
+LR_HD double inv_sqrt(double x) {
+#ifdef __CUDA_ARCH__
+  return rsqrt(x);
+#else
+  return 1.0 / sqrt(x);
+#endif
+}
+
 // time of sample n relative to knot 0
 LR_HD double sample_trel(const Params& P, int n) { return fma((double)n, P.dt, P.trel0); }
 
@@ -172,7 +180,7 @@ LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W
                           const double* bs, Store store, const Coef& coef = Coef{}) {
   // geometry first (everything that needs the positions and the basis), so that only 12 doubles stay live
   // across the nine interpolations: Dr[3] and, per arm, xi+, xix, k.n
-  double Dr[3], xip[3], xic[3], kn[3];
+  double Dr[3], xip[3], xic[3], kn[3], rden[3];
   {
     const double k0 = bs[0], k1 = bs[1], k2 = bs[2];
     const double u0 = bs[3], u1 = bs[4], u2 = bs[5];
@@ -190,11 +198,16 @@ LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W
     for (int arm = 0; arm < 3; ++arm) {
       const int i = arm, j = (arm + 1) % 3;
       const double d0 = x[i][0] - x[j][0], d1 = x[i][1] - x[j][1], d2 = x[i][2] - x[j][2];
-      const double inv = 1.0 / sqrt(d0 * d0 + d1 * d1 + d2 * d2);
+      const double inv = inv_sqrt(d0 * d0 + d1 * d1 + d2 * d2);
       const double n0v = d0 * inv, n1v = d1 * inv, n2v = d2 * inv;  // emitter j -> receiver i
       const double un = u0 * n0v + u1 * n1v + u2 * n2v;
       const double vn = v0 * n0v + v1 * n1v + v2 * n2v;
       kn[arm] = k0 * n0v + k1 * n1v + k2 * n2v;
+      // eq. 16 divides by 2 (1 - k.n) on one link of the arm and by 2 (1 + k.n) on the other: one reciprocal,
+      // 1 / (2 (1 - k.n)(1 + k.n)), computed here, serves both (an fp64 division is ~25 instructions and a branch;
+      // six of them at the end of the links' dependency chains, plus 1/sqrt as two operations, were 8 % of the
+      // kernel)
+      rden[arm] = 1.0 / (2.0 * ((1.0 - kn[arm]) * (1.0 + kn[arm])));
       xip[arm] = un * un - vn * vn;   // eq. 12
       xic[arm] = 2.0 * un * vn;
     }
@@ -236,7 +249,7 @@ LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W
       const D2 re = raw[ae], rr = raw[ar[rx]];
       const double dhp = (re.x - rr.x) - Se[0] + Sr[rx][0];
       const double dhc = (re.y - rr.y) - Se[1] + Sr[rx][1];
-      store(slot, (xip[arm] * dhp + xic[arm] * dhc) / (2.0 * (1.0 - kappa)));  // eq. 16
+      store(slot, (xip[arm] * dhp + xic[arm] * dhc) * ((1.0 + kappa) * rden[arm]));  // eq. 16: / (2 (1 - kappa))
     }
   }
 }
