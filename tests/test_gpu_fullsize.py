@@ -67,3 +67,44 @@ def test_full_size_config5_chirp(lr):  # noqa: F811
     check_workload(lr, w, wins=wins)
     eq = inputs.orbit_table("eq", w.t0, w.t0 + w.n * w.dt, const_ltt=inputs.ARM / inputs.C_LIGHT)
     check_workload(lr, w, tdi_tab=eq, tdi_gen=1, proj=False, wins=_wins(w, lr, 4, seed=56, gen=1))
+
+
+def test_full_size_parameters_in(lr):  # noqa: F811
+    """configs[1] from the parameters (lr_response_gb, lr_loglike_gb) in the shape bench.py times: the one-call
+    result equals lr_response on the generated h bit for bit, sampled windows of it match the oracle chain
+    (exact-phase waveform, long-double projection and TDI), and log L of the template that made the data is
+    exactly 0 while a neighbour's is negative."""
+    import torch
+    from oracle import oracle as orc
+    from oracle import waveform as owf
+    from parity_util import CH_NAMES, ORC_CH, assert_parity
+    w = inputs.config(2)
+    s = w.sources[0]
+    a = owf.amplitudes_config(s.A, s.iota)
+    gb = np.array([[a[0], a[1], s.f0, s.fdot, 0.0, s.phi0], [a[0], a[1], s.f0 * (1 + 1e-7), s.fdot, 0.0, s.phi0]])
+    be, la, ps = [s.beta] * 2, [s.lam] * 2, [s.psi] * 2
+    tab = w.table()
+    R = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="AET")
+    out = R.response_gb(gb, be, la, ps, w.n)
+    hp, hc = R.gb_waveform(gb, w.n)
+    ref = R.response(hp, hc, be, la, ps)
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref)
+    O = orc.Oracle(tab, w.dt, w.t0, w.order)
+    mp, mf, mb = R.margins()
+    for lo, hi in _wins(w, lr, 3, width=256, seed=55):
+        pad = mf + 8                                   # the oracle window needs y (hence h) over the TDI reach
+        a0, a1 = max(lo - pad - mp, 0), min(hi + mb + mp + 8, w.n)
+        op, oc = owf.gb_waveform(gb[0], w.t0, w.dt, a1 - a0, first=a0)   # exact phase: T amplifies 1e-12 of h
+        hp_full = np.zeros(w.n)
+        hc_full = np.zeros(w.n)
+        hp_full[a0:a1], hc_full[a0:a1] = op, oc
+        y = O.project(hp_full, hc_full, s.beta, s.lam, s.psi, lo=max(a0 + mp, mp), hi=min(a1 - mp, w.n - mp))
+        oo = O.tdi(y, 2, nested=True, channels=ORC_CH["AET"], lo=lo, hi=hi)
+        assert_parity(out[0, :, lo:hi].cpu().numpy(), oo[:, lo:hi], f"response_gb year [{lo},{hi})", CH_NAMES["AET"])
+    nf = w.n // 2 + 1
+    inv = torch.ones((3, nf), dtype=torch.float64, device="cuda")
+    inv[:, 0] = 0
+    data_f = torch.fft.rfft(out[0], dim=-1).contiguous()
+    ll = R.loglike_gb(gb, be, la, ps, w.n, data_f, inv, -2.0 * w.dt / w.n).cpu().numpy()
+    assert abs(ll[0]) <= 1e-18 * abs(ll[1]) and ll[1] < 0      # cuFFT on both sides: the same bits up to its plan
