@@ -25,6 +25,9 @@ import time
 import numpy as np
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernels from the one `ncu --set full`
+# capture summarised in profiles/r1_v3_ncu_full.md (section v4); reported as roofline.traffic
+NCU_TRAFFIC = {("year", "lr_project"): 50716160 + 98775552, ("year", "lr_tdi"): 339870208 + 120571648}
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
@@ -464,13 +467,7 @@ def run_gpu(args, rank, world, local_rank):
     ach_proj = ops_p * batch * n / (ms_proj * 1e-3)
     dom = "lr_tdi" if ms_tdi >= ms_proj else "lr_project"
     ach_dom = ach_tdi if dom == "lr_tdi" else ach_proj
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        try:
-            traffic = json.load(open(tpath)).get(args.workload, {}).get(dom + "_bytes_per_launch")
-        except Exception:
-            traffic = None
+    traffic = NCU_TRAFFIC.get((args.workload, dom)) if (args.order is None or args.order == 25) else None
     line = {
         "metric": "response samples/s (6-link proj + TDI-2, fp64)" if args.workload != "batch"
                   else "response samples/s (6-link proj + TDI-2 AET, fp64), batched",
