@@ -234,6 +234,12 @@ int lr_eval_orbit(lr_handle* h, int channel, const double* t, int64_t m, double*
  * Synchronous.  Errors: LR_EINVAL, LR_ECUDA. */
 int lr_measure_fp64_peak(double seconds, double* inst_per_s);
 
+/* DFMA issue rate of this device for streams whose instructions share 2, 1 or 0 source registers with their
+ * neighbours (mode 0, 1, 2), and for mode 1 with one shared-memory load per 7 DFMA (mode 3): the measurements
+ * behind the issue rules of DESIGN.md §6 (16 warps per SM, 7 accumulators per thread, a few milliseconds).
+ * *inst_per_s = DFMA thread-instructions per second.  Synchronous.  Errors: LR_EINVAL, LR_ECUDA. */
+int lr_probe_fp64_operands(int mode, double* inst_per_s);
+
 /* Number of kernels liblr has launched in this process (all handles); bench.py's gpu_launches. */
 int64_t lr_launch_count(void);
 

@@ -28,7 +28,7 @@ LR_MAX_ORDER = 65
 
 # every symbol include/lr.h declares
 SYMBOLS = ("lr_create", "lr_destroy", "lr_set_option", "lr_get_margins", "lr_project", "lr_tdi",
-           "lr_inner_product", "lr_gb_waveform", "lr_response_gb", "lr_loglike_gb", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count",
+           "lr_inner_product", "lr_gb_waveform", "lr_response_gb", "lr_loglike_gb", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_probe_fp64_operands", "lr_launch_count",
            "lr_last_cuda_error", "lr_strerror")
 
 
@@ -84,6 +84,7 @@ def lib():
     L.lr_loglike_gb.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, vp, vp, dbl, ci, vp, vp]
     L.lr_eval_orbit.argtypes = [vp, ci, vp, i64, vp, vp]
     L.lr_measure_fp64_peak.argtypes = [dbl, ctypes.POINTER(dbl)]
+    L.lr_probe_fp64_operands.argtypes = [ci, ctypes.POINTER(dbl)]
     L.lr_launch_count.argtypes = []
     L.lr_launch_count.restype = i64
     L.lr_last_cuda_error.argtypes = [vp]
@@ -321,6 +322,13 @@ def lr_eval_orbit(h, channel, t, out, stream=None):
 def lr_measure_fp64_peak(seconds=0.5):
     v = ctypes.c_double()
     _check(lib().lr_measure_fp64_peak(float(seconds), ctypes.byref(v)), "lr_measure_fp64_peak")
+    return v.value
+
+
+def lr_probe_fp64_operands(mode):
+    """DFMA thread-instructions/s with 2 / 1 / 0 shared source registers (mode 0 / 1 / 2), mode 3 = mode 1 + LDS."""
+    v = ctypes.c_double()
+    _check(lib().lr_probe_fp64_operands(int(mode), ctypes.byref(v)), "lr_probe_fp64_operands")
     return v.value
 
 

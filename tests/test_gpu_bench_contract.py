@@ -46,3 +46,16 @@ def test_bench_reference_arm():
     d = _run("--impl", "reference", "--steps", "1", "--warmup", "0", "--workload", "tiny", "--cpu-seconds", "0.5")
     assert d["impl"] == "reference" and d["value"] > 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
+
+
+@pytest.mark.gpu
+def test_fp64_operand_probe_orders_the_modes():
+    """lr_probe_fp64_operands: a DFMA stream that shares source registers between neighbours issues faster than
+    one that does not (the measurement behind DESIGN.md §6's issue rules), and none exceeds the nominal peak."""
+    import torch
+    import paper_2204_06633_b200 as lr
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    r = [lr.lr_probe_fp64_operands(m) for m in range(4)]
+    nominal = sms * 64 * 2.2e9
+    assert all(0 < x < nominal for x in r), r
+    assert r[2] < 0.9 * r[1] and r[1] <= 1.05 * r[0] and r[3] <= 1.02 * r[1], r
