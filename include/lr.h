@@ -243,7 +243,8 @@ int lr_probe_fp64_operands(int mode, double* inst_per_s);
 /* Number of kernels liblr has launched in this process (all handles); bench.py's gpu_launches. */
 int64_t lr_launch_count(void);
 
-/* CUDA error code (cudaError_t as int) of the last failed CUDA call on this handle, 0 if none. */
+/* CUDA error code (cudaError_t as int) of the last failed CUDA call on this handle, 0 if none.  A failed cuFFT
+ * call in lr_loglike_gb is reported as 10000 + cufftResult (planning) or 20000 + cufftResult (execution). */
 int lr_last_cuda_error(const lr_handle* h);
 
 /* Static description of an LR_* code. */
