@@ -499,6 +499,7 @@ def run_gpu(args, rank, world, local_rank):
                      "peak_nominal": torch.cuda.get_device_properties(dev).multi_processor_count * 64 *
                                      (clk.max_mhz or 1965) * 1e-3,   # SMs x 64 FP64 lanes x max SM clock [Gop/s]
                      "pipe_busy_pct_ncu": {"lr_project": 71.2, "lr_tdi": 64.5, "source": "profiles/r1_v3_ncu_full.md (v4)"},
+                     "shared_memory_pipe_busy_pct_ncu": {"lr_project": 85.7, "lr_tdi": 37.7},
                      "path_frac": (ops_t + ops_p) * batch * n / ((ms_proj + ms_tdi) * 1e-3) / peak},
         "clocks": clk.summary(), "wall_s_timed_region": wall,
     }
