@@ -184,6 +184,14 @@ int lr_response_host(lr_handle* h_proj, lr_handle* h_tdi, const double* h_plus, 
 int lr_gb_waveform(lr_handle* h, const double* gb, int64_t batch, int64_t n, double* h_plus, double* h_cross,
                    void* cuda_stream);
 
+/* The six numbers of lr_gb_waveform from the physical parameters (HOST arithmetic, no device needed):
+ *   LR_GB_PAPER : eqs. 8-9 — a_plus = -A (1 + cos^2 iota), a_cross = -2 A cos iota, fddot = 11/3 fdot^2 / f0
+ *   LR_GB_CONFIG: BASELINE.json's configs — a_plus = +A (1 + cos^2 iota), a_cross = -2 A cos iota, fddot = 0
+ * gb: HOST [LR_GB_NPAR] (written).  Errors: LR_EINVAL (null pointer, unknown form, f0 <= 0, non-finite input). */
+#define LR_GB_PAPER 0
+#define LR_GB_CONFIG 1
+int lr_gb_parameters(double A, double f0, double fdot, double phi0, double iota, int form, double* gb);
+
 /* Parameters -> TDI channels in one call: lr_gb_waveform, lr_project (on h_proj) and lr_tdi (on h_tdi, may be
  * the same handle) chunk by chunk along time; neither h nor y exists as a whole array, both live in scratch
  * of h_proj.  out: DEVICE [batch][3|6][n], bit-identical to

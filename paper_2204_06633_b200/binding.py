@@ -21,6 +21,7 @@ LR_OPT_TDI_PLAN_CACHE = 6
 LR_OPT_CHUNK_SAMPLES = 7
 LR_IP_CROSS, LR_IP_DIFF, LR_IP_BLOCKS = 0, 1, 1024
 LR_GB_NPAR = 6
+LR_GB_PAPER, LR_GB_CONFIG = 0, 1
 LR_TDI_AUTO, LR_TDI_PER_SAMPLE, LR_TDI_FIR3, LR_TDI_FIR4 = -1, 0, 3, 4
 LR_CHAIN_NESTED, LR_CHAIN_SUM = 0, 1
 LR_XYZ, LR_AET, LR_XYZ_AET = 0, 1, 2
@@ -28,7 +29,7 @@ LR_MAX_ORDER = 65
 
 # every symbol include/lr.h declares
 SYMBOLS = ("lr_create", "lr_destroy", "lr_set_option", "lr_get_margins", "lr_project", "lr_tdi",
-           "lr_inner_product", "lr_gb_waveform", "lr_response_gb", "lr_loglike_gb", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_probe_fp64_operands", "lr_launch_count",
+           "lr_inner_product", "lr_gb_parameters", "lr_gb_waveform", "lr_response_gb", "lr_loglike_gb", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_probe_fp64_operands", "lr_launch_count",
            "lr_last_cuda_error", "lr_strerror")
 
 
@@ -80,6 +81,7 @@ def lib():
     L.lr_response_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
     L.lr_inner_product.argtypes = [vp, vp, vp, dbl, ci, i64, i64, ci, i64, vp, vp, vp]
     L.lr_gb_waveform.argtypes = [vp, vp, i64, i64, vp, vp, vp]
+    L.lr_gb_parameters.argtypes = [dbl, dbl, dbl, dbl, dbl, ci, vp]
     L.lr_response_gb.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
     L.lr_loglike_gb.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, vp, vp, dbl, ci, vp, vp]
     L.lr_eval_orbit.argtypes = [vp, ci, vp, i64, vp, vp]
@@ -237,6 +239,14 @@ def _gb(gb):
         g = g[None]
     if g.ndim != 2 or g.shape[1] != LR_GB_NPAR:
         raise ValueError("gb must be [batch, 6] = a_plus, a_cross, f0, fdot, fddot, phi0")
+    return g
+
+
+def lr_gb_parameters(A, f0, fdot, phi0, iota, form=LR_GB_PAPER):
+    """lr_gb_parameters: the six numbers of one template (numpy [6])."""
+    g = np.empty(LR_GB_NPAR)
+    _check(lib().lr_gb_parameters(float(A), float(f0), float(fdot), float(phi0), float(iota), int(form),
+                                  g.ctypes.data), "lr_gb_parameters")
     return g
 
 

@@ -815,6 +815,21 @@ int lr_loglike_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const double
   return LR_OK;
 }
 
+int lr_gb_parameters(double A, double f0, double fdot, double phi0, double iota, int form, double* gb) {
+  if (!gb || (form != LR_GB_PAPER && form != LR_GB_CONFIG) || !(f0 > 0)) return LR_EINVAL;
+  if (!std::isfinite(A) || !std::isfinite(f0) || !std::isfinite(fdot) || !std::isfinite(phi0) || !std::isfinite(iota))
+    return LR_EINVAL;
+  const double ci = cos(iota);
+  const double plus = A * (1.0 + ci * ci), cross = -2.0 * A * ci;   // eq. 9's inclination factors
+  gb[0] = form == LR_GB_PAPER ? -plus : plus;                        // eq. 9 carries a minus sign on h+ too
+  gb[1] = cross;
+  gb[2] = f0;
+  gb[3] = fdot;
+  gb[4] = form == LR_GB_PAPER ? 11.0 / 3.0 * fdot * fdot / f0 : 0.0;  // eq. 8
+  gb[5] = phi0;
+  return LR_OK;
+}
+
 int lr_eval_orbit(lr_handle* h, int channel, const double* t, int64_t m, double* out, void* stream) {
   if (!h || !t || !out || channel < 0 || channel > 14 || m < 1) return LR_EINVAL;
   lr::Params P = make_params(h, 1);

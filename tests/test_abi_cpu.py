@@ -57,6 +57,22 @@ def test_host_only_entry_points(lib):
     lib.lr_destroy(None)
 
 
+def test_gb_parameters_host(lib):
+    """lr_gb_parameters (host arithmetic of eqs. 8-9) against the oracle's statement of the same equations."""
+    from oracle import waveform as owf
+    from paper_2204_06633_b200 import binding
+    A, f0, fdot, phi0, iota = 1.3e-22, 4.2e-3, 2.5e-16, 0.9, 1.1
+    g = binding.lr_gb_parameters(A, f0, fdot, phi0, iota, binding.LR_GB_PAPER)
+    ap, ac = owf.amplitudes_paper(A, iota)
+    assert np.allclose(g, [ap, ac, f0, fdot, owf.fddot_eq8(f0, fdot), phi0], rtol=1e-15, atol=0)
+    g = binding.lr_gb_parameters(A, f0, fdot, phi0, iota, binding.LR_GB_CONFIG)
+    ap, ac = owf.amplitudes_config(A, iota)
+    assert np.allclose(g, [ap, ac, f0, fdot, 0.0, phi0], rtol=1e-15, atol=0)
+    for bad in ((A, 0.0, fdot, phi0, iota, 0), (A, f0, fdot, phi0, iota, 7), (float("nan"), f0, fdot, phi0, iota, 0)):
+        with pytest.raises(binding.LrError):
+            binding.lr_gb_parameters(*bad)
+
+
 def test_create_rejects_bad_arguments_without_gpu(lib):
     from paper_2204_06633_b200 import binding, inputs
     tab = inputs.orbit_table("eq", 0.0, 86400.0)
