@@ -61,6 +61,7 @@ typedef struct {
 #define LR_OPT_TDI_GEN 4  /* 1 | 2: changes the generation given to lr_create */
 #define LR_OPT_TDI_PATH 5 /* LR_TDI_AUTO (default) | LR_TDI_PER_SAMPLE | LR_TDI_FIR3 | LR_TDI_FIR4 */
 #define LR_OPT_CHUNK_SAMPLES 7 /* time-chunk length of lr_response / lr_response_host (rounded up to 1792); 0 = automatic */
+#define LR_OPT_FFT_LENGTH 8 /* transform length of lr_loglike_gb (>= n, zero padded); 0 (default) = n */
 #define LR_OPT_TDI_PLAN_CACHE 6 /* 1 (default): keep the FIR plan between lr_tdi calls; 0: rebuild every call */
 
 /* How lr_tdi evaluates the Lagrange weights (same result to rounding).
@@ -225,6 +226,9 @@ int lr_inner_product(const double* fa, const double* fb, const double* inv_psd, 
  * with H_b[ch][k] = sum_n out_b[ch][n] exp(-2 pi i k n / N), k = 0 .. N/2 — the UNNORMALISED forward DFT of the
  * channels (margins are zeros); data_f must be in the same convention.  log L of eq. 3 with a~ = dt * DFT is
  * scale = -2 dt / N, mode LR_IP_DIFF, inv_psd[ch][0] = 0.
+ * With LR_OPT_FFT_LENGTH = M > n set on h_proj the channels are zero padded to M samples before the transform
+ * (N = M in the formulas above: data_f and inv_psd then have M/2+1 bins on the grid k / (M dt)); a length without
+ * prime factors above 7 (lr_fft_good_length) makes the transform 2-3x faster than e.g. 3,153,600 = 2^6 3^3 5^2 73.
  * h_tdi must produce three channels (LR_XYZ or LR_AET).  gb, beta, lambda, psi: HOST [batch]...; data_f: DEVICE
  * complex [3][N/2+1] (interleaved re, im); inv_psd: DEVICE [3][N/2+1]; out: DEVICE [batch].  Scratch (the
  * channels and spectra of 8 templates, the FFT plan) is owned by h_proj and kept until lr_destroy.
@@ -232,6 +236,9 @@ int lr_inner_product(const double* fa, const double* fb, const double* inv_psd, 
 int lr_loglike_gb(lr_handle* h_proj, lr_handle* h_tdi, const double* gb, const double* beta, const double* lambda,
                   const double* psi, int64_t batch, int64_t n, const double* data_f, const double* inv_psd,
                   double scale, int mode, double* out, void* cuda_stream);
+
+/* Smallest length >= n whose prime factors are 2, 3, 5, 7 (HOST arithmetic); -1 for n outside [1, 2^31). */
+int64_t lr_fft_good_length(int64_t n);
 
 /* Evaluate the device spline of one orbit channel (0..8 = x[i][a] as i*3+a, 9..14 = L link slots) at
  * `m` times t (DEVICE [m]) into out (DEVICE [m]); used by the tests to pin the orbit ingestion. */

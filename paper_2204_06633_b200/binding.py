@@ -19,6 +19,7 @@ LR_OK, LR_EINVAL, LR_ERANGE, LR_ECUDA, LR_ENOMEM = 0, -1, -2, -3, -4
 LR_OPT_T0, LR_OPT_CHAIN, LR_OPT_CHANNELS, LR_OPT_TDI_GEN, LR_OPT_TDI_PATH = 1, 2, 3, 4, 5
 LR_OPT_TDI_PLAN_CACHE = 6
 LR_OPT_CHUNK_SAMPLES = 7
+LR_OPT_FFT_LENGTH = 8
 LR_IP_CROSS, LR_IP_DIFF, LR_IP_BLOCKS = 0, 1, 1024
 LR_GB_NPAR = 6
 LR_GB_PAPER, LR_GB_CONFIG = 0, 1
@@ -29,7 +30,7 @@ LR_MAX_ORDER = 65
 
 # every symbol include/lr.h declares
 SYMBOLS = ("lr_create", "lr_destroy", "lr_set_option", "lr_get_margins", "lr_project", "lr_tdi",
-           "lr_inner_product", "lr_gb_parameters", "lr_gb_waveform", "lr_response_gb", "lr_loglike_gb", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_probe_fp64_operands", "lr_launch_count",
+           "lr_inner_product", "lr_gb_parameters", "lr_fft_good_length", "lr_gb_waveform", "lr_response_gb", "lr_loglike_gb", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_probe_fp64_operands", "lr_launch_count",
            "lr_last_cuda_error", "lr_strerror")
 
 
@@ -82,6 +83,8 @@ def lib():
     L.lr_inner_product.argtypes = [vp, vp, vp, dbl, ci, i64, i64, ci, i64, vp, vp, vp]
     L.lr_gb_waveform.argtypes = [vp, vp, i64, i64, vp, vp, vp]
     L.lr_gb_parameters.argtypes = [dbl, dbl, dbl, dbl, dbl, ci, vp]
+    L.lr_fft_good_length.argtypes = [i64]
+    L.lr_fft_good_length.restype = i64
     L.lr_response_gb.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
     L.lr_loglike_gb.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, vp, vp, dbl, ci, vp, vp]
     L.lr_eval_orbit.argtypes = [vp, ci, vp, i64, vp, vp]
@@ -242,6 +245,14 @@ def _gb(gb):
     return g
 
 
+def lr_fft_good_length(n):
+    """Smallest 7-smooth length >= n (a fast transform length for LR_OPT_FFT_LENGTH)."""
+    m = lib().lr_fft_good_length(int(n))
+    if m < 0:
+        raise ValueError("n out of range")
+    return int(m)
+
+
 def lr_gb_parameters(A, f0, fdot, phi0, iota, form=LR_GB_PAPER):
     """lr_gb_parameters: the six numbers of one template (numpy [6])."""
     g = np.empty(LR_GB_NPAR)
@@ -274,14 +285,14 @@ def lr_response_gb(h_proj, h_tdi, gb, beta, lam, psi, n, out, stream=None):
 
 
 def lr_loglike_gb(h_proj, h_tdi, gb, beta, lam, psi, n, data_f, inv_psd, scale, mode=LR_IP_DIFF, out=None,
-                  stream=None):
+                  stream=None, n_fft=None):
     """lr_loglike_gb: waveform parameters host [B, 6] + sky angles -> out CUDA float64 [B]; data_f CUDA
     complex128 [3, n//2+1] (unnormalised DFT), inv_psd CUDA float64 [3, n//2+1]."""
     import torch
     g = _gb(gb)
     beta, lam, psi = _host(beta), _host(lam), _host(psi)
     B = g.shape[0]
-    nf = n // 2 + 1
+    nf = (n_fft or n) // 2 + 1   # n_fft: the LR_OPT_FFT_LENGTH the caller set on h_proj (sizes are checked against it)
     if beta.size != B or lam.size != B or psi.size != B:
         raise ValueError("beta, lambda, psi must have one entry per template")
     if not (isinstance(data_f, torch.Tensor) and data_f.is_cuda and data_f.dtype == torch.complex128

@@ -64,6 +64,7 @@ struct lr_handle {
   int plan_cache = 1;    // LR_OPT_TDI_PLAN_CACHE
   int sm_count = 0;
   int64_t chunk_samples = 0;   // LR_OPT_CHUNK_SAMPLES: 0 = automatic
+  int64_t fft_length = 0;      // LR_OPT_FFT_LENGTH: 0 = n (no zero padding)
   Plan plan;
   double bk[lr::kPMax + 1];
   // device state
@@ -286,6 +287,9 @@ int lr_set_option(lr_handle* h, int key, double value) {
     case LR_OPT_CHUNK_SAMPLES:
       if (value < 0 || value > 2147483647.0 || value != floor(value)) return LR_EINVAL;
       h->chunk_samples = (int64_t)value; return LR_OK;
+    case LR_OPT_FFT_LENGTH:
+      if (value < 0 || value > 2147483647.0 || value != floor(value)) return LR_EINVAL;
+      h->fft_length = (int64_t)value; return LR_OK;
     case LR_OPT_TDI_PLAN_CACHE:
       if (value != 0 && value != 1) return LR_EINVAL;
       h->plan_cache = (int)value; h->plan.valid = false; return LR_OK;
@@ -778,29 +782,34 @@ int lr_loglike_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const double
   if (ht_->channels == LR_XYZ_AET || n < 2 || n > 0x7fffffff) return LR_EINVAL;   // three channels per template
   if (mode != LR_IP_CROSS && mode != LR_IP_DIFF) return LR_EINVAL;
   cudaStream_t st = (cudaStream_t)stream;
-  const int64_t nf = n / 2 + 1;
+  const int64_t nt = h->fft_length > 0 ? h->fft_length : n;   // transform length (zero padded beyond n)
+  if (nt < n) return LR_EINVAL;
+  const int64_t nf = nt / 2 + 1;
   const int64_t bc = batch < 8 ? batch : 8;
-  const int64_t np = n + (n & 1);   // row stride of the channels: cuFFT wants 16-byte aligned transforms
+  const int64_t np = nt + (nt & 1);   // row stride of the channels: cuFFT wants 16-byte aligned transforms
   int rc = ensure(h, &h->o_buf, &h->o_cap, (size_t)(bc * 3 * np));
   if (rc == LR_OK) rc = ensure(h, &h->f_buf, &h->f_cap, (size_t)(bc * 3 * nf * 2));
   if (rc == LR_OK) rc = ensure(h, &h->ip_work, &h->ip_cap, (size_t)(bc * LR_IP_BLOCKS));
   if (rc != LR_OK) return rc;
-  if (h->fft_n != n) {   // one plan of three real-to-complex transforms (the channels of one template), kept
+  if (h->fft_n != nt) {   // one plan of three real-to-complex transforms (the channels of one template), kept
     if (h->fft_n) { cufftDestroy(h->fft); h->fft_n = 0; }
-    int len = (int)n;
+    int len = (int)nt;
     int in_len = (int)np, out_len = (int)nf;
     const cufftResult fr = cufftPlanMany(&h->fft, 1, &len, &in_len, 1, (int)np, &out_len, 1, (int)nf, CUFFT_D2Z, 3);
     if (fr != CUFFT_SUCCESS) {
       h->last_cuda = 10000 + (int)fr;   // cuFFT result codes are reported as 10000 + cufftResult
       return LR_ECUDA;
     }
-    h->fft_n = n;
+    h->fft_n = nt;
   }
   if (cufftSetStream(h->fft, st) != CUFFT_SUCCESS) { h->last_cuda = 10000; return LR_ECUDA; }
   for (int64_t b0 = 0; b0 < batch; b0 += bc) {
     const int64_t nb = batch - b0 < bc ? batch - b0 : bc;
     rc = response_gb(hp_, ht_, gb + b0 * 6, beta + b0, lam + b0, psi + b0, nb, n, h->o_buf, np, stream);
     if (rc != LR_OK) return rc;
+    if (nt > n)   // the zero padding of every row (the response writes [0, n) only)
+      LR_CUDA(h, cudaMemset2DAsync(h->o_buf + n, (size_t)np * sizeof(double), 0, (size_t)(nt - n) * sizeof(double),
+                                   (size_t)nb * 3, st));
     for (int64_t b = 0; b < nb; ++b) {
       const cufftResult fr = cufftExecD2Z(h->fft, h->o_buf + b * 3 * np,
                                           reinterpret_cast<cufftDoubleComplex*>(h->f_buf) + b * 3 * nf);
@@ -828,6 +837,16 @@ int lr_gb_parameters(double A, double f0, double fdot, double phi0, double iota,
   gb[4] = form == LR_GB_PAPER ? 11.0 / 3.0 * fdot * fdot / f0 : 0.0;  // eq. 8
   gb[5] = phi0;
   return LR_OK;
+}
+
+int64_t lr_fft_good_length(int64_t n) {
+  if (n < 1 || n > 2147483647) return -1;
+  for (int64_t m = n;; ++m) {   // smallest m >= n with no prime factor above 7
+    int64_t r = m;
+    for (int p : {2, 3, 5, 7})
+      while (r % p == 0) r /= p;
+    if (r == 1) return m;
+  }
 }
 
 int lr_eval_orbit(lr_handle* h, int channel, const double* t, int64_t m, double* out, void* stream) {

@@ -157,11 +157,16 @@ class Response:
             out = torch.empty((nb, t.n_out, n), dtype=torch.float64, device="cuda")
         return B.lr_response_gb(self._h, t._h, gb, beta, lam, psi, n, out, stream)
 
+    def set_fft_length(self, m):
+        """Transform length of loglike_gb (>= n, zero padded; 0 = n).  See lr_fft_good_length."""
+        B.lr_set_option(self._h, B.LR_OPT_FFT_LENGTH, int(m))
+        self._fft_length = int(m)
+
     def loglike_gb(self, gb, beta, lam, psi, n, data_f, inv_psd, scale, mode=B.LR_IP_DIFF, out=None, tdi=None,
                    stream=None):
         """Parameters -> one scalar per template (CUDA [B]): waveform, response, FFT, noise-weighted inner product."""
         return B.lr_loglike_gb(self._h, (tdi or self)._h, gb, beta, lam, psi, n, data_f, inv_psd, scale, mode, out,
-                               stream)
+                               stream, n_fft=getattr(self, "_fft_length", 0) or None)
 
     def close(self):
         if self._h is not None:

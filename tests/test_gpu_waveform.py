@@ -153,6 +153,26 @@ def test_loglike_gb_against_oracle_pipeline(lr):
     assert np.abs(cross - want_c).max() <= 1e-10 * np.abs(want_c).max()
     again = R.loglike_gb(gb, beta, lam, psi, n, data_f, inv_d, -2.0 * dt / n).cpu().numpy()
     assert np.array_equal(got, again)
+    # zero-padded transform (LR_OPT_FFT_LENGTH): 12001 -> 12005 = 5 * 7^4; the oracle pads the same series
+    m = lr.lr_fft_good_length(n)
+    assert m == 12005
+    pad = np.concatenate([aet, np.zeros((nb, 3, m - n))], axis=-1)
+    fpad = lk.to_frequency(pad, dt)
+    psd_m = inputs.psd_standin(np.fft.rfftfreq(m, dt))
+    inv_m = np.zeros_like(psd_m)
+    inv_m[:, 1:] = 1.0 / psd_m[:, 1:]
+    want_m = np.array([lk.log_likelihood(fpad[1], fpad[b], psd_m, dt, m) for b in range(nb)], dtype=np.float64)
+    R.set_fft_length(m)
+    data_m = torch.from_numpy(np.ascontiguousarray(np.fft.rfft(pad[1], axis=-1))).cuda()
+    got_m = R.loglike_gb(gb, beta, lam, psi, n, data_m, to_dev(inv_m), -2.0 * dt / m).cpu().numpy()
+    assert np.abs(got_m[others] - want_m[others]).max() <= 1e-10 * np.abs(want_m).max()
+    assert np.abs(want_m[others] / want[others] - 1).max() < 0.05      # the same integral on a finer grid
+    R.set_fft_length(0)
+    assert np.array_equal(R.loglike_gb(gb, beta, lam, psi, n, data_f, inv_d, -2.0 * dt / n).cpu().numpy(), got)
+    with pytest.raises(lr.LrError):
+        R.set_fft_length(n - 1)
+        R.loglike_gb(gb, beta, lam, psi, n, data_f, inv_d, -2.0 * dt / n)
+    R.set_fft_length(0)
     R6 = lr.Response(tab, dt, w.order, 2, t0=w.t0, channels="XYZ_AET")
     with pytest.raises(lr.LrError):
         R6.loglike_gb(gb, beta, lam, psi, n, data_f, inv_d, 1.0)
