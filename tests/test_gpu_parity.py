@@ -607,3 +607,37 @@ def test_edge_cases_and_errors(lr):
     R3 = lr.Response(tab, w.dt, w.order, 1, t0=w.t0)
     y = R3.project(to_dev(hp2)[None], to_dev(hc)[None], [s.beta], [s.lam], [s.psi]).cpu().numpy()[0]
     assert np.isnan(y).any() and np.isfinite(y[:, mp:4000]).all()
+
+
+# ------------------------------------------------------------------------------------- seeded random sweep
+@pytest.mark.parametrize("seed", range(40))
+def test_random_configurations(lr, seed):
+    """Seeded draws over the whole option space at sizes that span several tiles and a ragged tail: order 1-41,
+    dt 2-20 s, generation, chain form, channel set, orbit family (equal-arm constant, Keplerian, perturbed),
+    batch 1-3, TDI path, start time; lr_project + lr_tdi against the oracle (check_workload), then lr_response in
+    odd chunks against the two-call result bit for bit."""
+    import torch
+    rng = np.random.default_rng(1000 + seed)
+    order = int(rng.choice([1, 3, 5, 7, 9, 11, 13, 15, 21, 25, 31, 41]))
+    dt = float(rng.choice([2.0, 5.0, 10.0, 15.0, 20.0]))
+    gen = int(rng.choice([1, 2]))
+    chain = str(rng.choice(["nested", "sum"]))
+    channels = str(rng.choice(["XYZ", "AET", "XYZ_AET"]))
+    kind = str(rng.choice(["eq", "kepler", "perturbed"]))
+    batch = int(rng.integers(1, 4))
+    n = int(rng.integers(2500, 5200))
+    t0 = float(rng.uniform(1e6, 9e7))
+    tdi_path = str(rng.choice(["auto", "per_sample", "fir3", "fir4"]))
+    if kind == "eq":
+        channels = "XYZ"   # T of exactly equal arms is a null (3e-5 of A): test_tdi_null_channel_absolute covers it
+    srcs = [inputs.draw_gb(np.random.default_rng(50 * seed + b)) for b in range(batch)]
+    w = inputs.Workload(f"random{seed}", n, dt, t0, order, gen, kind, 7 + seed,
+                        inputs.ARM / inputs.C_LIGHT if kind == "eq" else None, srcs, channels=channels)
+    errs, yh, oh = check_workload(lr, w, chain=chain, idx=tuple(range(batch)), tdi_path=tdi_path)
+    R = lr.Response(w.table(), dt, order, gen, t0=t0, chain=chain, channels=channels, tdi_path=tdi_path)
+    lr.lr_set_option(R.handle, lr.LR_OPT_CHUNK_SAMPLES, 1792 * int(rng.integers(1, 3)))
+    hp, hc = _stack(w, range(batch))
+    beta, lam, psi = ([getattr(s, k) for s in srcs] for k in ("beta", "lam", "psi"))
+    out = R.response(to_dev(hp), to_dev(hc), beta, lam, psi)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), oh), (order, dt, gen, chain, channels, kind, batch, n, tdi_path)
