@@ -373,7 +373,7 @@ def run_gpu(args, rank, world, local_rank):
     try:
         if args.workload not in ("year", "batch", "tiny") or not all(s.f0 > 0 for s in w.sources[:8]):
             raise RuntimeError("no Galactic-binary parameters in this workload")
-        nb = min(chunk, 8)
+        nb = min(chunk, 32)   # above 8 templates the call pipelines chunks of 8 (transforms beside the next response)
         Ra = lr.Response(w.table(), w.dt, w.order, w.tdi_gen, t0=w.t0, chain="nested", channels="AET")
         gb = np.array([[s.A * (1.0 + np.cos(s.iota) ** 2), -2.0 * s.A * np.cos(s.iota), s.f0, s.fdot, 0.0, s.phi0]
                        for s in w.sources[:nb]])

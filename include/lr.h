@@ -231,7 +231,10 @@ int lr_inner_product(const double* fa, const double* fb, const double* inv_psd, 
  * prime factors above 7 (lr_fft_good_length) makes the transform 2-3x faster than e.g. 3,153,600 = 2^6 3^3 5^2 73.
  * h_tdi must produce three channels (LR_XYZ or LR_AET).  gb, beta, lambda, psi: HOST [batch]...; data_f: DEVICE
  * complex [3][N/2+1] (interleaved re, im); inv_psd: DEVICE [3][N/2+1]; out: DEVICE [batch].  Scratch (the
- * channels and spectra of 8 templates, the FFT plan) is owned by h_proj and kept until lr_destroy.
+ * channels and spectra of 8 templates — twice that for batch > 8 — and the FFT plan) is owned by h_proj and kept
+ * until lr_destroy.  Templates are processed in chunks of 8; for batch > 8 the transforms and the inner product of
+ * one chunk run on a stream of the handle beside the response of the next chunk and are joined to `cuda_stream`
+ * before the call returns, so the caller sees ordinary stream ordering.
  * Errors: LR_EINVAL (as lr_response_gb, or six output channels), LR_ECUDA (CUDA or cuFFT failure). */
 int lr_loglike_gb(lr_handle* h_proj, lr_handle* h_tdi, const double* gb, const double* beta, const double* lambda,
                   const double* psi, int64_t batch, int64_t n, const double* data_f, const double* inv_psd,

@@ -83,6 +83,8 @@ struct lr_handle {
   double* f_buf = nullptr; size_t f_cap = 0;
   double* ip_work = nullptr; size_t ip_cap = 0;
   cufftHandle fft = 0; int64_t fft_n = 0;
+  cudaStream_t s_fft = nullptr;                     // transforms + inner product of chunk c beside the response of c+1
+  cudaEvent_t ev_resp[2] = {nullptr, nullptr}, ev_fft[2] = {nullptr, nullptr};
   int last_cuda = 0;
 
   int64_t m_proj() const {
@@ -260,7 +262,10 @@ void lr_destroy(lr_handle* h) {
     if (h->ev_comp[i]) cudaEventDestroy(h->ev_comp[i]);
     if (h->ev_out[i]) cudaEventDestroy(h->ev_out[i]);
     if (h->ev_fix[i]) cudaEventDestroy(h->ev_fix[i]);
+    if (h->ev_resp[i]) cudaEventDestroy(h->ev_resp[i]);
+    if (h->ev_fft[i]) cudaEventDestroy(h->ev_fft[i]);
   }
+  if (h->s_fft) cudaStreamDestroy(h->s_fft);
   if (h->s_in) cudaStreamDestroy(h->s_in);
   if (h->s_out) cudaStreamDestroy(h->s_out);
   if (h->coef) cudaFree(h->coef);
@@ -787,10 +792,26 @@ int lr_loglike_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const double
   const int64_t nf = nt / 2 + 1;
   const int64_t bc = batch < 8 ? batch : 8;
   const int64_t np = nt + (nt & 1);   // row stride of the channels: cuFFT wants 16-byte aligned transforms
-  int rc = ensure(h, &h->o_buf, &h->o_cap, (size_t)(bc * 3 * np));
-  if (rc == LR_OK) rc = ensure(h, &h->f_buf, &h->f_cap, (size_t)(bc * 3 * nf * 2));
+  // More than one template chunk: two slots of channels and spectra, and the transforms + inner product of chunk c
+  // run on a stream of the handle beside the response of chunk c+1 (the response is bound by FP64 issue, the
+  // transforms mostly by HBM: they share the SMs well).  One chunk: everything on the caller's stream.
+  const int nslot = batch > bc ? 2 : 1;
+  const size_t o_slot = (size_t)(bc * 3 * np), f_slot = (size_t)(bc * 3 * nf * 2);
+  int rc = ensure(h, &h->o_buf, &h->o_cap, nslot * o_slot);
+  if (rc == LR_OK) rc = ensure(h, &h->f_buf, &h->f_cap, nslot * f_slot);
   if (rc == LR_OK) rc = ensure(h, &h->ip_work, &h->ip_cap, (size_t)(bc * LR_IP_BLOCKS));
   if (rc != LR_OK) return rc;
+  if (nslot == 2 && !h->s_fft) {
+    // highest priority: the transforms' CTAs take SM slots as the response's CTAs retire instead of queueing
+    // behind the whole grid of the response kernel launched before them
+    int prio_lo = 0, prio_hi = 0;
+    LR_CUDA(h, cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+    LR_CUDA(h, cudaStreamCreateWithPriority(&h->s_fft, cudaStreamNonBlocking, prio_hi));
+    for (int i = 0; i < 2; ++i) {
+      LR_CUDA(h, cudaEventCreateWithFlags(&h->ev_resp[i], cudaEventDisableTiming));
+      LR_CUDA(h, cudaEventCreateWithFlags(&h->ev_fft[i], cudaEventDisableTiming));
+    }
+  }
   if (h->fft_n != nt) {   // one plan of three real-to-complex transforms (the channels of one template), kept
     if (h->fft_n) { cufftDestroy(h->fft); h->fft_n = 0; }
     int len = (int)nt;
@@ -802,25 +823,45 @@ int lr_loglike_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const double
     }
     h->fft_n = nt;
   }
-  if (cufftSetStream(h->fft, st) != CUFFT_SUCCESS) { h->last_cuda = 10000; return LR_ECUDA; }
-  for (int64_t b0 = 0; b0 < batch; b0 += bc) {
+  cudaStream_t sf = nslot == 2 ? h->s_fft : st;
+  if (cufftSetStream(h->fft, sf) != CUFFT_SUCCESS) { h->last_cuda = 10000; return LR_ECUDA; }
+  bool busy[2] = {false, false};   // ev_fft[slot] recorded and not yet waited for by the caller's stream
+  int64_t c = 0;
+  for (int64_t b0 = 0; b0 < batch; b0 += bc, ++c) {
     const int64_t nb = batch - b0 < bc ? batch - b0 : bc;
-    rc = response_gb(hp_, ht_, gb + b0 * 6, beta + b0, lam + b0, psi + b0, nb, n, h->o_buf, np, stream);
+    const int slot = nslot == 2 ? (int)(c & 1) : 0;
+    double* ob = h->o_buf + slot * o_slot;
+    double* fb = h->f_buf + slot * f_slot;
+    if (busy[slot]) {   // the transforms of chunk c-2 have read this slot
+      LR_CUDA(h, cudaStreamWaitEvent(st, h->ev_fft[slot], 0));
+      busy[slot] = false;
+    }
+    rc = response_gb(hp_, ht_, gb + b0 * 6, beta + b0, lam + b0, psi + b0, nb, n, ob, np, stream);
     if (rc != LR_OK) return rc;
     if (nt > n)   // the zero padding of every row (the response writes [0, n) only)
-      LR_CUDA(h, cudaMemset2DAsync(h->o_buf + n, (size_t)np * sizeof(double), 0, (size_t)(nt - n) * sizeof(double),
+      LR_CUDA(h, cudaMemset2DAsync(ob + n, (size_t)np * sizeof(double), 0, (size_t)(nt - n) * sizeof(double),
                                    (size_t)nb * 3, st));
+    if (nslot == 2) {
+      LR_CUDA(h, cudaEventRecord(h->ev_resp[slot], st));
+      LR_CUDA(h, cudaStreamWaitEvent(sf, h->ev_resp[slot], 0));
+    }
     for (int64_t b = 0; b < nb; ++b) {
-      const cufftResult fr = cufftExecD2Z(h->fft, h->o_buf + b * 3 * np,
-                                          reinterpret_cast<cufftDoubleComplex*>(h->f_buf) + b * 3 * nf);
+      const cufftResult fr = cufftExecD2Z(h->fft, ob + b * 3 * np, reinterpret_cast<cufftDoubleComplex*>(fb) + b * 3 * nf);
       if (fr != CUFFT_SUCCESS) {
         h->last_cuda = 20000 + (int)fr;   // 20000 + cufftResult: the transform itself
         return LR_ECUDA;
       }
     }
-    rc = lr_inner_product(h->f_buf, data_f, inv_psd, scale, mode, nb, 1, 3, nf, h->ip_work, out + b0, stream);
+    // (ip_work is shared by the slots: the inner products run one after the other on sf)
+    rc = lr_inner_product(fb, data_f, inv_psd, scale, mode, nb, 1, 3, nf, h->ip_work, out + b0, (void*)sf);
     if (rc != LR_OK) return rc;
+    if (nslot == 2) {
+      LR_CUDA(h, cudaEventRecord(h->ev_fft[slot], sf));
+      busy[slot] = true;
+    }
   }
+  for (int i = 0; i < 2; ++i)   // join: `out` is complete on the caller's stream
+    if (busy[i]) LR_CUDA(h, cudaStreamWaitEvent(st, h->ev_fft[i], 0));
   return LR_OK;
 }
 

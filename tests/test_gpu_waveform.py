@@ -176,3 +176,39 @@ def test_loglike_gb_against_oracle_pipeline(lr):
     R6 = lr.Response(tab, dt, w.order, 2, t0=w.t0, channels="XYZ_AET")
     with pytest.raises(lr.LrError):
         R6.loglike_gb(gb, beta, lam, psi, n, data_f, inv_d, 1.0)
+
+
+def test_loglike_gb_pipelined_chunks_bitwise(lr):
+    """batch > 8: lr_loglike_gb runs the transforms and the inner product of one chunk of 8 templates on a stream
+    of the handle beside the response of the next chunk (two slots, reused from the third chunk on).  The 27
+    scalars must equal, bit for bit, those of four separate calls of <= 8 templates (the one-slot path), on the
+    default and on a caller's stream, twice in a row."""
+    import torch
+    w = inputs.config(2, n=9001, f0=4e-3, t0=2.5e7)
+    tab = w.table()
+    rng = np.random.default_rng(27)
+    nb = 27
+    gb = np.empty((nb, 6))
+    for b in range(nb):
+        a = owf.amplitudes_paper(1e-22 * (1 + 0.05 * b), 0.2 + 0.1 * b)
+        gb[b] = (a[0], a[1], 4e-3 * (1 + 1e-4 * rng.standard_normal()), 1e-16, 0.0, rng.uniform(0, 2 * math.pi))
+    beta, lam, psi = rng.uniform(-1, 1, nb), rng.uniform(0, 6, nb), rng.uniform(0, 3, nb)
+    n, dt = w.n, w.dt
+    R = lr.Response(tab, dt, w.order, 2, t0=w.t0, channels="AET")
+    data_f = torch.fft.rfft(R.response_gb(gb[3:4], beta[3:4], lam[3:4], psi[3:4], n)[0], dim=-1).contiguous()
+    inv = np.zeros((3, n // 2 + 1))
+    inv[:, 1:] = 1.0 / inputs.psd_standin(np.fft.rfftfreq(n, dt))[:, 1:]
+    inv_d = to_dev(inv)
+    parts = [R.loglike_gb(gb[lo:lo + 8], beta[lo:lo + 8], lam[lo:lo + 8], psi[lo:lo + 8], n, data_f, inv_d,
+                          -2.0 * dt / n).cpu().numpy() for lo in range(0, nb, 8)]
+    want = np.concatenate(parts)
+    assert want[3] == 0.0 and np.all(want[np.arange(nb) != 3] < 0)
+    for _ in range(2):
+        got = R.loglike_gb(gb, beta, lam, psi, n, data_f, inv_d, -2.0 * dt / n).cpu().numpy()
+        assert np.array_equal(got, want)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        got_s = R.loglike_gb(gb, beta, lam, psi, n, data_f, inv_d, -2.0 * dt / n, stream=s)
+        got_s = got_s.cpu().numpy()      # ordered behind the call on s: the side stream is joined before it returns
+    assert np.array_equal(got_s, want)
