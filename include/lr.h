@@ -120,7 +120,8 @@ int lr_get_margins(const lr_handle* h, int64_t* m_proj, int64_t* m_tdi_front, in
  *   y_ij = [xi+ (h+(t_e) - h+(t_r)) + xix (hx(t_e) - hx(t_r))] / (2 (1 - k.n_ij))               (eq. 16)
  *   t_e = t - L_ij(t) - k.x_j(t)/c,  t_r = t - k.x_i(t)/c, h evaluated by Lagrange interpolation.
  * h_plus, h_cross : DEVICE [batch][n];  beta (ecliptic latitude), lambda (ecliptic longitude), psi : HOST [batch]
- * y_out : DEVICE [batch][6][n].  Requires n > 2 m_proj and n < 2^31 - 2^20.
+ * (the three angles are copied to the device as they are; k, u, v are computed there by a one-thread-per-template
+ * kernel in front of the projection kernel).  y_out : DEVICE [batch][6][n].  Requires n > 2 m_proj and n < 2^31 - 2^20.
  * Errors: LR_EINVAL, LR_ERANGE, LR_ECUDA. */
 int lr_project(lr_handle* h, const double* h_plus, const double* h_cross, const double* beta,
                const double* lambda, const double* psi, int64_t batch, int64_t n, double* y_out,

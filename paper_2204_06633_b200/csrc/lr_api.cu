@@ -142,8 +142,9 @@ bool in_table(const lr_handle* h, int64_t n_first, int64_t n_last, double back_r
   return lo >= 0 && hi <= span;
 }
 
-// Stages the per-template constants of one launch: the source basis [batch][9] and, when `gb` is given, the
-// waveform parameters [batch][6] right behind it (device pointer returned in *gb_dev).
+// Stages the per-template constants of one launch.  Host -> device: the sky angles [batch][3] = (beta, lambda, psi)
+// and, when `gb` is given, the waveform parameters [batch][6]; source_basis_kernel then writes the source basis
+// [batch][9] (step P1 of the path) on the caller's stream.  Device layout of a slot: basis | gb | angles.
 int stage_basis(lr_handle* h, const double* beta, const double* lam, const double* psi, int64_t batch,
                 cudaStream_t st, Stage** used, const double* gb = nullptr, const double** gb_dev = nullptr) {
   Stage& S = h->stage[h->next_slot];
@@ -154,15 +155,35 @@ int stage_basis(lr_handle* h, const double* beta, const double* lam, const doubl
     if (S.host) cudaFreeHost(S.host);
     if (S.dev) cudaFree(S.dev);
     S.host = nullptr; S.dev = nullptr; S.cap = 0;
-    LR_CUDA(h, cudaMallocHost(&S.host, (size_t)batch * 15 * sizeof(double)));
-    LR_CUDA(h, cudaMalloc(&S.dev, (size_t)batch * 15 * sizeof(double)));
+    LR_CUDA(h, cudaMallocHost(&S.host, (size_t)batch * 9 * sizeof(double)));
+    LR_CUDA(h, cudaMalloc(&S.dev, (size_t)batch * 18 * sizeof(double)));
     S.cap = batch;
   }
-  for (int64_t b = 0; b < batch; ++b) lr::source_basis(beta[b], lam[b], psi[b], S.host + 9 * b);
-  if (gb) memcpy(S.host + 9 * batch, gb, (size_t)batch * 6 * sizeof(double));
-  LR_CUDA(h, cudaMemcpyAsync(S.dev, S.host, (size_t)batch * (gb ? 15 : 9) * sizeof(double), cudaMemcpyHostToDevice,
-                             st));
-  if (gb_dev) *gb_dev = S.dev + 9 * batch;
+  double* dev_gb = S.dev + 9 * batch;
+  double* dev_ang = S.dev + 15 * batch;
+  if (batch <= lr::kSmallStage) {   // the constants travel in the kernel's parameter buffer: no copy in front of it
+    lr::SmallStage ss;
+    memset(&ss, 0, sizeof(ss));
+    ss.n = (int)batch; ss.has_gb = gb ? 1 : 0;
+    if (gb) memcpy(ss.v, gb, (size_t)batch * 6 * sizeof(double));
+    for (int64_t b = 0; b < batch; ++b) {
+      ss.v[6 * batch + 3 * b] = beta[b]; ss.v[6 * batch + 3 * b + 1] = lam[b]; ss.v[6 * batch + 3 * b + 2] = psi[b];
+    }
+    LR_CUDA(h, (cudaError_t)lr::launch_source_basis_small(ss, S.dev, (void*)st));
+    if (gb_dev) *gb_dev = dev_gb;
+    *used = &S;
+    return LR_OK;
+  }
+  // host side of the slot: gb [batch][6] | angles [batch][3] (the order they have on the device)
+  double* ang = S.host + 6 * batch;
+  for (int64_t b = 0; b < batch; ++b) { ang[3 * b] = beta[b]; ang[3 * b + 1] = lam[b]; ang[3 * b + 2] = psi[b]; }
+  if (gb) memcpy(S.host, gb, (size_t)batch * 6 * sizeof(double));
+  if (gb)
+    LR_CUDA(h, cudaMemcpyAsync(dev_gb, S.host, (size_t)batch * 9 * sizeof(double), cudaMemcpyHostToDevice, st));
+  else
+    LR_CUDA(h, cudaMemcpyAsync(dev_ang, ang, (size_t)batch * 3 * sizeof(double), cudaMemcpyHostToDevice, st));
+  LR_CUDA(h, (cudaError_t)lr::launch_source_basis(dev_ang, batch, S.dev, (void*)st));
+  if (gb_dev) *gb_dev = dev_gb;
   *used = &S;
   return LR_OK;
 }

@@ -323,8 +323,8 @@ LR_HD void tdi_sample(const Params& prm, const double* raw, const double* dif, i
 }
 
 // Source basis (eq. 10) with the polarisation angle applied to (u, v) (reading A4):
-// out[0..2] = k, out[3..5] = u, out[6..8] = v.  Host-side helper of lr_project.
-inline void source_basis(double beta, double lam, double psi, double* out) {
+// out[0..2] = k, out[3..5] = u, out[6..8] = v.  Runs in source_basis_kernel (one thread per template).
+LR_HD void source_basis(double beta, double lam, double psi, double* out) {
   const double cb = cos(beta), sb = sin(beta), cl = cos(lam), sl = sin(lam);
   const double k[3] = {-cb * cl, -cb * sl, -sb};
   const double u0[3] = {sl, -cl, 0.0};                 // -e_phi

@@ -19,6 +19,43 @@ __global__ void eval_orbit_kernel(const Params prm, int ch, double t_start, cons
   if (i < m) out[i] = spline_eval(prm, ch, t[i] - t_start);
 }
 
+__global__ void source_basis_kernel(const double* __restrict__ angles, int64_t batch, double* __restrict__ basis) {
+  const int64_t b = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (b >= batch) return;
+  double o[9];
+  source_basis(angles[3 * b], angles[3 * b + 1], angles[3 * b + 2], o);
+#pragma unroll
+  for (int a = 0; a < 9; ++a) basis[9 * b + a] = o[a];
+}
+
+int launch_source_basis(const double* angles, int64_t batch, double* basis, void* stream) {
+  const int threads = 128;
+  source_basis_kernel<<<(unsigned)((batch + threads - 1) / threads), threads, 0, (cudaStream_t)stream>>>(angles, batch,
+                                                                                                       basis);
+  g_launches.fetch_add(1);
+  return (int)cudaGetLastError();
+}
+
+__global__ void source_basis_small_kernel(const SmallStage s, double* __restrict__ slot) {
+  const int b = threadIdx.x, n = s.n;
+  if (b >= n) return;
+  const double* ang = s.v + 6 * n + 3 * b;
+  double o[9];
+  source_basis(ang[0], ang[1], ang[2], o);
+#pragma unroll
+  for (int a = 0; a < 9; ++a) slot[9 * b + a] = o[a];
+  if (s.has_gb) {
+#pragma unroll
+    for (int a = 0; a < 6; ++a) slot[9 * n + 6 * b + a] = s.v[6 * b + a];
+  }
+}
+
+int launch_source_basis_small(const SmallStage& s, double* slot, void* stream) {
+  source_basis_small_kernel<<<1, 32, 0, (cudaStream_t)stream>>>(s, slot);
+  g_launches.fetch_add(1);
+  return (int)cudaGetLastError();
+}
+
 int launch_project(const Params& prm, int order, const double* hp, const double* hc, const double* basis,
                    double* y, int64_t batch, void* stream) {
   switch (order) {

@@ -171,6 +171,17 @@ struct FirPlanArgs {
 __global__ void eval_orbit_kernel(const Params prm, int ch, double t_start, const double* __restrict__ t,
                                   int64_t m, double* __restrict__ out);
 
+// step P1 of the path (eq. 10): angles [batch][3] = (beta, lambda, psi) -> basis [batch][9] =
+// (k, u, v), one thread per template; launched by every call that takes sky angles, in front of project_kernel
+__global__ void source_basis_kernel(const double* __restrict__ angles, int64_t batch, double* __restrict__ basis);
+int launch_source_basis(const double* angles, int64_t batch, double* basis, void* stream);
+// the same for up to kSmallStage templates whose constants travel in the kernel's parameter buffer (no host ->
+// device copy in front of the launch): v = gb [n][6] | angles [n][3]; slot = basis [n][9] | gb [n][6] | angles [n][3]
+constexpr int kSmallStage = 16;
+struct SmallStage { double v[kSmallStage * 9]; int n; int has_gb; };
+__global__ void source_basis_small_kernel(const SmallStage s, double* __restrict__ slot);
+int launch_source_basis_small(const SmallStage& s, double* slot, void* stream);
+
 // Launchers, one explicit instantiation per compile-time pair count PT (lr_inst.cu is compiled once per
 // PT; PT = 0 reads P at run time).  They return cudaError_t as int.
 template <int PT>

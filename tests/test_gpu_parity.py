@@ -204,6 +204,37 @@ def test_config3_batch_reduced(lr):
     check_workload(lr, w, idx=tuple(range(7)))
 
 
+def test_source_basis_staging_paths_bitwise(lr):
+    """Step P1 runs on the device: up to 16 templates per call carry their angles in the parameter buffer of
+    source_basis_small_kernel, larger batches go through a host -> device copy and source_basis_kernel.  Both run
+    the same device function, so a 19-template launch must equal 19 one-template launches bit for bit
+    (lr_project, and lr_gb_waveform whose six numbers are staged the same way); template 0 against the oracle."""
+    import torch
+    w = inputs.config(3, batch=19, n=3001)
+    R = lr.Response(w.table(), w.dt, 9, 2, t0=w.t0)
+    hp, hc = _stack(w, range(19))
+    hp_d, hc_d = to_dev(hp), to_dev(hc)
+    be = [s.beta for s in w.sources]
+    la = [s.lam for s in w.sources]
+    ps = [s.psi for s in w.sources]
+    y = R.project(hp_d, hc_d, be, la, ps).cpu().numpy()
+    for b in range(19):
+        yb = R.project(hp_d[b:b + 1], hc_d[b:b + 1], be[b:b + 1], la[b:b + 1], ps[b:b + 1]).cpu().numpy()
+        assert np.array_equal(yb[0], y[b]), b
+    O = orc.Oracle(w.table(), w.dt, w.t0, 9)
+    mp = O.margins(2)[0]
+    yo = O.project(hp[0], hc[0], be[0], la[0], ps[0])
+    assert_parity(y[0, :, mp:w.n - mp], yo[:, mp:w.n - mp], "lr_project", LINK_NAMES)
+    gb = np.array([[s.A * (1.0 + np.cos(s.iota) ** 2), -2.0 * s.A * np.cos(s.iota), s.f0, s.fdot, 0.0, s.phi0]
+                   for s in w.sources])
+    gp, gc = R.gb_waveform(gb, w.n)
+    for b in (0, 7, 18):
+        p1, c1 = R.gb_waveform(gb[b:b + 1], w.n)
+        assert torch.equal(p1[0], gp[b]) and torch.equal(c1[0], gc[b])
+    out = R.response_gb(gb, be, la, ps, w.n)
+    assert torch.equal(out, R.response(gp, gc, be, la, ps))
+
+
 # ------------------------------------------------------------------------------------------- config 4
 @pytest.mark.parametrize("tdi_path", ["auto", "per_sample", "fir4"])
 def test_config4_numerical_orbits_reduced(lr, tdi_path):
