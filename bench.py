@@ -26,8 +26,8 @@ import numpy as np
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernels from the one `ncu --set full`
-# capture summarised in profiles/r1_v3_ncu_full.md (section v4); reported as roofline.traffic
-NCU_TRAFFIC = {("year", "lr_project"): 50716160 + 98775552, ("year", "lr_tdi"): 339870208 + 120571648}
+# capture summarised in profiles/r1_v5_launches.md (full capture of the final build); reported as roofline.traffic
+NCU_TRAFFIC = {("year", "lr_project"): 50714112 + 97300480, ("year", "lr_tdi"): 339880704 + 118690560}
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
@@ -521,8 +521,8 @@ def run_gpu(args, rank, world, local_rank):
                      "peak_source": f"lr_measure_fp64_peak({args.peak_seconds} s DFMA kernel) on this device, this run",
                      "peak_nominal": torch.cuda.get_device_properties(dev).multi_processor_count * 64 *
                                      (clk.max_mhz or 1965) * 1e-3,   # SMs x 64 FP64 lanes x max SM clock [Gop/s]
-                     "pipe_busy_pct_ncu": {"lr_project": 71.2, "lr_tdi": 64.5, "source": "profiles/r1_v3_ncu_full.md (v4)"},
-                     "shared_memory_pipe_busy_pct_ncu": {"lr_project": 85.7, "lr_tdi": 37.7},
+                     "pipe_busy_pct_ncu": {"lr_project": 71.1, "lr_tdi": 64.4, "source": "profiles/r1_v5_launches.md"},
+                     "shared_memory_pipe_busy_pct_ncu": {"lr_project": 85.6, "lr_tdi": 37.6},
                      "path_frac": (ops_t + ops_p) * batch * n / ((ms_proj + ms_tdi) * 1e-3) / peak},
         "clocks": clk.summary(), "wall_s_timed_region": wall,
     }
