@@ -435,7 +435,12 @@ int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, do
     }
     pa.fixup_grid = 2 * h->sm_count;
     if (!pl.side) {
-      LR_CUDA(h, cudaStreamCreateWithFlags(&pl.side, cudaStreamNonBlocking));
+      // highest priority: the side stream starts a few microseconds behind the apply kernel (it waits for the fork
+      // event), by which time the apply kernel's CTAs hold every SM; at equal priority the fix-up CTAs were only
+      // dispatched once the apply grid had drained and became a 40 us tail of every lr_tdi call
+      int prio_lo = 0, prio_hi = 0;
+      LR_CUDA(h, cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+      LR_CUDA(h, cudaStreamCreateWithPriority(&pl.side, cudaStreamNonBlocking, prio_hi));
       LR_CUDA(h, cudaEventCreateWithFlags(&pl.fork, cudaEventDisableTiming));
       LR_CUDA(h, cudaEventCreateWithFlags(&pl.join, cudaEventDisableTiming));
     }
