@@ -510,7 +510,7 @@ def run_gpu(args, rank, world, local_rank):
                                "frac_fp64": ach_tdi / peak, "alg_GBps": bytes_tdi(nout) * batch * n / (ms_tdi * 1e6)}},
         "likelihood": lk,
         "params_to_loglike": pl,
-        "lr_response": {"ms_per_step": ms_resp, "note": "one call, h -> out, y only in a scratch of two <= 256 MB slots"},
+        "lr_response": {"ms_per_step": ms_resp, "note": "one call, h -> out, y only in a scratch of two <= 1 GB slots"},
         "tdi_plan": {"cached_between_calls": True, "ms_tdi_with_plan_rebuilt_every_call": ms_tdi_cold,
                      "value_with_plan_rebuilt_every_call": units / (max_over_ranks(ms_proj + ms_tdi_cold) * 1e-3)
                      if world == 1 else None},

@@ -135,7 +135,7 @@ int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out,
 
 /* Both stages with DEVICE buffers and no [batch][6][n] array: h_plus, h_cross DEVICE [batch][n] -> out DEVICE
  * [batch][3|6][n], bit-identical to lr_project followed by lr_tdi.  The path runs in chunks of time (and of
- * 8 templates) through a y scratch of two slots of <= 256 MB owned by h_proj, so the device footprint
+ * 8 templates) through a y scratch of two slots of <= 1 GB owned by h_proj, so the device footprint
  * is h + out + that scratch (the paper's real call is waveform -> projection -> TDI with nothing
  * in between leaving the GPU).  Enqueues on `cuda_stream` and returns without synchronising.
  * beta, lambda, psi: HOST [batch].  Errors: as lr_project / lr_tdi. */

@@ -515,7 +515,7 @@ constexpr int64_t lcm_(int64_t a, int64_t b) { return a / gcd_(a, b) * b; }
 constexpr int64_t kChunkUnit = lcm_(lcm_(lr::kProjThreads, lr::kTdiThreads), lr::kFirTile);
 // y of one chunk: longer chunks mean fewer kernel tails (one year: 0.88 ms at 40 MB, 0.83 ms in one chunk); L2
 // residency of y buys nothing, the kernels are bound by FP64 issue.  Two slots of this size per handle at most.
-constexpr int64_t kYSlotBytes = (int64_t)256 << 20;
+constexpr int64_t kYSlotBytes = (int64_t)1024 << 20;
 
 int ensure(lr_handle* h, double** buf, size_t* cap, size_t need) {
   if (*cap >= need) return LR_OK;
