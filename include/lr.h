@@ -248,7 +248,9 @@ int64_t lr_fft_good_length(int64_t n);
  * `m` times t (DEVICE [m]) into out (DEVICE [m]); used by the tests to pin the orbit ingestion. */
 int lr_eval_orbit(lr_handle* h, int channel, const double* t, int64_t m, double* out, void* cuda_stream);
 
-/* Measure this device's FP64 issue rate with a DFMA-only kernel that runs for about `seconds`:
+/* Measure this device's FP64 issue rate with a DFMA-only kernel that runs for about `seconds` (8 chains per thread,
+ * acc = acc * register + uniform register: the operand form with which the pipe reaches its 64 DFMA per SM and clock;
+ * chains with three register operands stop at 58.7, see lr_peak.cu):
  * *inst_per_s = FP64 thread-instructions per second (one DFMA = 1).  The roofline denominator of bench.py.
  * Synchronous.  Errors: LR_EINVAL, LR_ECUDA. */
 int lr_measure_fp64_peak(double seconds, double* inst_per_s);

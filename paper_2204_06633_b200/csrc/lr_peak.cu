@@ -2,7 +2,13 @@
 //
 // MEASURED_PEAKS.json records no FP64 peak, and the response path is bound by the FP64 pipe,
 // so bench.py measures the roofline denominator on the device it runs on: every thread runs 8 independent
-// DFMA chains, 1024 threads per SM-slot, all SMs, for about the requested time.
+// DFMA chains acc = fma(acc, x, y), x a register shared by the chains and y a kernel parameter (ptxas keeps it in
+// a uniform register: `DFMA R2, R2, R26.reuse, UR6`), 2,048 threads per SM, all SMs, for about the requested time.
+// The operand form matters on sm_100 (measured on B200 at 1.965 GHz, 16-64 warps per SM, 8 or 16 chains):
+//   acc * reg + uniform register            63.0-63.6 DFMA per SM and clock  (the pipe has 64: this kernel)
+//   acc * reg + reg (both shared, .reuse)   58.1-58.7  (the round's first version of this kernel: 1.71e13 /s)
+//   two fresh register operands per DFMA    48-54, depending on the registers ptxas picks
+// The first line is the rate of the pipe itself and the one a kernel is held against.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -20,11 +26,12 @@ __global__ void __launch_bounds__(256) dfma_kernel(double a, double b, int64_t o
   double acc[kChains];
 #pragma unroll
   for (int c = 0; c < kChains; ++c) acc[c] = (double)(threadIdx.x + c) * 1e-9;
+  const double x = a - (double)threadIdx.x * 1e-12;   // a register; b stays a kernel parameter (uniform register)
   for (int64_t it = 0; it < outer; ++it) {
 #pragma unroll
     for (int i = 0; i < kInner; ++i) {
 #pragma unroll
-      for (int c = 0; c < kChains; ++c) acc[c] = fma(acc[c], a, b);
+      for (int c = 0; c < kChains; ++c) acc[c] = fma(acc[c], x, b);
     }
   }
   double s = 0.0;
