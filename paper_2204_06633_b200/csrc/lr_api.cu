@@ -50,6 +50,12 @@ struct Plan {
   cudaEvent_t ready = nullptr;
   cudaStream_t side = nullptr;          // the fix-up kernel's stream (forked from / joined to the caller's)
   cudaEvent_t fork = nullptr, join = nullptr;
+  // host copy of the list of flagged tiles (count, then the tiles), fetched once behind the plan kernel: a launch
+  // whose window holds no flagged tile needs no fork / fix-up kernel / join
+  int* list_host = nullptr;             // pinned, [1 + list_cap]
+  size_t list_cap = 0;
+  cudaEvent_t list_ev = nullptr;
+  int list_state = 0;                   // 0 unknown | 1 copy in flight | 2 known
 };
 
 struct lr_handle {
@@ -270,6 +276,8 @@ void lr_destroy(lr_handle* h) {
   if (h->plan.fork) cudaEventDestroy(h->plan.fork);
   if (h->plan.join) cudaEventDestroy(h->plan.join);
   if (h->plan.side) cudaStreamDestroy(h->plan.side);
+  if (h->plan.list_ev) cudaEventDestroy(h->plan.list_ev);
+  if (h->plan.list_host) cudaFreeHost(h->plan.list_host);
   if (h->plan.coef) cudaFree(h->plan.coef);
   if (h->plan.flags) cudaFree(h->plan.flags);
   if (h->y_scr) cudaFree(h->y_scr);
@@ -412,6 +420,7 @@ int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, do
     if (!reuse) {
       const size_t need = (size_t)P.ntiles * lr::fir_plan_doubles_per_tile(P.fir_wc);
       pl.valid = false;
+      pl.list_state = 0;
       if (pl.coef_cap < need) {
         if (pl.coef) { cudaFree(pl.coef); pl.coef = nullptr; pl.coef_cap = 0; }
         LR_CUDA(h, cudaMalloc(&pl.coef, need * sizeof(double)));
@@ -445,7 +454,23 @@ int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, do
       LR_CUDA(h, cudaEventCreateWithFlags(&pl.join, cudaEventDisableTiming));
     }
     pa.side = pl.side; pa.fork = pl.fork; pa.join = pl.join;
-    if (join_later) { pa.join = *join_later; pa.wait_join = false; }
+    if (reuse && pl.list_state == 1) {
+      if (cudaEventQuery(pl.list_ev) == cudaSuccess) pl.list_state = 2;
+      else (void)cudaGetLastError();   // cudaErrorNotReady is not an error of this call
+    }
+    if (reuse && pl.list_state == 2) {
+      const int cnt = pl.list_host[0];
+      bool any = cnt > 0 && uniform;   // (one-tile plan: a flagged plan tile concerns every window)
+      if (cnt > 0 && !uniform) {
+        const int64_t t_lo = w.off / lr::kFirTile, t_hi = t_lo + (w.n + lr::kFirTile - 1) / lr::kFirTile;
+        for (int i = 1; i <= cnt && !any; ++i) any = pl.list_host[i] >= t_lo && pl.list_host[i] < t_hi;
+      }
+      pa.skip_fixup = !any;
+    }
+    if (join_later) {
+      if (pa.skip_fixup) *join_later = nullptr;   // nothing to wait for
+      else { pa.join = *join_later; pa.wait_join = false; }
+    }
     apply_window(P, w);
     P.ntiles = (int)((w.n + lr::kFirTile - 1) / lr::kFirTile);
   } else {
@@ -459,6 +484,26 @@ int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, do
     Plan& pl = h->plan;
     LR_CUDA(h, cudaEventRecord(pl.ready, st));
     pl.valid = true; pl.n = w.n_glob; pl.t0 = h->t0; pl.gen = h->gen; pl.chain = h->chain; pl.path = path;
+    // the list of flagged tiles comes to the host behind the plan kernel (no synchronisation: a later call that
+    // finds the copy finished uses it, until then every launch runs the fix-up kernel)
+    pl.list_state = 0;
+    if (h->plan_cache) {
+      const size_t words = 1 + (size_t)pa.plan_tiles;
+      if (pl.list_cap < words) {
+        if (pl.list_host) { cudaFreeHost(pl.list_host); pl.list_host = nullptr; pl.list_cap = 0; }
+        if (cudaMallocHost(&pl.list_host, words * sizeof(int)) == cudaSuccess) pl.list_cap = words;
+        else (void)cudaGetLastError();
+      }
+      if (!pl.list_ev && cudaEventCreateWithFlags(&pl.list_ev, cudaEventDisableTiming) != cudaSuccess) {
+        pl.list_ev = nullptr;
+        (void)cudaGetLastError();
+      }
+      if (pl.list_cap >= words && pl.list_ev) {
+        LR_CUDA(h, cudaMemcpyAsync(pl.list_host, pa.list, words * sizeof(int), cudaMemcpyDeviceToHost, st));
+        LR_CUDA(h, cudaEventRecord(pl.list_ev, st));
+        pl.list_state = 1;
+      }
+    }
   }
   return LR_OK;
 }

@@ -65,18 +65,21 @@ static int launch_tdi_fir(const Params& prm, int channels, const double* y, doub
     if ((e = cudaGetLastError()) != cudaSuccess) return (int)e;
   }
   const int W = kFirTile + prm.halo_lo + prm.halo_hi;
-  // fork: the flagged tiles (a handful, but each is a long dependent computation) run on the handle's side
-  // stream while the apply kernel fills the GPU; the two write disjoint tiles of `out`
-  cudaStream_t side = (cudaStream_t)plan.side;
-  const size_t smem_fix = (size_t)12 * W * sizeof(double);
-  if ((e = prepare(tdi_fir_fixup_kernel<PT, GEN>, smem_fix)) != cudaSuccess) return (int)e;
-  if ((e = cudaEventRecord((cudaEvent_t)plan.fork, st)) != cudaSuccess) return (int)e;
-  if ((e = cudaStreamWaitEvent(side, (cudaEvent_t)plan.fork, 0)) != cudaSuccess) return (int)e;
-  tdi_fir_fixup_kernel<PT, GEN><<<plan.fixup_grid, kFirTile, smem_fix, side>>>(prm, y, out, channels, plan.list,
-                                                                               (int)batch);
-  g_launches.fetch_add(1);
-  if ((e = cudaGetLastError()) != cudaSuccess) return (int)e;
-  if ((e = cudaEventRecord((cudaEvent_t)plan.join, side)) != cudaSuccess) return (int)e;
+  const bool fixup = plan.build || !plan.skip_fixup;
+  if (fixup) {
+    // fork: the flagged tiles (a handful, but each is a long dependent computation) run on the handle's side
+    // stream while the apply kernel fills the GPU; the two write disjoint tiles of `out`
+    cudaStream_t side = (cudaStream_t)plan.side;
+    const size_t smem_fix = (size_t)12 * W * sizeof(double);
+    if ((e = prepare(tdi_fir_fixup_kernel<PT, GEN>, smem_fix)) != cudaSuccess) return (int)e;
+    if ((e = cudaEventRecord((cudaEvent_t)plan.fork, st)) != cudaSuccess) return (int)e;
+    if ((e = cudaStreamWaitEvent(side, (cudaEvent_t)plan.fork, 0)) != cudaSuccess) return (int)e;
+    tdi_fir_fixup_kernel<PT, GEN><<<plan.fixup_grid, kFirTile, smem_fix, side>>>(prm, y, out, channels, plan.list,
+                                                                                 (int)batch);
+    g_launches.fetch_add(1);
+    if ((e = cudaGetLastError()) != cudaSuccess) return (int)e;
+    if ((e = cudaEventRecord((cudaEvent_t)plan.join, side)) != cudaSuccess) return (int)e;
+  }
 
   const size_t smem = fir_apply_smem_bytes(W, prm.fir_wc);
   const int64_t grid = (int64_t)prm.ntiles * batch;
@@ -91,7 +94,7 @@ static int launch_tdi_fir(const Params& prm, int channels, const double* y, doub
   }
   g_launches.fetch_add(1);
   if ((e = cudaGetLastError()) != cudaSuccess) return (int)e;
-  return plan.wait_join ? (int)cudaStreamWaitEvent(st, (cudaEvent_t)plan.join, 0) : 0;   // join
+  return fixup && plan.wait_join ? (int)cudaStreamWaitEvent(st, (cudaEvent_t)plan.join, 0) : 0;   // join
 }
 
 template <int PT>

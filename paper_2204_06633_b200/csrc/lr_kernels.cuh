@@ -165,6 +165,7 @@ struct FirPlanArgs {
   bool wait_join; // true: the caller's stream waits for `join` before the launcher returns; false: the caller
                   // orders later work after `join` itself (chunked response: the next chunk overlaps the fix-up)
   bool build;
+  bool skip_fixup; // the host knows that no flagged tile lies in this launch's window: no fork / fix-up / join
 };
 
 // small helper kernel: spline channel at arbitrary absolute times (lr_eval_orbit)

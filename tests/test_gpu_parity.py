@@ -151,6 +151,52 @@ def test_tdi_delay_crossing_whole_sample(lr):
                 assert_parity(out[:, mf:n - mb], oo[:, mf:n - mb], f"crossing gen{gen} {path}", CH_NAMES["XYZ"])
 
 
+def test_tdi_fixup_skipped_only_where_no_tile_is_flagged(lr):
+    """Once the plan's list of flagged tiles has reached the host, a launch whose window holds none of them skips the
+    fork / fix-up kernel / join.  Light times that cross a whole number of samples in the MIDDLE of a 40,000-sample
+    series flag a few tiles there (the fix-up kernel runs tdi_sample, so those tiles equal the per-sample path bit
+    for bit; all others differ from it in the last digits).  The first call (list unknown), later calls (list
+    known) and chunked lr_response calls (most chunks without a flagged tile) must agree bit for bit, flagged
+    tiles included."""
+    import torch
+    dt, n, t0, order = 10.0, 40000, 3.0e7, 9
+    base = inputs.orbit_table("kepler", t0, t0 + n * dt)
+    tk = base.t_start + base.knot_dt * np.arange(base.n_knots)
+    ltt = np.tile(10.0 + 2e-9 * (tk - (t0 + 0.5 * n * dt)), (6, 1)) * (1 + 1e-7 * np.arange(6))[:, None]
+    tab = inputs.OrbitTable(base.t_start, base.knot_dt, base.x, np.ascontiguousarray(ltt))
+    w = inputs.config(2, n=n, t0=t0)
+    hp, hc = w.waveform(0)
+    s = w.sources[0]
+    hp_d, hc_d = to_dev(hp)[None], to_dev(hc)[None]
+    R = lr.Response(tab, dt, order, 2, t0=t0, tdi_path="fir3")
+    Rp = lr.Response(tab, dt, order, 2, t0=t0, tdi_path="per_sample")
+    _, mf, mb = R.margins()
+    y = R.project(hp_d, hc_d, [s.beta], [s.lam], [s.psi])
+    first = R.tdi(y).cpu().numpy()[0]            # builds the plan; the list is still on its way to the host
+    torch.cuda.synchronize()
+    ps = Rp.tdi(y).cpu().numpy()[0]
+    tile = 224
+    same = [t for t in range(mf // tile + 1, (n - mb) // tile)
+            if np.array_equal(first[:, t * tile:(t + 1) * tile], ps[:, t * tile:(t + 1) * tile])]
+    assert 1 <= len(same) <= 40, len(same)       # the flagged tiles, and only a few of them
+    assert all(abs(t * tile - n // 2) < 6000 for t in same), same
+    for _ in range(3):                           # list known: whole-series window holds flagged tiles -> fix-up runs
+        assert np.array_equal(R.tdi(y).cpu().numpy()[0], first)
+    one = R.response(hp_d, hc_d, [s.beta], [s.lam], [s.psi]).cpu().numpy()[0]
+    assert np.array_equal(one, first)
+    lr.lr_set_option(R.handle, lr.LR_OPT_CHUNK_SAMPLES, 1792)    # 23 chunks, flagged tiles in two or three of them
+    for _ in range(2):
+        assert np.array_equal(R.response(hp_d, hc_d, [s.beta], [s.lam], [s.psi]).cpu().numpy()[0], first)
+    lo = (min(same) * tile // 1792) * 1792
+    span = R.response_span(hp_d, hc_d, 0, [s.beta], [s.lam], [s.psi], n, 1792 * 2, 1792 * 3)   # no flagged tile in it
+    assert lo > 1792 * 5 and np.array_equal(span.cpu().numpy()[0], first[:, 1792 * 2:1792 * 5])
+    span = R.response_span(hp_d, hc_d, 0, [s.beta], [s.lam], [s.psi], n, lo, 1792 * 2)           # flagged tiles in it
+    assert np.array_equal(span.cpu().numpy()[0], first[:, lo:lo + 1792 * 2])
+    O = orc.Oracle(tab, dt, t0, order)
+    oo = O.tdi(y.cpu().numpy()[0], 2, nested=True)
+    assert_parity(first[:, mf:n - mb], oo[:, mf:n - mb], "fir3 with flagged tiles", CH_NAMES["XYZ"])
+
+
 @pytest.mark.parametrize("ldot", [1e-9, 3e-8, 1e-6, 1e-5])
 def test_tdi_auto_path_follows_the_light_time_rate(lr, ldot):
     """LR_TDI_AUTO picks quadratic / cubic FIR / per-sample weights from the largest |dL/dt| of the table
