@@ -683,11 +683,18 @@ int lr_response_host(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const
   // three-stage pipeline over (template chunk, time chunk): H2D of the next chunk's h and D2H of the previous
   // chunk's out run on the handle's copy streams while the kernels of the current chunk run on `stream`
   const int64_t bc = batch < 8 ? batch : 8;
-  int64_t lc = round_up((n + 7) / 8, kChunkUnit);                       // about 8 chunks per template
-  const int64_t cap = ((int64_t)40 << 20) / (bc * 6 * (int64_t)sizeof(double)) / kChunkUnit * kChunkUnit;
-  if (lc > cap) lc = cap;
-  if (lc < 4 * kChunkUnit) lc = 4 * kChunkUnit;
-  if (h->chunk_samples > 0) lc = round_up(h->chunk_samples, kChunkUnit);
+  // Chunk lengths.  The call is bound by the device-to-host copy of `out` (3-6 rows per template against 2 rows of
+  // h going in), so the first copy should start as early as possible and every chunk costs a fixed ~10 us per
+  // stream: the chunks double from n/32 up to the largest the 80 MB slots hold (6 chunks for one year of one
+  // template instead of 8 equal ones: 3.26 -> 3.16 ms on a box whose D2H of the 151 MB alone takes 2.66 ms; n/64 first
+  // is no better).  LR_OPT_CHUNK_SAMPLES asks for equal chunks of that length.
+  const int64_t cap = ((int64_t)80 << 20) / (bc * 6 * (int64_t)sizeof(double)) / kChunkUnit * kChunkUnit;
+  int64_t lc = cap < 4 * kChunkUnit ? 4 * kChunkUnit : cap;               // the longest chunk
+  int64_t lc_first = round_up((n + 31) / 32, kChunkUnit);
+  if (lc_first < 4 * kChunkUnit) lc_first = 4 * kChunkUnit;
+  if (h->chunk_samples > 0) lc = lc_first = round_up(h->chunk_samples, kChunkUnit);
+  if (lc > round_up(n, kChunkUnit)) lc = round_up(n, kChunkUnit);
+  if (lc_first > lc) lc_first = lc;
   const int64_t ly = round_up(lc + ts.halo_lo + ts.halo_hi, 2);
   const int64_t lh = ly + 2 * mp;
   rc = ensure(h, &h->y_scr, &h->y_cap, (size_t)(2 * bc * 6 * ly));
@@ -716,9 +723,10 @@ int lr_response_host(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const
     Stage* S = nullptr;
     rc = stage_basis(h, beta + b0, lam + b0, psi + b0, nb, st, &S);
     if (rc != LR_OK) return rc;
-    for (int64_t a = 0; a < n; a += lc, ++c) {
+    int64_t len = lc_first;
+    for (int64_t a = 0, b = 0; a < n; a = b, ++c, len = 2 * len < lc ? 2 * len : lc) {
       const int slot = (int)(c & 1);
-      const int64_t b = a + lc < n ? a + lc : n;
+      b = a + len < n ? a + len : n;
       const int64_t ya = a - ts.halo_lo > 0 ? a - ts.halo_lo : 0, yb = b + ts.halo_hi < n ? b + ts.halo_hi : n;
       const int64_t ha = ya - mp > 0 ? ya - mp : 0, hb = yb + mp < n ? yb + mp : n;
       double* hp_d = h->h_buf + (size_t)slot * 2 * bc * lh;
