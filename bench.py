@@ -25,6 +25,7 @@ import time
 import numpy as np
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
+DEFAULT_CHUNK = 64   # templates per launch of the batched config (tests/test_gpu_fullsize.py checks this shape)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernels from the one `ncu --set full`
 # capture summarised in profiles/r1_v5_launches.md (full capture of the final build); reported as roofline.traffic
 NCU_TRAFFIC = {("year", "lr_project"): 50714112 + 97300480, ("year", "lr_tdi"): 339880704 + 118690560}
@@ -138,7 +139,7 @@ def make_workload(kind, rank, order=None):
 
 
 def _make_workload(kind, rank):
-    from paper_2204_06633_b200 import inputs
+    from harness import inputs
     if kind == "year":
         w = inputs.config(2)
         if rank:  # other ranks: same shape, their own seeded source
@@ -158,17 +159,8 @@ def _make_workload(kind, rank):
 
 
 def gb_waveform_device(srcs, n, dt, t0, device):
-    """The configs' GB waveform family evaluated on the device (input generation only; not timed)."""
-    import torch
-    t = t0 + dt * torch.arange(n, dtype=torch.float64, device=device)
-    hp = torch.empty((len(srcs), n), dtype=torch.float64, device=device)
-    hc = torch.empty_like(hp)
-    for b, s in enumerate(srcs):
-        ph = s.phi0 + 2.0 * np.pi * (s.f0 * t + 0.5 * s.fdot * t * t)
-        ci = np.cos(s.iota)
-        hp[b] = s.A * (1.0 + ci * ci) * torch.cos(ph)
-        hc[b] = -2.0 * s.A * ci * torch.sin(ph)
-    return hp, hc
+    from harness import inputs
+    return inputs.gb_waveform_device(srcs, n, dt, t0, device)
 
 
 # ------------------------------------------------------------------------------------------ CPU oracle
@@ -246,7 +238,7 @@ def run_gpu(args, rank, world, local_rank):
                     tdi_path=args.tdi_path)
     Rt, tdi_gen = R, w.tdi_gen
     if args.workload == "hybrid":
-        from paper_2204_06633_b200 import inputs as _inp
+        from harness import inputs as _inp
         eq = _inp.orbit_table("eq", w.t0, w.t0 + w.n * w.dt, const_ltt=_inp.ARM / _inp.C_LIGHT)
         tdi_gen = 1
         Rt = lr.Response(eq, w.dt, w.order, 1, t0=w.t0, chain="nested", channels=w.channels, tdi_path=args.tdi_path)
@@ -605,7 +597,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="year", choices=["year", "batch", "tiny", "4yr", "chirp", "hybrid"])
     ap.add_argument("--order", type=int, default=None, help="override the Lagrange order (order sweep)")
-    ap.add_argument("--chunk", type=int, default=64, help="templates per launch (batch workload)")
+    ap.add_argument("--chunk", type=int, default=DEFAULT_CHUNK, help="templates per launch (batch workload)")
     ap.add_argument("--e2e-templates", type=int, default=4)
     ap.add_argument("--peak-seconds", type=float, default=1.0)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)

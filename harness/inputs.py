@@ -228,6 +228,23 @@ def chirp_waveform(n, dt, t0, mchirp_msun, iota, phi_c, f_end=1e-2, f_lo=1e-4, a
     return amp * win * (1.0 + ci * ci) * np.cos(phase), -2.0 * amp * win * ci * np.sin(phase)
 
 
+def gb_waveform_device(srcs, n, dt, t0, device):
+    """The configs' GB waveform family for a list of sources, evaluated with torch ON THE DEVICE (input generation
+    only: config 3's chunks of 64 templates x 1.58e6 samples are made here instead of on the host).  Returns
+    (h_plus, h_cross), CUDA float64 [len(srcs), n].  Rounding differs from `gb_waveform` (torch vs numpy cos):
+    whoever needs the oracle's view of these inputs copies THESE arrays back."""
+    import torch
+    t = t0 + dt * torch.arange(n, dtype=torch.float64, device=device)
+    hp = torch.empty((len(srcs), n), dtype=torch.float64, device=device)
+    hc = torch.empty_like(hp)
+    for b, s in enumerate(srcs):
+        ph = s.phi0 + 2.0 * np.pi * (s.f0 * t + 0.5 * s.fdot * t * t)
+        ci = np.cos(s.iota)
+        hp[b] = s.A * (1.0 + ci * ci) * torch.cos(ph)
+        hc[b] = -2.0 * s.A * ci * torch.sin(ph)
+    return hp, hc
+
+
 def band_limited_noise(seed, n_series=3, n_tones=40, f_max=5e-3):
     """Parameters of `n_series` independent sums of sinusoids (laser-noise pin P3).
 

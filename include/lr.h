@@ -106,6 +106,11 @@ void lr_destroy(lr_handle* h);
 /* Set an option (see LR_OPT_*).  Errors: LR_EINVAL for an unknown key or value. */
 int lr_set_option(lr_handle* h, int key, double value);
 
+/* Read an option back (*value receives what lr_set_option stored, or the default).  The binding uses
+ * LR_OPT_CHANNELS to check the size of `out` before a call writes 3 or 6 rows per template.
+ * Errors: LR_EINVAL for a null pointer or an unknown key. */
+int lr_get_option(const lr_handle* h, int key, double* value);
+
 /* Fixed margins in samples (reading A8), computed once from the table maxima R_max = max|x_i|
  * and L_max = max L_ij over the knots, p = (order+1)/2:
  *   m_proj      = ceil((1.001 R_max/c + 1.001 L_max)/dt) + p + 2          y is 0 outside [m_proj, n - m_proj)
@@ -168,6 +173,28 @@ int lr_get_span_halo(const lr_handle* h_proj, const lr_handle* h_tdi, int64_t* l
 int lr_response_host(lr_handle* h_proj, lr_handle* h_tdi, const double* h_plus, const double* h_cross,
                      const double* beta, const double* lambda, const double* psi, int64_t batch, int64_t n,
                      double* out, void* cuda_stream);
+
+/* A shareable TDI plan (the orbit information is "pre-computed and stored for the entirety of the
+ * sampling run").  lr_tdi's FIR path keeps, per tile of 224 samples, the merged Lagrange filters of eqs. 17-20 (the
+ * "plan": a function of the orbits, dt, order, n, t0, generation and chain mode, not of y).  By default every handle
+ * builds and caches its own on first use.  An MCMC driver that runs several handles / streams on the same orbits can
+ * instead build the plan ONCE and attach it to all of them:
+ *   lr_plan_create : builds the plan for h's current options (LR_OPT_T0, generation, chain, path) and a series of n
+ *                    samples on `cuda_stream`, waits for it, and returns an object that is read-only from then on
+ *                    (reference count 1).  LR_EINVAL if h's lr_tdi path is LR_TDI_PER_SAMPLE (no plan), else errors
+ *                    as lr_tdi.
+ *   lr_plan_attach : h uses `plan` (one more reference) for every lr_tdi / lr_response* call whose grid and options
+ *                    equal the plan's; any other call falls back to h's own cached plan.  The plan must come from a
+ *                    handle with the same orbit table, dt and order (LR_EINVAL otherwise).  NULL detaches.
+ *   lr_plan_release: drops the caller's reference; the device memory goes when the last attached handle is destroyed.
+ * Results with an attached plan are bit-identical to those with the handle's own.  Handles that share a plan may be
+ * used from different host threads and streams at the same time (each handle still from one thread at a time). */
+typedef struct lr_plan lr_plan;
+int lr_plan_create(lr_handle* h, int64_t n, void* cuda_stream, lr_plan** out);
+int lr_plan_attach(lr_handle* h, lr_plan* plan);
+void lr_plan_release(lr_plan* plan);
+/* Device bytes the plan holds (0 for NULL). */
+int64_t lr_plan_bytes(const lr_plan* plan);
 
 /* Template generator (eqs. 5-9; SURVEY.md §8(f) NEXT-1 "generate the GB waveform
  * from the parameters").  One template is LR_GB_NPAR doubles
@@ -254,12 +281,6 @@ int lr_eval_orbit(lr_handle* h, int channel, const double* t, int64_t m, double*
  * *inst_per_s = FP64 thread-instructions per second (one DFMA = 1).  The roofline denominator of bench.py.
  * Synchronous.  Errors: LR_EINVAL, LR_ECUDA. */
 int lr_measure_fp64_peak(double seconds, double* inst_per_s);
-
-/* DFMA issue rate of this device for streams whose instructions share 2, 1 or 0 source registers with their
- * neighbours (mode 0, 1, 2), and for mode 1 with one shared-memory load per 7 DFMA (mode 3): the measurements
- * behind the issue rules of DESIGN.md §6 (16 warps per SM, 7 accumulators per thread, a few milliseconds).
- * *inst_per_s = DFMA thread-instructions per second.  Synchronous.  Errors: LR_EINVAL, LR_ECUDA. */
-int lr_probe_fp64_operands(int mode, double* inst_per_s);
 
 /* Number of kernels liblr has launched in this process (all handles); bench.py's gpu_launches. */
 int64_t lr_launch_count(void);

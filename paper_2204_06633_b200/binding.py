@@ -29,8 +29,8 @@ LR_XYZ, LR_AET, LR_XYZ_AET = 0, 1, 2
 LR_MAX_ORDER = 65
 
 # every symbol include/lr.h declares
-SYMBOLS = ("lr_create", "lr_destroy", "lr_set_option", "lr_get_margins", "lr_project", "lr_tdi",
-           "lr_inner_product", "lr_gb_parameters", "lr_fft_good_length", "lr_gb_waveform", "lr_response_gb", "lr_loglike_gb", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_probe_fp64_operands", "lr_launch_count",
+SYMBOLS = ("lr_create", "lr_destroy", "lr_set_option", "lr_get_option", "lr_get_margins", "lr_project", "lr_tdi",
+           "lr_inner_product", "lr_gb_parameters", "lr_fft_good_length", "lr_gb_waveform", "lr_response_gb", "lr_loglike_gb", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count", "lr_plan_create", "lr_plan_attach", "lr_plan_release", "lr_plan_bytes",
            "lr_last_cuda_error", "lr_strerror")
 
 
@@ -73,6 +73,7 @@ def lib():
     L.lr_destroy.argtypes = [vp]
     L.lr_destroy.restype = None
     L.lr_set_option.argtypes = [vp, ci, dbl]
+    L.lr_get_option.argtypes = [vp, ci, ctypes.POINTER(dbl)]
     L.lr_get_margins.argtypes = [vp, pi64, pi64, pi64]
     L.lr_project.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
     L.lr_tdi.argtypes = [vp, vp, i64, i64, vp, vp]
@@ -89,7 +90,12 @@ def lib():
     L.lr_loglike_gb.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, vp, vp, dbl, ci, vp, vp]
     L.lr_eval_orbit.argtypes = [vp, ci, vp, i64, vp, vp]
     L.lr_measure_fp64_peak.argtypes = [dbl, ctypes.POINTER(dbl)]
-    L.lr_probe_fp64_operands.argtypes = [ci, ctypes.POINTER(dbl)]
+    L.lr_plan_create.argtypes = [vp, i64, vp, ctypes.POINTER(vp)]
+    L.lr_plan_attach.argtypes = [vp, vp]
+    L.lr_plan_release.argtypes = [vp]
+    L.lr_plan_release.restype = None
+    L.lr_plan_bytes.argtypes = [vp]
+    L.lr_plan_bytes.restype = i64
     L.lr_launch_count.argtypes = []
     L.lr_launch_count.restype = i64
     L.lr_last_cuda_error.argtypes = [vp]
@@ -148,6 +154,24 @@ def lr_set_option(h, key, value):
     _check(lib().lr_set_option(h, int(key), float(value)), "lr_set_option", h)
 
 
+def lr_get_option(h, key):
+    v = ctypes.c_double()
+    _check(lib().lr_get_option(h, int(key), ctypes.byref(v)), "lr_get_option", h)
+    return v.value
+
+
+def _n_out(h):
+    """Rows per template lr_tdi writes with this handle's LR_OPT_CHANNELS (the C ABI takes no size for `out`)."""
+    return 6 if int(lr_get_option(h, LR_OPT_CHANNELS)) == LR_XYZ_AET else 3
+
+
+def _angles(beta, lam, psi):
+    beta, lam, psi = _host(beta), _host(lam), _host(psi)
+    if lam.size != beta.size or psi.size != beta.size:
+        raise ValueError("beta, lambda, psi must have one entry per template")
+    return beta, lam, psi, beta.size
+
+
 def lr_get_margins(h):
     a, b, c = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
     _check(lib().lr_get_margins(h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)), "lr_get_margins", h)
@@ -156,10 +180,7 @@ def lr_get_margins(h):
 
 def lr_project(h, h_plus, h_cross, beta, lam, psi, y_out, stream=None):
     """lr_project: h_plus, h_cross CUDA [B,N]; beta, lam, psi host [B]; y_out CUDA [B,6,N] (written)."""
-    beta, lam, psi = _host(beta), _host(lam), _host(psi)
-    B = beta.size
-    if lam.size != B or psi.size != B:
-        raise ValueError("beta, lambda, psi must have one entry per template")
+    beta, lam, psi, B = _angles(beta, lam, psi)
     if h_plus.numel() % B:
         raise ValueError("h_plus size is not a multiple of the batch")
     n = h_plus.numel() // B
@@ -174,21 +195,20 @@ def lr_tdi(h, y, out, batch, stream=None):
     if y.numel() % (6 * batch):
         raise ValueError("y must be [batch,6,n]")
     n = y.numel() // (6 * batch)
-    if out.numel() not in (3 * batch * n, 6 * batch * n):
-        raise ValueError("out must be [batch,3,n] or [batch,6,n]")
+    if out.numel() != _n_out(h) * batch * n:
+        raise ValueError(f"out must be [batch,{_n_out(h)},n] for this handle's LR_OPT_CHANNELS")
     _check(lib().lr_tdi(h, _dev_ptr(y, "y"), batch, n, _dev_ptr(out, "out"), _stream(stream)), "lr_tdi", h)
     return out
 
 
 def lr_response(h_proj, h_tdi, h_plus, h_cross, beta, lam, psi, out, stream=None):
     """lr_response: h_plus, h_cross CUDA [B,N] -> out CUDA [B,3|6,N], no y array (chunked through L2)."""
-    beta, lam, psi = _host(beta), _host(lam), _host(psi)
-    B = beta.size
+    beta, lam, psi, B = _angles(beta, lam, psi)
     if h_plus.numel() % B:
         raise ValueError("h_plus size is not a multiple of the batch")
     n = h_plus.numel() // B
-    if out.numel() not in (3 * B * n, 6 * B * n):
-        raise ValueError("out must be [batch,3,n] or [batch,6,n]")
+    if out.numel() != _n_out(h_tdi) * B * n:
+        raise ValueError(f"out must be [batch,{_n_out(h_tdi)},n] for h_tdi's LR_OPT_CHANNELS")
     _check(lib().lr_response(h_proj, h_tdi, _dev_ptr(h_plus, "h_plus"), _dev_ptr(h_cross, "h_cross", B * n),
                              beta.ctypes.data, lam.ctypes.data, psi.ctypes.data, B, n, _dev_ptr(out, "out"),
                              _stream(stream)), "lr_response", h_proj)
@@ -206,13 +226,12 @@ def lr_get_span_halo(h_proj, h_tdi):
 def lr_response_span(h_proj, h_tdi, h_plus, h_cross, h_first, beta, lam, psi, n, first, count, out, stream=None):
     """lr_response_span: h_plus, h_cross CUDA [B, h_len] = global samples [h_first, h_first+h_len) of a series
     of n samples; out CUDA [B, 3|6, count] receives the global samples [first, first+count)."""
-    beta, lam, psi = _host(beta), _host(lam), _host(psi)
-    B = beta.size
+    beta, lam, psi, B = _angles(beta, lam, psi)
     if h_plus.numel() % B:
         raise ValueError("h_plus size is not a multiple of the batch")
     h_len = h_plus.numel() // B
-    if out.numel() not in (3 * B * count, 6 * B * count):
-        raise ValueError("out must be [batch,3,count] or [batch,6,count]")
+    if out.numel() != _n_out(h_tdi) * B * count:
+        raise ValueError(f"out must be [batch,{_n_out(h_tdi)},count] for h_tdi's LR_OPT_CHANNELS")
     _check(lib().lr_response_span(h_proj, h_tdi, _dev_ptr(h_plus, "h_plus"), _dev_ptr(h_cross, "h_cross", B * h_len),
                                   int(h_first), h_len, beta.ctypes.data, lam.ctypes.data, psi.ctypes.data, B, int(n),
                                   int(first), int(count), _dev_ptr(out, "out"), _stream(stream)),
@@ -222,13 +241,13 @@ def lr_response_span(h_proj, h_tdi, h_plus, h_cross, h_first, beta, lam, psi, n,
 
 def lr_response_host(h_proj, h_tdi, h_plus, h_cross, beta, lam, psi, out, stream=None):
     """lr_response_host: host numpy (or pinned CPU tensors viewed as numpy) in, host out; synchronous."""
-    beta, lam, psi = _host(beta), _host(lam), _host(psi)
-    B = beta.size
+    beta, lam, psi, B = _angles(beta, lam, psi)
     hp, hc = _as_host_f64(h_plus), _as_host_f64(h_cross)
     o = _as_host_f64(out)
     n = hp.size // B
-    if hp.size != B * n or hc.size != B * n or o.size not in (3 * B * n, 6 * B * n):
-        raise ValueError("lr_response_host: inconsistent sizes")
+    if hp.size != B * n or hc.size != B * n or o.size != _n_out(h_tdi) * B * n:
+        raise ValueError("lr_response_host: inconsistent sizes (out must hold 3 or 6 rows per template, per "
+                         "h_tdi's LR_OPT_CHANNELS)")
     _check(lib().lr_response_host(h_proj, h_tdi, hp.ctypes.data, hc.ctypes.data, beta.ctypes.data,
                                   lam.ctypes.data, psi.ctypes.data, B, n, o.ctypes.data,
                                   _stream(stream) if stream is not None else _stream(None)),
@@ -277,8 +296,8 @@ def lr_response_gb(h_proj, h_tdi, gb, beta, lam, psi, n, out, stream=None):
     B = g.shape[0]
     if beta.size != B or lam.size != B or psi.size != B:
         raise ValueError("beta, lambda, psi must have one entry per template")
-    if out.numel() not in (3 * B * n, 6 * B * n):
-        raise ValueError("out must be [batch,3,n] or [batch,6,n]")
+    if out.numel() != _n_out(h_tdi) * B * n:
+        raise ValueError(f"out must be [batch,{_n_out(h_tdi)},n] for h_tdi's LR_OPT_CHANNELS")
     _check(lib().lr_response_gb(h_proj, h_tdi, g.ctypes.data, beta.ctypes.data, lam.ctypes.data, psi.ctypes.data,
                                 B, int(n), _dev_ptr(out, "out"), _stream(stream)), "lr_response_gb", h_proj)
     return out
@@ -346,11 +365,23 @@ def lr_measure_fp64_peak(seconds=0.5):
     return v.value
 
 
-def lr_probe_fp64_operands(mode):
-    """DFMA thread-instructions/s with 2 / 1 / 0 shared source registers (mode 0 / 1 / 2), mode 3 = mode 1 + LDS."""
-    v = ctypes.c_double()
-    _check(lib().lr_probe_fp64_operands(int(mode), ctypes.byref(v)), "lr_probe_fp64_operands")
-    return v.value
+def lr_plan_create(h, n, stream=None):
+    """lr_plan_create: the shareable, read-only TDI plan of handle h for a series of n samples."""
+    p = ctypes.c_void_p()
+    _check(lib().lr_plan_create(h, int(n), _stream(stream), ctypes.byref(p)), "lr_plan_create", h)
+    return p
+
+
+def lr_plan_attach(h, plan):
+    _check(lib().lr_plan_attach(h, plan), "lr_plan_attach", h)
+
+
+def lr_plan_release(plan):
+    lib().lr_plan_release(plan)
+
+
+def lr_plan_bytes(plan):
+    return int(lib().lr_plan_bytes(plan))
 
 
 def lr_launch_count():

@@ -71,16 +71,15 @@ def build(force=False, verbose=False):
 
 
 def ensure_built(local_rank=0, timeout_s=900.0):
-    """Build liblr.so if it is MISSING (a fresh checkout: the .so is git-ignored).  Under torchrun only local
-    rank 0 compiles; the other ranks wait for the file.  Building the product is not a fallback: without nvcc
-    this raises."""
+    """Make sure liblr.so exists AND is newer than every source it is built from (the .so is git-ignored but
+    travels with the repo snapshot, so a stale one can sit beside edited sources).  Under torchrun only local
+    rank 0 compiles; the other ranks wait until the library is no longer stale.  Building the product is not a
+    fallback: without nvcc this raises."""
     import time
-    if os.path.exists(LIB):
-        return LIB
     if local_rank == 0:
-        return build(force=True)
+        return build(force=False)
     t0 = time.time()
-    while not os.path.exists(LIB):
+    while _stale():
         if time.time() - t0 > timeout_s:
             raise RuntimeError("timed out waiting for local rank 0 to build liblr.so")
         time.sleep(1.0)

@@ -38,25 +38,40 @@ struct Stage {
 
 }  // namespace
 
-// lr_tdi's FIR plan (lr_tdi_fir.cuh): a function of the orbits and the time grid only, kept between calls
-struct Plan {
+// lr_tdi's FIR plan (lr_tdi_fir.cuh): a function of the orbits and the time grid only, not of y.  Read-only once
+// built, reference counted: the private plan of a handle (rebuilt when the grid or an option changes) or a plan
+// made by lr_plan_create that any number of handles on the same orbits attach to (never rebuilt).
+struct lr_plan {
+  std::atomic<int> refs{1};
+  bool shared = false;                  // made by lr_plan_create: immutable
   double* coef = nullptr;
   int* flags = nullptr;                 // [2 * ntiles + 1]: flags, then count + list of flagged tiles
   size_t coef_cap = 0, flags_cap = 0;   // elements
   bool valid = false;
+  // what the plan was built for
+  uint64_t orbit_id = 0;
   int64_t n = 0;
-  double t0 = 0;
-  int gen = 0, chain = 0, path = 0;
+  double t0 = 0, dt = 0;
+  int order = 0, gen = 0, chain = 0, path = 0;
+  int tiles = 0;                        // plan tiles (1 for constant light times)
   cudaEvent_t ready = nullptr;
-  cudaStream_t side = nullptr;          // the fix-up kernel's stream (forked from / joined to the caller's)
-  cudaEvent_t fork = nullptr, join = nullptr;
   // host copy of the list of flagged tiles (count, then the tiles), fetched once behind the plan kernel: a launch
   // whose window holds no flagged tile needs no fork / fix-up kernel / join
   int* list_host = nullptr;             // pinned, [1 + list_cap]
   size_t list_cap = 0;
   cudaEvent_t list_ev = nullptr;
-  int list_state = 0;                   // 0 unknown | 1 copy in flight | 2 known
+  std::atomic<int> list_state{0};       // 0 unknown | 1 copy in flight | 2 known
 };
+
+static void plan_unref(lr_plan* pl) {
+  if (!pl || pl->refs.fetch_sub(1) != 1) return;
+  if (pl->ready) cudaEventDestroy(pl->ready);
+  if (pl->list_ev) cudaEventDestroy(pl->list_ev);
+  if (pl->list_host) cudaFreeHost(pl->list_host);
+  if (pl->coef) cudaFree(pl->coef);
+  if (pl->flags) cudaFree(pl->flags);
+  delete pl;
+}
 
 struct lr_handle {
   // configuration
@@ -71,7 +86,15 @@ struct lr_handle {
   int sm_count = 0;
   int64_t chunk_samples = 0;   // LR_OPT_CHUNK_SAMPLES: 0 = automatic
   int64_t fft_length = 0;      // LR_OPT_FFT_LENGTH: 0 = n (no zero padding)
-  Plan plan;
+  uint64_t orbit_id = 0;       // hash of the spline coefficients and the knot grid: which orbits a plan belongs to
+  lr_plan* plan = nullptr;     // this handle's own plan (implicit cache)
+  lr_plan* attached = nullptr; // a shared plan (lr_plan_attach), used whenever it matches the call
+  // the fix-up kernel of the FIR path runs on a side stream of the handle, forked from / joined to the caller's
+  cudaStream_t fix_side = nullptr;
+  cudaEvent_t fix_fork = nullptr, fix_join = nullptr;
+  cudaEvent_t last_join = nullptr;   // the event most recently recorded behind a fix-up kernel (it reads plan->flags)
+  // LR_OPT_TDI_PLAN_CACHE = 0 rebuilds the plan once per API call, not once per chunk of a chunked call
+  bool in_call = false, built_in_call = false;
   double bk[lr::kPMax + 1];
   // device state
   lr::D4* coef = nullptr;
@@ -156,7 +179,13 @@ int stage_basis(lr_handle* h, const double* beta, const double* lam, const doubl
   Stage& S = h->stage[h->next_slot];
   h->next_slot = (h->next_slot + 1) % kSlots;
   if (!S.done) LR_CUDA(h, cudaEventCreateWithFlags(&S.done, cudaEventDisableTiming));
-  if (S.pending) { LR_CUDA(h, cudaEventSynchronize(S.done)); S.pending = false; }
+  if (S.pending) {
+    // the slot's earlier users must be done with it: only a rewrite of the pinned host side needs the HOST to wait;
+    // the small path (constants in the kernel's parameter buffer) orders the device side on the stream instead
+    if (batch <= lr::kSmallStage && S.cap >= batch) LR_CUDA(h, cudaStreamWaitEvent(st, S.done, 0));
+    else LR_CUDA(h, cudaEventSynchronize(S.done));
+    S.pending = false;
+  }
   if (S.cap < batch) {
     if (S.host) cudaFreeHost(S.host);
     if (S.dev) cudaFree(S.dev);
@@ -251,6 +280,16 @@ int lr_create(const lr_orbits* orb, double dt, int order, int tdi_gen, lr_handle
       h->max_ldot = fmax(h->max_ldot, m / orb->knot_dt);
     }
 
+  {  // FNV-1a over the coefficients and the knot grid
+    uint64_t id = 1469598103934665603ull;
+    auto mix = [&](const void* p, size_t bytes) {
+      const unsigned char* c = static_cast<const unsigned char*>(p);
+      for (size_t i = 0; i < bytes; ++i) { id ^= c[i]; id *= 1099511628211ull; }
+    };
+    mix(coef.data(), coef.size() * sizeof(lr::D4));
+    mix(&h->n_knots, sizeof(h->n_knots)); mix(&h->t_start, sizeof(h->t_start)); mix(&h->knot_dt, sizeof(h->knot_dt));
+    h->orbit_id = id;
+  }
   cudaError_t e = cudaMalloc(&h->coef, coef.size() * sizeof(lr::D4));
   if (e == cudaSuccess) e = cudaMemcpy(h->coef, coef.data(), coef.size() * sizeof(lr::D4), cudaMemcpyHostToDevice);
   if (e != cudaSuccess) {
@@ -272,14 +311,11 @@ void lr_destroy(lr_handle* h) {
     if (S.host) cudaFreeHost(S.host);
     if (S.dev) cudaFree(S.dev);
   }
-  if (h->plan.ready) cudaEventDestroy(h->plan.ready);
-  if (h->plan.fork) cudaEventDestroy(h->plan.fork);
-  if (h->plan.join) cudaEventDestroy(h->plan.join);
-  if (h->plan.side) cudaStreamDestroy(h->plan.side);
-  if (h->plan.list_ev) cudaEventDestroy(h->plan.list_ev);
-  if (h->plan.list_host) cudaFreeHost(h->plan.list_host);
-  if (h->plan.coef) cudaFree(h->plan.coef);
-  if (h->plan.flags) cudaFree(h->plan.flags);
+  if (h->fix_fork) cudaEventDestroy(h->fix_fork);
+  if (h->fix_join) cudaEventDestroy(h->fix_join);
+  if (h->fix_side) cudaStreamDestroy(h->fix_side);
+  plan_unref(h->plan);
+  plan_unref(h->attached);
   if (h->y_scr) cudaFree(h->y_scr);
   if (h->h_buf) cudaFree(h->h_buf);
   if (h->o_buf) cudaFree(h->o_buf);
@@ -326,7 +362,22 @@ int lr_set_option(lr_handle* h, int key, double value) {
       h->fft_length = (int64_t)value; return LR_OK;
     case LR_OPT_TDI_PLAN_CACHE:
       if (value != 0 && value != 1) return LR_EINVAL;
-      h->plan_cache = (int)value; h->plan.valid = false; return LR_OK;
+      h->plan_cache = (int)value; if (h->plan) h->plan->valid = false; return LR_OK;
+    default: return LR_EINVAL;
+  }
+}
+
+int lr_get_option(const lr_handle* h, int key, double* value) {
+  if (!h || !value) return LR_EINVAL;
+  switch (key) {
+    case LR_OPT_T0: *value = h->t0; return LR_OK;
+    case LR_OPT_CHAIN: *value = h->chain; return LR_OK;
+    case LR_OPT_CHANNELS: *value = h->channels; return LR_OK;
+    case LR_OPT_TDI_GEN: *value = h->gen; return LR_OK;
+    case LR_OPT_TDI_PATH: *value = h->tdi_path; return LR_OK;
+    case LR_OPT_CHUNK_SAMPLES: *value = (double)h->chunk_samples; return LR_OK;
+    case LR_OPT_FFT_LENGTH: *value = (double)h->fft_length; return LR_OK;
+    case LR_OPT_TDI_PLAN_CACHE: *value = h->plan_cache; return LR_OK;
     default: return LR_EINVAL;
   }
 }
@@ -396,6 +447,82 @@ TdiShape tdi_shape(const lr_handle* h) {
   return t;
 }
 
+bool plan_matches(const lr_plan* pl, const lr_handle* h, int64_t n_glob, int path) {
+  return pl && pl->valid && pl->orbit_id == h->orbit_id && pl->n == n_glob && pl->t0 == h->t0 && pl->dt == h->dt &&
+         pl->order == h->order && pl->gen == h->gen && pl->chain == h->chain && pl->path == path;
+}
+
+// FIR-path fields of the kernel parameters that do not depend on the launch window
+void fir_params(const lr_handle* h, const TdiShape& ts, int64_t n_glob, lr::Params& P) {
+  P.halo_lo = ts.halo_lo; P.halo_hi = ts.halo_hi; P.fir_wc = ts.wc; P.fir_taps = ts.taps;
+  // the plan covers the whole series (global tiles); with constant light times every tile has the same
+  // filters, so the plan is ONE tile (the constant-delay fast path of SURVEY.md §8(f) NEXT-4)
+  const bool uniform = h->const_ltt;
+  P.fir_uniform = uniform ? 1 : 0;
+  P.fir_tile0 = uniform ? (int)(h->m_front(h->gen) / lr::kFirTile) : 0;
+  P.ntiles = uniform ? 1 : (int)((n_glob + lr::kFirTile - 1) / lr::kFirTile);
+}
+
+// (Re)build `pl` for this handle's grid and options on `st`.  wait_list: block until the list of flagged tiles
+// is on the host (lr_plan_create: the plan is then complete and immutable when the call returns).
+int build_plan(lr_handle* h, lr_plan* pl, const TdiShape& ts, int64_t n_glob, cudaStream_t st, bool wait_list) {
+  lr::Params P = make_params(h, n_glob);
+  fir_params(h, ts, n_glob, P);
+  const size_t need = (size_t)P.ntiles * lr::fir_plan_doubles_per_tile(P.fir_wc);
+  pl->valid = false;
+  pl->list_state = 0;
+  if (pl->coef_cap < need) {
+    if (pl->coef) { cudaFree(pl->coef); pl->coef = nullptr; pl->coef_cap = 0; }
+    LR_CUDA(h, cudaMalloc(&pl->coef, need * sizeof(double)));
+    pl->coef_cap = need;
+  }
+  if (pl->flags_cap < (size_t)P.ntiles) {
+    if (pl->flags) { cudaFree(pl->flags); pl->flags = nullptr; pl->flags_cap = 0; }
+    LR_CUDA(h, cudaMalloc(&pl->flags, (2 * (size_t)P.ntiles + 1) * sizeof(int)));
+    pl->flags_cap = (size_t)P.ntiles;
+  }
+  if (!pl->ready) LR_CUDA(h, cudaEventCreateWithFlags(&pl->ready, cudaEventDisableTiming));
+  // a fix-up kernel of an earlier launch may still be reading the list this build rewrites
+  if (h->last_join) LR_CUDA(h, cudaStreamWaitEvent(st, h->last_join, 0));
+  int* list = pl->flags + P.ntiles;
+  const int e = lr::launch_fir_plan(P, h->order, h->gen, ts.path, pl->coef, pl->flags, list, P.ntiles, (void*)st);
+  if (e != 0) { h->last_cuda = e; return LR_ECUDA; }
+  LR_CUDA(h, cudaEventRecord(pl->ready, st));
+  pl->orbit_id = h->orbit_id; pl->n = n_glob; pl->t0 = h->t0; pl->dt = h->dt; pl->order = h->order;
+  pl->gen = h->gen; pl->chain = h->chain; pl->path = ts.path; pl->tiles = P.ntiles;
+  pl->valid = true;
+  // the list of flagged tiles comes to the host behind the plan kernel (no synchronisation unless asked: a later
+  // call that finds the copy finished uses it, until then every launch runs the fix-up kernel)
+  const size_t words = 1 + (size_t)P.ntiles;
+  if (pl->list_cap < words) {
+    if (pl->list_host) { cudaFreeHost(pl->list_host); pl->list_host = nullptr; pl->list_cap = 0; }
+    if (cudaMallocHost(&pl->list_host, words * sizeof(int)) == cudaSuccess) pl->list_cap = words;
+    else (void)cudaGetLastError();
+  }
+  if (!pl->list_ev && cudaEventCreateWithFlags(&pl->list_ev, cudaEventDisableTiming) != cudaSuccess) {
+    pl->list_ev = nullptr;
+    (void)cudaGetLastError();
+  }
+  if (pl->list_cap >= words && pl->list_ev) {
+    LR_CUDA(h, cudaMemcpyAsync(pl->list_host, list, words * sizeof(int), cudaMemcpyDeviceToHost, st));
+    LR_CUDA(h, cudaEventRecord(pl->list_ev, st));
+    pl->list_state = 1;
+    if (wait_list) {
+      LR_CUDA(h, cudaEventSynchronize(pl->list_ev));
+      pl->list_state = 2;
+    }
+  }
+  return LR_OK;
+}
+
+// With LR_OPT_TDI_PLAN_CACHE = 0 the plan is rebuilt once per API call (before its first launch), not once per
+// chunk of a chunked call: the entry points open a PlanCall on the TDI handle.
+struct PlanCall {
+  lr_handle* h; bool outer;
+  explicit PlanCall(lr_handle* h_) : h(h_), outer(h_ && !h_->in_call) { if (outer) { h->in_call = true; h->built_in_call = false; } }
+  ~PlanCall() { if (outer) h->in_call = false; }
+};
+
 // join_later: if non-null and the FIR path runs, the fix-up kernel's completion is recorded there and the
 // caller's stream does NOT wait for it (set to nullptr by the per-sample path, which has no fix-up kernel).
 int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, double* out, void* stream,
@@ -404,38 +531,30 @@ int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, do
   const TdiShape ts = tdi_shape(h);
   const int path = ts.path;
   cudaStream_t st = (cudaStream_t)stream;
-  lr::FirPlanArgs pa{nullptr, nullptr, nullptr, 0, 0, nullptr, nullptr, nullptr, true, false};
+  lr::FirPlanArgs pa{};
+  pa.wait_join = true;
   P.halo_lo = ts.halo_lo; P.halo_hi = ts.halo_hi; P.fir_wc = ts.wc; P.fir_taps = ts.taps;
   if (path != LR_TDI_PER_SAMPLE) {
     if (w.off % lr::kFirTile != 0) return LR_EINVAL;   // windows of the FIR path start on a tile
-    // the plan covers the whole series (global tiles); with constant light times every tile has the same
-    // filters, so the plan is ONE tile (the constant-delay fast path of SURVEY.md §8(f) NEXT-4)
+    fir_params(h, ts, w.n_glob, P);
     const bool uniform = h->const_ltt;
-    P.fir_uniform = uniform ? 1 : 0;
-    P.fir_tile0 = uniform ? (int)(h->m_front(h->gen) / lr::kFirTile) : 0;
-    P.ntiles = uniform ? 1 : (int)((w.n_glob + lr::kFirTile - 1) / lr::kFirTile);
-    Plan& pl = h->plan;
-    const bool reuse = h->plan_cache && pl.valid && pl.n == w.n_glob && pl.t0 == h->t0 && pl.gen == h->gen &&
-                       pl.chain == h->chain && pl.path == path;
-    if (!reuse) {
-      const size_t need = (size_t)P.ntiles * lr::fir_plan_doubles_per_tile(P.fir_wc);
-      pl.valid = false;
-      pl.list_state = 0;
-      if (pl.coef_cap < need) {
-        if (pl.coef) { cudaFree(pl.coef); pl.coef = nullptr; pl.coef_cap = 0; }
-        LR_CUDA(h, cudaMalloc(&pl.coef, need * sizeof(double)));
-        pl.coef_cap = need;
+    // which plan: a shared one that fits this call, else the handle's own (built on first use, kept while it fits)
+    lr_plan* pl = plan_matches(h->attached, h, w.n_glob, path) ? h->attached : nullptr;
+    if (!pl) {
+      if (!h->plan) {
+        h->plan = new (std::nothrow) lr_plan();
+        if (!h->plan) return LR_ENOMEM;
       }
-      if (pl.flags_cap < (size_t)P.ntiles) {
-        if (pl.flags) { cudaFree(pl.flags); pl.flags = nullptr; pl.flags_cap = 0; }
-        LR_CUDA(h, cudaMalloc(&pl.flags, (2 * (size_t)P.ntiles + 1) * sizeof(int)));
-        pl.flags_cap = (size_t)P.ntiles;
+      pl = h->plan;
+      const bool fresh = h->plan_cache || (h->in_call && h->built_in_call);
+      if (!(fresh && plan_matches(pl, h, w.n_glob, path))) {
+        const int rc = build_plan(h, pl, ts, w.n_glob, st, false);
+        if (rc != LR_OK) return rc;
+        h->built_in_call = true;
       }
-      if (!pl.ready) LR_CUDA(h, cudaEventCreateWithFlags(&pl.ready, cudaEventDisableTiming));
-    } else {
-      LR_CUDA(h, cudaStreamWaitEvent(st, pl.ready, 0));   // the plan may have been built on another stream
     }
-    pa.coef = pl.coef; pa.flags = pl.flags; pa.list = pl.flags + P.ntiles; pa.build = !reuse;
+    LR_CUDA(h, cudaStreamWaitEvent(st, pl->ready, 0));   // the plan may have been built on another stream
+    pa.coef = pl->coef; pa.flags = pl->flags; pa.list = pl->flags + P.ntiles;
     pa.plan_tiles = P.ntiles;
     if (h->sm_count == 0) {
       int dev = 0;
@@ -443,34 +562,35 @@ int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, do
       LR_CUDA(h, cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev));
     }
     pa.fixup_grid = 2 * h->sm_count;
-    if (!pl.side) {
+    if (!h->fix_side) {
       // highest priority: the side stream starts a few microseconds behind the apply kernel (it waits for the fork
       // event), by which time the apply kernel's CTAs hold every SM; at equal priority the fix-up CTAs were only
       // dispatched once the apply grid had drained and became a 40 us tail of every lr_tdi call
       int prio_lo = 0, prio_hi = 0;
       LR_CUDA(h, cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
-      LR_CUDA(h, cudaStreamCreateWithPriority(&pl.side, cudaStreamNonBlocking, prio_hi));
-      LR_CUDA(h, cudaEventCreateWithFlags(&pl.fork, cudaEventDisableTiming));
-      LR_CUDA(h, cudaEventCreateWithFlags(&pl.join, cudaEventDisableTiming));
+      LR_CUDA(h, cudaStreamCreateWithPriority(&h->fix_side, cudaStreamNonBlocking, prio_hi));
+      LR_CUDA(h, cudaEventCreateWithFlags(&h->fix_fork, cudaEventDisableTiming));
+      LR_CUDA(h, cudaEventCreateWithFlags(&h->fix_join, cudaEventDisableTiming));
     }
-    pa.side = pl.side; pa.fork = pl.fork; pa.join = pl.join;
-    if (reuse && pl.list_state == 1) {
-      if (cudaEventQuery(pl.list_ev) == cudaSuccess) pl.list_state = 2;
+    pa.side = h->fix_side; pa.fork = h->fix_fork; pa.join = h->fix_join;
+    if (pl->list_state.load() == 1) {
+      if (cudaEventQuery(pl->list_ev) == cudaSuccess) pl->list_state = 2;
       else (void)cudaGetLastError();   // cudaErrorNotReady is not an error of this call
     }
-    if (reuse && pl.list_state == 2) {
-      const int cnt = pl.list_host[0];
+    if (pl->list_state.load() == 2) {
+      const int cnt = pl->list_host[0];
       bool any = cnt > 0 && uniform;   // (one-tile plan: a flagged plan tile concerns every window)
       if (cnt > 0 && !uniform) {
         const int64_t t_lo = w.off / lr::kFirTile, t_hi = t_lo + (w.n + lr::kFirTile - 1) / lr::kFirTile;
-        for (int i = 1; i <= cnt && !any; ++i) any = pl.list_host[i] >= t_lo && pl.list_host[i] < t_hi;
+        for (int i = 1; i <= cnt && !any; ++i) any = pl->list_host[i] >= t_lo && pl->list_host[i] < t_hi;
       }
       pa.skip_fixup = !any;
     }
     if (join_later) {
       if (pa.skip_fixup) *join_later = nullptr;   // nothing to wait for
-      else { pa.join = *join_later; pa.wait_join = false; }
+      else { pa.join_extra = *join_later; pa.wait_join = false; }
     }
+    if (!pa.skip_fixup) h->last_join = h->fix_join;
     apply_window(P, w);
     P.ntiles = (int)((w.n + lr::kFirTile - 1) / lr::kFirTile);
   } else {
@@ -480,31 +600,6 @@ int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, do
   }
   const int e = lr::launch_tdi(P, h->order, h->gen, path, h->channels, y, out, batch, pa, stream);
   if (e != 0) { h->last_cuda = e; return LR_ECUDA; }
-  if (pa.build) {
-    Plan& pl = h->plan;
-    LR_CUDA(h, cudaEventRecord(pl.ready, st));
-    pl.valid = true; pl.n = w.n_glob; pl.t0 = h->t0; pl.gen = h->gen; pl.chain = h->chain; pl.path = path;
-    // the list of flagged tiles comes to the host behind the plan kernel (no synchronisation: a later call that
-    // finds the copy finished uses it, until then every launch runs the fix-up kernel)
-    pl.list_state = 0;
-    if (h->plan_cache) {
-      const size_t words = 1 + (size_t)pa.plan_tiles;
-      if (pl.list_cap < words) {
-        if (pl.list_host) { cudaFreeHost(pl.list_host); pl.list_host = nullptr; pl.list_cap = 0; }
-        if (cudaMallocHost(&pl.list_host, words * sizeof(int)) == cudaSuccess) pl.list_cap = words;
-        else (void)cudaGetLastError();
-      }
-      if (!pl.list_ev && cudaEventCreateWithFlags(&pl.list_ev, cudaEventDisableTiming) != cudaSuccess) {
-        pl.list_ev = nullptr;
-        (void)cudaGetLastError();
-      }
-      if (pl.list_cap >= words && pl.list_ev) {
-        LR_CUDA(h, cudaMemcpyAsync(pl.list_host, pa.list, words * sizeof(int), cudaMemcpyDeviceToHost, st));
-        LR_CUDA(h, cudaEventRecord(pl.list_ev, st));
-        pl.list_state = 1;
-      }
-    }
-  }
   return LR_OK;
 }
 
@@ -547,6 +642,7 @@ int lr_tdi(lr_handle* h, const double* y, int64_t batch, int64_t n, double* out,
   const int rc = check_tdi(h, batch, n);
   if (rc != LR_OK) return rc;
   const Window w{n, 0, n, 0, n, n, n};
+  PlanCall call(h);
   return tdi_window(h, y, batch, w, out, stream);
 }
 
@@ -626,6 +722,7 @@ int lr_response_span(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const
   const int64_t need_a = first - ts.halo_lo - mp > 0 ? first - ts.halo_lo - mp : 0;
   const int64_t need_b = first + count + ts.halo_hi + mp < n ? first + count + ts.halo_hi + mp : n;
   if (h_first > need_a || h_first + h_len < need_b) return LR_EINVAL;
+  PlanCall call(ht_);
   cudaStream_t st = (cudaStream_t)stream;
   const int nout = ht_->channels == LR_XYZ_AET ? 6 : 3;
   // y of one chunk bounds the footprint: no [batch][6][n] buffer
@@ -676,6 +773,13 @@ int lr_response_host(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const
   int rc = check_project(h, batch, n);
   if (rc == LR_OK) rc = check_tdi(ht_, batch, n);
   if (rc != LR_OK) return rc;
+  {   // the 2-D copies below use the row pitch n * 8 bytes
+    int dev = 0, max_pitch = 0;
+    LR_CUDA(h, cudaGetDevice(&dev));
+    LR_CUDA(h, cudaDeviceGetAttribute(&max_pitch, cudaDevAttrMaxPitch, dev));
+    if (n * (int64_t)sizeof(double) > (int64_t)max_pitch) return LR_EINVAL;
+  }
+  PlanCall call(ht_);
   cudaStream_t st = (cudaStream_t)stream;
   const TdiShape ts = tdi_shape(ht_);
   const int nout = ht_->channels == LR_XYZ_AET ? 6 : 3;
@@ -800,6 +904,7 @@ int response_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const double* 
   if (rc != LR_OK) return rc;
   for (int64_t i = 0; i < batch * 6; ++i)
     if (!std::isfinite(gb[i])) return LR_EINVAL;
+  PlanCall call(ht_);
   cudaStream_t st = (cudaStream_t)stream;
   const TdiShape ts = tdi_shape(ht_);
   const int nout = ht_->channels == LR_XYZ_AET ? 6 : 3;
@@ -865,6 +970,12 @@ int lr_loglike_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const double
   if (!h || !ht_ || !gb || !beta || !lam || !psi || !data_f || !inv_psd || !out) return LR_EINVAL;
   if (ht_->channels == LR_XYZ_AET || n < 2 || n > 0x7fffffff) return LR_EINVAL;   // three channels per template
   if (mode != LR_IP_CROSS && mode != LR_IP_DIFF) return LR_EINVAL;
+  {   // sizes before any allocation (batch < 1 is LR_EINVAL, not a failed cudaMalloc)
+    int rc0 = check_project(h, batch, n);
+    if (rc0 == LR_OK) rc0 = check_tdi(ht_, batch, n);
+    if (rc0 != LR_OK) return rc0;
+  }
+  PlanCall call(ht_);
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t nt = h->fft_length > 0 ? h->fft_length : n;   // transform length (zero padded beyond n)
   if (nt < n) return LR_EINVAL;
@@ -942,6 +1053,37 @@ int lr_loglike_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const double
   for (int i = 0; i < 2; ++i)   // join: `out` is complete on the caller's stream
     if (busy[i]) LR_CUDA(h, cudaStreamWaitEvent(st, h->ev_fft[i], 0));
   return LR_OK;
+}
+
+int lr_plan_create(lr_handle* h, int64_t n, void* stream, lr_plan** out) {
+  if (!h || !out) return LR_EINVAL;
+  *out = nullptr;
+  const int rc = check_tdi(h, 1, n);
+  if (rc != LR_OK) return rc;
+  const TdiShape ts = tdi_shape(h);
+  if (ts.path == LR_TDI_PER_SAMPLE) return LR_EINVAL;   // the per-sample path has no plan
+  lr_plan* pl = new (std::nothrow) lr_plan();
+  if (!pl) return LR_ENOMEM;
+  pl->shared = true;
+  const int rb = build_plan(h, pl, ts, n, (cudaStream_t)stream, true);
+  if (rb != LR_OK) { plan_unref(pl); return rb; }
+  *out = pl;
+  return LR_OK;
+}
+
+int lr_plan_attach(lr_handle* h, lr_plan* plan) {
+  if (!h) return LR_EINVAL;
+  if (plan && (plan->orbit_id != h->orbit_id || plan->dt != h->dt || plan->order != h->order)) return LR_EINVAL;
+  if (plan) plan->refs.fetch_add(1);
+  plan_unref(h->attached);
+  h->attached = plan;
+  return LR_OK;
+}
+
+void lr_plan_release(lr_plan* plan) { plan_unref(plan); }
+
+int64_t lr_plan_bytes(const lr_plan* plan) {
+  return plan ? (int64_t)(plan->coef_cap * sizeof(double) + (2 * plan->flags_cap + 1) * sizeof(int)) : 0;
 }
 
 int lr_gb_parameters(double A, double f0, double fdot, double phi0, double iota, int form, double* gb) {

@@ -46,26 +46,38 @@ static int launch_tdi_generic(const Params& prm, int channels, const double* y, 
   return (int)cudaGetLastError();
 }
 
-// FIR path: (re)build the plan if asked, apply it, then run the flagged tiles with per-sample weights
+// FIR path, plan: one CTA per tile of the whole series (prm.ntiles = plan_tiles, window = the whole series)
+template <int PT, int GEN, int NN>
+static int launch_fir_plan_g(const Params& prm, double* coef, int* flags, int* list, int plan_tiles, cudaStream_t st) {
+  const int P = PT > 0 ? PT : prm.p;
+  cudaError_t e;
+  const size_t smem = ((sizeof(FirTile<GEN, NN>) + 15) / 16) * 16 +
+                      (size_t)FirTile<GEN, NN>::NT * NN * (2 * P - 1) * sizeof(double);
+  if ((e = prepare(tdi_fir_setup_kernel<PT, GEN, NN>, smem)) != cudaSuccess) return (int)e;
+  if ((e = cudaMemsetAsync(list, 0, sizeof(int), st)) != cudaSuccess) return (int)e;
+  tdi_fir_setup_kernel<PT, GEN, NN><<<(unsigned)plan_tiles, kFirSetupThreads, smem, st>>>(prm, coef, flags, list);
+  g_launches.fetch_add(1);
+  return (int)cudaGetLastError();
+}
+
+template <int PT>
+int launch_fir_plan_t(const Params& prm, int gen, int path, double* coef, int* flags, int* list, int plan_tiles,
+                      void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  if (path == kPathFir3)
+    return gen == 1 ? launch_fir_plan_g<PT, 1, 3>(prm, coef, flags, list, plan_tiles, st)
+                    : launch_fir_plan_g<PT, 2, 3>(prm, coef, flags, list, plan_tiles, st);
+  return gen == 1 ? launch_fir_plan_g<PT, 1, 4>(prm, coef, flags, list, plan_tiles, st)
+                  : launch_fir_plan_g<PT, 2, 4>(prm, coef, flags, list, plan_tiles, st);
+}
+
+// FIR path, apply: filter every tile the plan did not flag, and run the flagged tiles with per-sample weights
 template <int PT, int GEN, int NN>
 static int launch_tdi_fir(const Params& prm, int channels, const double* y, double* out, int64_t batch,
                           const FirPlanArgs& plan, cudaStream_t st) {
-  const int P = PT > 0 ? PT : prm.p;
   cudaError_t e;
-  if (plan.build) {
-    const size_t smem = ((sizeof(FirTile<GEN, NN>) + 15) / 16) * 16 +
-                        (size_t)FirTile<GEN, NN>::NT * NN * (2 * P - 1) * sizeof(double);
-    if ((e = prepare(tdi_fir_setup_kernel<PT, GEN, NN>, smem)) != cudaSuccess) return (int)e;
-    if ((e = cudaMemsetAsync(plan.list, 0, sizeof(int), st)) != cudaSuccess) return (int)e;
-    Params full = prm;   // the plan covers the whole series, whatever window this launch filters
-    full.n = prm.n_glob; full.n_off = 0;
-    tdi_fir_setup_kernel<PT, GEN, NN><<<(unsigned)plan.plan_tiles, kFirSetupThreads, smem, st>>>(full, plan.coef,
-                                                                                             plan.flags, plan.list);
-    g_launches.fetch_add(1);
-    if ((e = cudaGetLastError()) != cudaSuccess) return (int)e;
-  }
   const int W = kFirTile + prm.halo_lo + prm.halo_hi;
-  const bool fixup = plan.build || !plan.skip_fixup;
+  const bool fixup = !plan.skip_fixup;
   if (fixup) {
     // fork: the flagged tiles (a handful, but each is a long dependent computation) run on the handle's side
     // stream while the apply kernel fills the GPU; the two write disjoint tiles of `out`
@@ -79,6 +91,7 @@ static int launch_tdi_fir(const Params& prm, int channels, const double* y, doub
     g_launches.fetch_add(1);
     if ((e = cudaGetLastError()) != cudaSuccess) return (int)e;
     if ((e = cudaEventRecord((cudaEvent_t)plan.join, side)) != cudaSuccess) return (int)e;
+    if (plan.join_extra && (e = cudaEventRecord((cudaEvent_t)plan.join_extra, side)) != cudaSuccess) return (int)e;
   }
 
   const size_t smem = fir_apply_smem_bytes(W, prm.fir_wc);
@@ -113,6 +126,7 @@ int launch_tdi_t(const Params& prm, int gen, int path, int channels, const doubl
 
 template int launch_project_t<LR_INST_PT>(const Params&, const double*, const double*, const double*, double*,
                                           int64_t, void*);
+template int launch_fir_plan_t<LR_INST_PT>(const Params&, int, int, double*, int*, int*, int, void*);
 template int launch_tdi_t<LR_INST_PT>(const Params&, int, int, int, const double*, double*, int64_t,
                                       const FirPlanArgs&, void*);
 

@@ -59,7 +59,6 @@ int launch_source_basis_small(const SmallStage& s, double* slot, void* stream) {
 int launch_project(const Params& prm, int order, const double* hp, const double* hc, const double* basis,
                    double* y, int64_t batch, void* stream) {
   switch (order) {
-#ifndef LR_DEV_ONLY_P13
     case 1: return launch_project_t<1>(prm, hp, hc, basis, y, batch, stream);
     case 3: return launch_project_t<2>(prm, hp, hc, basis, y, batch, stream);
     case 5: return launch_project_t<3>(prm, hp, hc, basis, y, batch, stream);
@@ -71,7 +70,6 @@ int launch_project(const Params& prm, int order, const double* hp, const double*
     case 21: return launch_project_t<11>(prm, hp, hc, basis, y, batch, stream);
     case 31: return launch_project_t<16>(prm, hp, hc, basis, y, batch, stream);
     case 41: return launch_project_t<21>(prm, hp, hc, basis, y, batch, stream);
-#endif
     case 25: return launch_project_t<13>(prm, hp, hc, basis, y, batch, stream);
     default: return launch_project_t<0>(prm, hp, hc, basis, y, batch, stream);
   }
@@ -80,7 +78,6 @@ int launch_project(const Params& prm, int order, const double* hp, const double*
 int launch_tdi(const Params& prm, int order, int gen, int path, int channels, const double* y, double* out,
                int64_t batch, const FirPlanArgs& plan, void* stream) {
   switch (order) {
-#ifndef LR_DEV_ONLY_P13
     case 1: return launch_tdi_t<1>(prm, gen, path, channels, y, out, batch, plan, stream);
     case 3: return launch_tdi_t<2>(prm, gen, path, channels, y, out, batch, plan, stream);
     case 5: return launch_tdi_t<3>(prm, gen, path, channels, y, out, batch, plan, stream);
@@ -92,9 +89,27 @@ int launch_tdi(const Params& prm, int order, int gen, int path, int channels, co
     case 21: return launch_tdi_t<11>(prm, gen, path, channels, y, out, batch, plan, stream);
     case 31: return launch_tdi_t<16>(prm, gen, path, channels, y, out, batch, plan, stream);
     case 41: return launch_tdi_t<21>(prm, gen, path, channels, y, out, batch, plan, stream);
-#endif
     case 25: return launch_tdi_t<13>(prm, gen, path, channels, y, out, batch, plan, stream);
     default: return launch_tdi_t<0>(prm, gen, path, channels, y, out, batch, plan, stream);
+  }
+}
+
+int launch_fir_plan(const Params& prm, int order, int gen, int path, double* coef, int* flags, int* list,
+                    int plan_tiles, void* stream) {
+  switch (order) {
+    case 1: return launch_fir_plan_t<1>(prm, gen, path, coef, flags, list, plan_tiles, stream);
+    case 3: return launch_fir_plan_t<2>(prm, gen, path, coef, flags, list, plan_tiles, stream);
+    case 5: return launch_fir_plan_t<3>(prm, gen, path, coef, flags, list, plan_tiles, stream);
+    case 7: return launch_fir_plan_t<4>(prm, gen, path, coef, flags, list, plan_tiles, stream);
+    case 9: return launch_fir_plan_t<5>(prm, gen, path, coef, flags, list, plan_tiles, stream);
+    case 11: return launch_fir_plan_t<6>(prm, gen, path, coef, flags, list, plan_tiles, stream);
+    case 13: return launch_fir_plan_t<7>(prm, gen, path, coef, flags, list, plan_tiles, stream);
+    case 15: return launch_fir_plan_t<8>(prm, gen, path, coef, flags, list, plan_tiles, stream);
+    case 21: return launch_fir_plan_t<11>(prm, gen, path, coef, flags, list, plan_tiles, stream);
+    case 31: return launch_fir_plan_t<16>(prm, gen, path, coef, flags, list, plan_tiles, stream);
+    case 41: return launch_fir_plan_t<21>(prm, gen, path, coef, flags, list, plan_tiles, stream);
+    case 25: return launch_fir_plan_t<13>(prm, gen, path, coef, flags, list, plan_tiles, stream);
+    default: return launch_fir_plan_t<0>(prm, gen, path, coef, flags, list, plan_tiles, stream);
   }
 }
 

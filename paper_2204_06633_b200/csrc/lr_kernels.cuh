@@ -152,7 +152,7 @@ constexpr int kPathGeneric = 0;  // tdi_kernel: exact per-sample weights
 constexpr int kPathFir3 = 3;     // tdi_fir_kernel, quadratic in tile time
 constexpr int kPathFir4 = 4;     // tdi_fir_kernel, cubic in tile time
 
-// FIR plan buffers (owned by the handle) and whether this launch must (re)build them
+// FIR plan buffers (a plan object of lr_api.cu) and the fix-up machinery of the launching handle
 struct FirPlanArgs {
   double* coef;   // DEVICE [ntiles][12][Wc][kFirKStride]
   int* flags;     // DEVICE [ntiles]: != 0 marks a tile that needs per-sample weights
@@ -160,11 +160,11 @@ struct FirPlanArgs {
   int plan_tiles; // tiles of the plan (the whole series)
   int fixup_grid; // CTAs of the fix-up kernel (2 per SM)
   void* side;     // cudaStream_t owned by the handle: the fix-up kernel runs there, beside the apply kernel
-  void* fork;     // cudaEvent_t: the caller's stream reached the plan
-  void* join;     // cudaEvent_t: the fix-up kernel finished
+  void* fork;     // cudaEvent_t: the caller's stream reached the launch
+  void* join;     // cudaEvent_t owned by the handle: the fix-up kernel finished
+  void* join_extra; // optional second cudaEvent_t recorded at the same point (a chunked caller's per-slot event)
   bool wait_join; // true: the caller's stream waits for `join` before the launcher returns; false: the caller
-                  // orders later work after `join` itself (chunked response: the next chunk overlaps the fix-up)
-  bool build;
+                  // orders later work after `join_extra` itself (chunked response: the next chunk overlaps the fix-up)
   bool skip_fixup; // the host knows that no flagged tile lies in this launch's window: no fork / fix-up / join
 };
 
@@ -192,7 +192,13 @@ template <int PT>
 int launch_tdi_t(const Params& prm, int gen, int path, int channels, const double* y, double* out, int64_t batch,
                  const FirPlanArgs& plan, void* stream);
 
+template <int PT>
+int launch_fir_plan_t(const Params& prm, int gen, int path, double* coef, int* flags, int* list, int plan_tiles,
+                      void* stream);
+
 // dispatch on the Lagrange order (lr_kernels.cu)
+int launch_fir_plan(const Params& prm, int order, int gen, int path, double* coef, int* flags, int* list,
+                    int plan_tiles, void* stream);
 int launch_project(const Params& prm, int order, const double* hp, const double* hc, const double* basis,
                    double* y, int64_t batch, void* stream);
 int launch_tdi(const Params& prm, int order, int gen, int path, int channels, const double* y, double* out,

@@ -39,80 +39,7 @@ __global__ void __launch_bounds__(256) dfma_kernel(double a, double b, int64_t o
   for (int c = 0; c < kChains; ++c) s += acc[c];
   if (s == 123.456) sink[0] = s;  // never true for the arguments used; keeps the chains alive
 }
-// The DFMA streams behind DESIGN.md §6's issue rules: 7 accumulators per thread, each instruction
-// acc[i] = fma(x, y, acc[i]) with (x, y) =
-//   mode 0: (c[j], w[j])      both sources shared with the neighbouring instructions
-//   mode 1: (c[i], w[j])      one source shared
-//   mode 2: (c[i], w[i])      none shared: three registers the previous instruction did not read
-//   mode 3: mode 1 plus one shared-memory load (LDS.64, immediate offset) per 7 DFMA, as in a filter loop
-template <int MODE>
-__global__ void __launch_bounds__(128) dfma_operand_kernel(const double* __restrict__ in, int iters, double* out) {
-  __shared__ double ks[64];
-  if (threadIdx.x < 64) ks[threadIdx.x] = in[threadIdx.x];
-  __syncthreads();
-  double acc[7], c[7], w[7];
-#pragma unroll
-  for (int i = 0; i < 7; ++i) { acc[i] = in[i]; c[i] = in[7 + i + threadIdx.x % 3]; w[i] = in[14 + i + threadIdx.x % 5]; }
-  for (int it = 0; it < iters; ++it) {
-    const double* kp = ks + (it & 31);
-#pragma unroll
-    for (int j = 0; j < 7; ++j) {
-      const double wj = MODE == 3 ? kp[j] : w[j];
-#pragma unroll
-      for (int i = 0; i < 7; ++i) {
-        if (MODE == 0) acc[i] = fma(c[j], w[j], acc[i]);
-        if (MODE == 1 || MODE == 3) acc[i] = fma(c[i], wj, acc[i]);
-        if (MODE == 2) acc[i] = fma(c[i], w[i], acc[i]);
-      }
-    }
-  }
-  double s = 0.0;
-#pragma unroll
-  for (int i = 0; i < 7; ++i) s += acc[i];
-  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
-}
-
-template <int MODE>
-static int run_operand_probe(int sms, int iters, double* rate) {
-  const int blocks = sms * 4, threads = 128;
-  double *in = nullptr, *out = nullptr;
-  if (cudaMalloc(&in, 64 * sizeof(double)) != cudaSuccess) return LR_ECUDA;
-  if (cudaMalloc(&out, (size_t)blocks * threads * sizeof(double)) != cudaSuccess) { cudaFree(in); return LR_ECUDA; }
-  cudaMemset(in, 0, 64 * sizeof(double));
-  cudaEvent_t e0, e1;
-  cudaEventCreate(&e0);
-  cudaEventCreate(&e1);
-  dfma_operand_kernel<MODE><<<blocks, threads>>>(in, 16, out);
-  cudaEventRecord(e0);
-  dfma_operand_kernel<MODE><<<blocks, threads>>>(in, iters, out);
-  cudaEventRecord(e1);
-  g_launches.fetch_add(2);
-  int rc = LR_OK;
-  if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = LR_ECUDA;
-  float ms = 0;
-  cudaEventElapsedTime(&ms, e0, e1);
-  *rate = (double)blocks * threads * 49.0 * (double)iters / (ms * 1e-3);
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  cudaFree(in);
-  cudaFree(out);
-  return rc;
-}
 }  // namespace lr
-
-extern "C" int lr_probe_fp64_operands(int mode, double* inst_per_s) {
-  if (!inst_per_s || mode < 0 || mode > 3) return LR_EINVAL;
-  int dev = 0, sms = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess) return LR_ECUDA;
-  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return LR_ECUDA;
-  const int iters = 4000;
-  switch (mode) {
-    case 0: return lr::run_operand_probe<0>(sms, iters, inst_per_s);
-    case 1: return lr::run_operand_probe<1>(sms, iters, inst_per_s);
-    case 2: return lr::run_operand_probe<2>(sms, iters, inst_per_s);
-    default: return lr::run_operand_probe<3>(sms, iters, inst_per_s);
-  }
-}
 
 extern "C" int lr_measure_fp64_peak(double seconds, double* inst_per_s) {
   if (!inst_per_s || !(seconds > 0) || seconds > 30) return LR_EINVAL;

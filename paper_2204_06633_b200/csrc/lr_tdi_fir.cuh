@@ -246,7 +246,7 @@ LR_HD void fir_apply(const double* dif, int W, const double* K, int Wc, int pad,
     for (int sl = 0; sl < 4; ++sl) {
       const double* d = dif + ((slots >> (3 * sl)) & 7) * W + (nl0 + i0 - back);
       int koff = (ch * 4 + sl) * Wc * kFirKStride;
-#if defined(__CUDA_ARCH__) && !defined(LR_FIR_NO_PIN)
+#ifdef __CUDA_ARCH__
       asm volatile("" : "+r"(koff));   // keep the tap offset in a register (ptxas otherwise rebuilds it per tap)
 #endif
       const double* kk = K + koff;

@@ -18,7 +18,7 @@ sys.path.insert(0, ROOT)
 sys.path.insert(0, os.path.join(ROOT, "tests"))
 
 from oracle import oracle as orc  # noqa: E402
-from paper_2204_06633_b200 import inputs  # noqa: E402
+from harness import inputs  # noqa: E402
 from parity_util import CH_NAMES, ORC_CH, channel_errors, to_dev  # noqa: E402
 
 

@@ -74,7 +74,8 @@ def test_gb_parameters_host(lib):
 
 
 def test_create_rejects_bad_arguments_without_gpu(lib):
-    from paper_2204_06633_b200 import binding, inputs
+    from harness import inputs
+    from paper_2204_06633_b200 import binding
     tab = inputs.orbit_table("eq", 0.0, 86400.0)
     for order, gen, dt in ((24, 2, 10.0), (0, 2, 10.0), (67, 2, 10.0), (25, 3, 10.0), (25, 2, 0.0)):
         with pytest.raises(binding.LrError) as e:
@@ -91,7 +92,8 @@ def test_no_cpu_fallback_without_device(lib):
     import torch
     if torch.cuda.is_available():
         pytest.skip("a CUDA device is present")
-    from paper_2204_06633_b200 import binding, inputs
+    from harness import inputs
+    from paper_2204_06633_b200 import binding
     tab = inputs.orbit_table("eq", 0.0, 86400.0)
     with pytest.raises(binding.LrError) as e:
         binding.lr_create(tab, 10.0, 25, 2)

@@ -48,14 +48,25 @@ def test_bench_reference_arm():
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
 
 
-@pytest.mark.gpu
-def test_fp64_operand_probe_orders_the_modes():
-    """lr_probe_fp64_operands: a DFMA stream that shares source registers between neighbours issues faster than
-    one that does not (the measurement behind DESIGN.md §6's issue rules), and none exceeds the nominal peak."""
+def test_fp64_operand_probe_orders_the_modes(tmp_path):
+    """tests/probes/dfma_operand_probe.cu (a test-only translation unit, not part of liblr.so): a DFMA stream that
+    shares source registers between neighbours issues faster than one that does not (the measurement behind
+    DESIGN.md §6's issue rules), and none exceeds the nominal peak."""
+    import ctypes
+    import shutil
     import torch
-    import paper_2204_06633_b200 as lr
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    so = str(tmp_path / "dfma_operand_probe.so")
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-shared", "-Xcompiler", "-fPIC",
+                    os.path.join(ROOT, "tests", "probes", "dfma_operand_probe.cu"), "-o", so], check=True)
+    L = ctypes.CDLL(so)
+    L.probe_fp64_operands.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
     sms = torch.cuda.get_device_properties(0).multi_processor_count
-    r = [lr.lr_probe_fp64_operands(m) for m in range(4)]
+    r = []
+    for m in range(4):
+        v = ctypes.c_double()
+        assert L.probe_fp64_operands(m, ctypes.byref(v)) == 0
+        r.append(v.value)
     nominal = sms * 64 * 2.2e9
     assert all(0 < x < nominal for x in r), r
     assert r[2] < 0.9 * r[1] and r[1] <= 1.05 * r[0] and r[3] <= 1.02 * r[1], r

@@ -8,7 +8,7 @@ cases: 1e-10 per channel (parity_util).
 import numpy as np
 import pytest
 
-from paper_2204_06633_b200 import inputs
+from harness import inputs
 from parity_util import windows
 from test_gpu_parity import check_workload, lr  # noqa: F401  (fixture)
 
@@ -32,19 +32,60 @@ def test_full_size_config2_year(lr):  # noqa: F811
     check_workload(lr, w, wins=wins[:3], chain="sum", proj=False)
 
 
-def test_full_size_config3_batch_chunk(lr):  # noqa: F811
-    """configs[2]: one chunk of 16 templates at the full 1,576,800 samples (the chunked launch bench.py
-    uses); the first, the last and one middle template of the chunk are compared on sampled windows."""
-    w = inputs.config(3, batch=16)
-    assert w.n == 1576800
-    wins = _wins(w, lr, 4, seed=33)
-    errs, yh, oh = check_workload(lr, w, idx=tuple(range(16)), wins=wins[:1], proj=True)
-    # templates differ: no two outputs may coincide (batch indexing)
-    assert not np.array_equal(oh[0], oh[15])
-    del errs, yh, oh
+BENCH_CHUNK = 64   # bench.py's --chunk default: templates per launch of the batch leg
+
+
+def test_full_size_config3_bench_launch_shape(lr):  # noqa: F811
+    """configs[2] at the launch shape bench.py times: chunks of 64 templates x 1,576,800 samples (12,319 projection
+    tiles x 64 = 788,416 CTAs, 4.8 GB of y per launch), A,E,T.  Compared with the oracle on sampled windows of
+    template 0, template 1023 and six seeded picks across the 1,024 ("the first, the last and 6
+    seeded picks"); only the chunks that hold a pick are generated and run.  The inputs are made on the device by
+    the harness generator bench.py uses, and the oracle reads those same arrays."""
+    import bench
+    import torch
+    from oracle import oracle as orc
+    from parity_util import CH_NAMES, LINK_NAMES, ORC_CH, assert_parity
+    assert bench.DEFAULT_CHUNK == BENCH_CHUNK
+    w = inputs.config(3)
+    assert w.n == 1576800 and len(w.sources) == 1024 and w.channels == "AET"
+    n = w.n
+    picks = sorted({0, 1023} | {int(i) for i in np.random.default_rng(633).choice(np.arange(1, 1023), 6, replace=False)})
+    assert len(picks) == 8
+    tab = w.table()
+    R = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="AET")
+    O = orc.Oracle(tab, w.dt, w.t0, w.order)
+    mp, mf, mb = R.margins()
+    assert (mp, mf, mb) == O.margins(2)
+    wins = _wins(w, lr, 3, seed=35)
+    y = torch.empty((BENCH_CHUNK, 6, n), dtype=torch.float64, device="cuda")
+    out = torch.empty((BENCH_CHUNK, 3, n), dtype=torch.float64, device="cuda")
+    seen = {}
+    for lo in sorted({(p // BENCH_CHUNK) * BENCH_CHUNK for p in picks}):
+        src = w.sources[lo:lo + BENCH_CHUNK]
+        hp, hc = inputs.gb_waveform_device(src, n, w.dt, w.t0, "cuda")
+        be, la, ps = ([getattr(s, k) for s in src] for k in ("beta", "lam", "psi"))
+        R.project(hp, hc, be, la, ps, y_out=y)
+        R.tdi(y, out=out)
+        torch.cuda.synchronize()
+        for p in (p for p in picks if lo <= p < lo + BENCH_CHUNK):
+            k = p - lo
+            hpk, hck, yk, ok = (t[k].cpu().numpy() for t in (hp, hc, y, out))
+            assert not yk[:, :mp].any() and not yk[:, n - mp:].any()
+            assert not ok[:, :mf].any() and not ok[:, n - mb:].any()
+            for a, b in wins:
+                yo = O.project(hpk, hck, be[k], la[k], ps[k], lo=a, hi=b)
+                assert_parity(yk[:, a:b], yo[:, a:b], f"batch project template {p} [{a},{b})", LINK_NAMES)
+                oo = O.tdi(yk, 2, nested=True, channels=ORC_CH["AET"], lo=a, hi=b)
+                assert_parity(ok[:, a:b], oo[:, a:b], f"batch tdi template {p} [{a},{b})", CH_NAMES["AET"])
+            seen[p] = ok[:, wins[0][0]:wins[0][1]].copy()
+        del hp, hc
+    # templates differ: no two outputs may coincide (batch indexing across and inside chunks)
+    vals = list(seen.values())
+    assert all(not np.array_equal(vals[i], vals[j]) for i in range(len(vals)) for j in range(i))
 
 
 def test_full_size_config3_sampled_templates(lr):  # noqa: F811
+    """configs[2], three templates in one small launch (host-generated inputs), four windows each."""
     w = inputs.config(3, batch=16)
     wins = _wins(w, lr, 4, seed=34)
     w.sources = [w.sources[i] for i in (0, 7, 15)]

@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 
 from oracle import oracle as orc
-from paper_2204_06633_b200 import inputs
+from harness import inputs
 from parity_util import (CH_NAMES, LINK_NAMES, ORC_CH, assert_parity, to_dev, windows)
 
 pytestmark = pytest.mark.gpu
@@ -103,24 +103,30 @@ def test_config1_tiny_fixed_point_ltt(lr):
                                proj=(path == "per_sample"))
 
 
-def test_tdi_null_channel_absolute(lr):
-    """The same equal-arm case with A, E, T: the error of the null channel T is bounded relative to max|A|
-    (1e-10 of the live channels), for every path."""
+@pytest.mark.parametrize("ltt", ["fixed_point", "constant"])
+def test_tdi_null_channel_strict(lr, ltt):
+    """The same equal-arm cases with A, E, T.  T is a null channel here (|T| = 2.5e-5 |A|), the hardest per-call
+    case of the repository: the STRICT bar (1e-10 relative to T itself, rel-L2 and max-abs) holds on every lr_tdi
+    path, both generations and both chain forms (measured round 2: worst 2.6e-11 rel-L2 / 8.4e-11 max-abs, TDI-2,
+    eq. 20 sums, per-sample path), and is asserted for all of them."""
     w = inputs.config(1)
-    tab = inputs.orbit_table("eq", w.t0, w.t0 + w.n * w.dt)
+    tab = inputs.orbit_table("eq", w.t0, w.t0 + w.n * w.dt) if ltt == "fixed_point" else w.table()
     O = orc.Oracle(tab, w.dt, w.t0, w.order)
     s = w.sources[0]
     hp, hc = w.waveform(0)
-    for path in ("per_sample", "fir3", "fir4"):
-        R = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="AET", tdi_path=path)
-        mp, mf, mb = R.margins()
-        y = R.project(to_dev(hp)[None], to_dev(hc)[None], [s.beta], [s.lam], [s.psi])
-        out = R.tdi(y).cpu().numpy()[0]
-        oo = O.tdi(y.cpu().numpy()[0], 2, nested=True, channels=orc.CH_AET)
-        v = slice(mf, w.n - mb)
-        assert_parity(out[:2, v], oo[:2, v], f"equal-arm A,E ({path})", ["A", "E"])
-        scale = float(np.abs(oo[0, v]).max())
-        assert float(np.abs(out[2, v] - oo[2, v].astype(np.float64)).max()) <= 1e-10 * scale
+    for gen in (1, 2):
+        for chain in ("nested", "sum"):
+            oo = None
+            for path in ("auto", "per_sample", "fir3", "fir4"):
+                R = lr.Response(tab, w.dt, w.order, gen, t0=w.t0, channels="AET", tdi_path=path, chain=chain)
+                mp, mf, mb = R.margins()
+                y = R.project(to_dev(hp)[None], to_dev(hc)[None], [s.beta], [s.lam], [s.psi])
+                out = R.tdi(y).cpu().numpy()[0]
+                if oo is None:   # (the projection does not depend on the TDI path: one oracle run per case)
+                    oo = O.tdi(y.cpu().numpy()[0], gen, nested=(chain == "nested"), channels=orc.CH_AET)
+                v = slice(mf, w.n - mb)
+                assert np.abs(oo[2, v]).max() < 1e-4 * np.abs(oo[0, v]).max()      # T really is the null channel
+                assert_parity(out[:, v], oo[:, v], f"equal-arm {ltt} gen{gen} {chain} ({path})", ["A", "E", "T"])
 
 
 def test_tdi_delay_crossing_whole_sample(lr):
@@ -586,6 +592,117 @@ def test_tdi_plan_cache(lr):
     assert np.array_equal(both[1:], fresh(yb, 5000, w.t0 + 12345.0, "nested"))
 
 
+def test_plan_rebuilt_once_per_call_with_flagged_tiles(lr):
+    """LR_OPT_TDI_PLAN_CACHE = 0 with more than 8 templates (two template chunks, several time chunks) and tiles the
+    plan flags: the plan is rebuilt once per call, behind every fix-up kernel that still reads the old list, and the
+    result equals the cached-plan two-call path bit for bit (the rebuild used to race with the deferred
+    fix-up kernel of the previous chunk)."""
+    import torch
+    dt, n, t0, order = 10.0, 40000, 3.0e7, 9
+    base = inputs.orbit_table("kepler", t0, t0 + n * dt)
+    tk = base.t_start + base.knot_dt * np.arange(base.n_knots)
+    ltt = np.tile(10.0 + 2e-9 * (tk - (t0 + 0.5 * n * dt)), (6, 1)) * (1 + 1e-7 * np.arange(6))[:, None]
+    tab = inputs.OrbitTable(base.t_start, base.knot_dt, base.x, np.ascontiguousarray(ltt))
+    w = inputs.config(3, batch=11, n=n, t0=t0)
+    hp, hc = _stack(w, range(11))
+    hpd, hcd = to_dev(hp), to_dev(hc)
+    beta, lam, psi = ([getattr(s, k) for s in w.sources] for k in ("beta", "lam", "psi"))
+    R = lr.Response(tab, dt, order, 2, t0=t0, tdi_path="fir3")
+    ref = R.tdi(R.project(hpd, hcd, beta, lam, psi)).cpu().numpy()
+    Rn = lr.Response(tab, dt, order, 2, t0=t0, tdi_path="fir3")
+    Rn.set_plan_cache(False)
+    lr.lr_set_option(Rn.handle, lr.LR_OPT_CHUNK_SAMPLES, 1792 * 3)
+    for _ in range(4):
+        l0 = lr.lr_launch_count()
+        got = Rn.response(hpd, hcd, beta, lam, psi)
+        torch.cuda.synchronize()
+        assert np.array_equal(got.cpu().numpy(), ref)
+        chunks = 2 * -(-n // (1792 * 3))
+        # source basis x2, ONE plan kernel, per chunk: projection + apply (+ fix-up where a flagged tile lies)
+        assert 2 + 1 + 2 * chunks <= lr.lr_launch_count() - l0 <= 2 + 1 + 3 * chunks
+    assert np.array_equal(Rn.tdi(R.project(hpd, hcd, beta, lam, psi)).cpu().numpy(), ref)
+
+
+def test_shared_plan_two_streams_bitwise(lr):
+    """lr_plan_create / lr_plan_attach (orbit information pre-computed once for the whole run): two
+    handles on two streams share ONE read-only plan; results equal a handle's own plan bit for bit; no plan kernel
+    runs in the attached handles; the plan outlives the handle that built it; a call on another grid falls back to
+    the handle's own plan; a plan of other orbits is refused."""
+    import torch
+    w = inputs.config(2, n=60011, f0=3e-3, t0=3.0e7)
+    tab = w.table()
+    s = w.sources[0]
+    hp, hc = w.waveform(0)
+    mk = lambda: lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="XYZ_AET")
+    Ra = mk()
+    y1 = Ra.project(to_dev(hp)[None], to_dev(hc)[None], [s.beta], [s.lam], [s.psi])
+    y2 = (y1 * 0.5).contiguous()
+    ref1, ref2 = Ra.tdi(y1).cpu().numpy(), Ra.tdi(y2).cpu().numpy()
+    plan = lr.lr_plan_create(Ra.handle, w.n)
+    assert lr.lr_plan_bytes(plan) > 12 * 31 * 3 * 8 * (w.n // 224)
+    Ra.close()                                     # the creator goes, the plan stays
+    Rc, Rd = mk(), mk()
+    lr.lr_plan_attach(Rc.handle, plan)
+    lr.lr_plan_attach(Rd.handle, plan)
+    lr.lr_plan_release(plan)                       # the attached handles hold the remaining references
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    s1.wait_stream(torch.cuda.current_stream())
+    s2.wait_stream(torch.cuda.current_stream())
+    l0 = lr.lr_launch_count()
+    for _ in range(3):
+        o1 = Rc.tdi(y1, stream=s1)
+        o2 = Rd.tdi(y2, stream=s2)
+    s1.synchronize()
+    s2.synchronize()
+    assert lr.lr_launch_count() - l0 <= 6 * 2      # apply (+ fix-up) per call: no plan kernel
+    assert np.array_equal(o1.cpu().numpy(), ref1) and np.array_equal(o2.cpu().numpy(), ref2)
+    # another grid: the attached plan does not fit, the handle builds its own
+    m = 30011
+    Re = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="XYZ_AET")
+    short = y1[:, :, :m].contiguous()
+    assert np.array_equal(Rc.tdi(short).cpu().numpy(), Re.tdi(short).cpu().numpy())
+    assert np.array_equal(Rc.tdi(y1).cpu().numpy(), ref1)          # and the shared one still serves its grid
+    # other orbits / other order: refused
+    other = lr.Response(inputs.orbit_table("eq", w.t0, w.t0 + w.n * w.dt), w.dt, w.order, 2, t0=w.t0)
+    p2 = lr.lr_plan_create(Rc.handle, w.n)
+    with pytest.raises(lr.LrError) as e:
+        lr.lr_plan_attach(other.handle, p2)
+    assert e.value.code == lr.LR_EINVAL
+    lr.lr_plan_attach(Rc.handle, None)
+    lr.lr_plan_release(p2)
+    Rp = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, tdi_path="per_sample")
+    with pytest.raises(lr.LrError):
+        lr.lr_plan_create(Rp.handle, w.n)
+
+
+def test_binding_checks_out_against_the_channel_option(lr):
+    """The C ABI takes no size for `out`: the binding checks it against the handle's LR_OPT_CHANNELS (lr_get_option),
+    so a [B,3,N] buffer is never handed to a handle that writes six rows; angle arrays must match the batch."""
+    import torch
+    w = inputs.config(2, n=4001, t0=2.0e7)
+    s = w.sources[0]
+    hp, hc = w.waveform(0)
+    R = lr.Response(w.table(), w.dt, w.order, 2, t0=w.t0, channels="XYZ_AET")
+    assert lr.lr_get_option(R.handle, lr.LR_OPT_CHANNELS) == lr.LR_XYZ_AET
+    assert lr.lr_get_option(R.handle, lr.LR_OPT_T0) == w.t0
+    hpd, hcd = to_dev(hp)[None], to_dev(hc)[None]
+    y = R.project(hpd, hcd, [s.beta], [s.lam], [s.psi])
+    small = torch.empty((1, 3, w.n), dtype=torch.float64, device="cuda")
+    with pytest.raises(ValueError):
+        R.tdi(y, out=small)
+    with pytest.raises(ValueError):
+        R.response(hpd, hcd, [s.beta], [s.lam], [s.psi], out=small)
+    with pytest.raises(ValueError):
+        R.response_host(hp[None].copy(), hc[None].copy(), [s.beta], [s.lam], [s.psi], np.empty((1, 3, w.n)))
+    with pytest.raises(ValueError):
+        R.response(hpd, hcd, [s.beta], [s.lam, s.lam], [s.psi])
+    R3 = lr.Response(w.table(), w.dt, w.order, 2, t0=w.t0, channels="AET")
+    with pytest.raises(ValueError):
+        R3.tdi(y, out=torch.empty((1, 6, w.n), dtype=torch.float64, device="cuda"))
+    with pytest.raises(lr.LrError):
+        lr.lr_get_option(R.handle, 99)
+
+
 # ------------------------------------------------------------------------------- likelihood (NEXT-2)
 def test_gpu_inner_product_parity(lr):
     """lr_inner_product against the likelihood oracle on the SAME frequency-domain arrays (numpy FFT of real
@@ -666,8 +783,7 @@ def test_edge_cases_and_errors(lr):
     out = R.tdi(to_dev(yy)[None]).cpu().numpy()[0]
     oo = O.tdi(yy, 1)
     assert np.count_nonzero(out) == 3
-    # (white-noise y: the interpolation is the same linear map on both sides)
-    assert_parity(out[:, mf:mf + 1], oo[:, mf:mf + 1], "single valid tdi sample", rel_tol=1e-9, abs_tol=1e-9)
+    assert_parity(out[:, mf:mf + 1], oo[:, mf:mf + 1], "single valid tdi sample")
     with pytest.raises(lr.LrError) as e:
         R.tdi(to_dev(yy[:, :-1])[None])
     assert e.value.code == lr.LR_EINVAL

@@ -7,7 +7,7 @@ import pytest
 
 from oracle import oracle as orc
 from oracle import waveform as owf
-from paper_2204_06633_b200 import inputs
+from harness import inputs
 from parity_util import CH_NAMES, ORC_CH, assert_parity, to_dev
 
 pytestmark = pytest.mark.gpu

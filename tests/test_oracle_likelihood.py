@@ -3,7 +3,7 @@ fixes — none of them re-types the oracle's formula."""
 import numpy as np
 
 from oracle import likelihood as lk
-from paper_2204_06633_b200 import inputs
+from harness import inputs
 
 LD = np.longdouble
 

@@ -6,6 +6,7 @@ library routines (scipy CubicSpline / BarycentricInterpolator), continuous-time 
 with mpmath, and printed worked-example values (tests/golden/worked_example_p2.json).
 """
 import json
+import math
 import os
 
 import mpmath as mp
@@ -14,7 +15,7 @@ import pytest
 from scipy.interpolate import BarycentricInterpolator, CubicSpline
 
 from oracle import oracle as O
-from paper_2204_06633_b200 import inputs as I
+from harness import inputs as I
 
 LD = np.longdouble
 C = I.C_LIGHT
@@ -511,3 +512,27 @@ def test_margins_cover_every_stencil():
         nl = 3 if w.tdi_gen == 1 else 7
         assert mf >= mpj + int(np.ceil(nl * l_max / w.dt)) + p     # TDI reads only valid y
         assert mb >= mpj + p
+
+
+def test_margins_are_reading_a8():
+    """Reading A8 itself (the paper is silent on edges): from the TABLE maxima
+    R_max = max |x_i| and L_max = max L_ij over the knots,
+        M_proj = ceil((1.001 R_max/c + 1.001 L_max)/dt) + p + 2,
+        M_front = M_proj + ceil(G 1.001 L_max/dt) + p + 2 (G = 4 | 8),  M_back = M_proj + p + 2,
+    so a joint drift of the 1.001 factors or of the `+ p + 2` on both sides (oracle and library assert equality with
+    each other on the GPU) cannot go unnoticed.  The survey prints M_proj = 67 for Keplerian orbits at dt = 10 s,
+    order 25 (R_max/c = 501.4 s, L_max = 8.34 s)."""
+    for cfg, kw in ((1, {}), (2, {"n": 4000}), (3, {"n": 4000, "batch": 1}), (4, {"n": 4000}), (5, {"n": 4000})):
+        w = I.config(cfg, **kw)
+        tb = w.table()
+        orc = O.Oracle(tb, w.dt, w.t0, w.order)
+        p = (w.order + 1) // 2
+        x = np.asarray(tb.x, dtype=np.float64).reshape(3, 3, -1)
+        r_max = float(np.sqrt((x ** 2).sum(axis=1)).max())
+        l_max = float(np.asarray(tb.ltt).max())
+        m_proj = math.ceil((1.001 * r_max / C + 1.001 * l_max) / w.dt) + p + 2
+        for gen, G in ((1, 4), (2, 8)):
+            want = (m_proj, m_proj + math.ceil(G * 1.001 * l_max / w.dt) + p + 2, m_proj + p + 2)
+            assert orc.margins(gen) == want, (cfg, gen)
+    w = I.config(2)     # the whole year of knots: R_max reaches the aphelion
+    assert O.Oracle(w.table(), w.dt, w.t0, w.order).margins(2)[0] == 67
