@@ -63,6 +63,19 @@ typedef struct {
 #define LR_OPT_CHUNK_SAMPLES 7 /* time-chunk length of lr_response / lr_response_host (rounded up to 1792); 0 = automatic */
 #define LR_OPT_FFT_LENGTH 8 /* transform length of lr_loglike_gb (>= n, zero padded); 0 (default) = n */
 #define LR_OPT_TDI_PLAN_CACHE 6 /* 1 (default): keep the FIR plan between lr_tdi calls; 0: rebuild every call */
+#define LR_OPT_PROJ_PATH 9 /* LR_PROJ_AUTO (default) | LR_PROJ_SINGLE | LR_PROJ_PAIR */
+
+/* How lr_project maps time samples to threads (the results are the same bit for bit).
+ *   LR_PROJ_SINGLE : one sample per thread.
+ *   LR_PROJ_PAIR   : two consecutive samples per thread; the two Lagrange stencils of every interpolation time share
+ *                    all but one of their first differences, which are then read from shared memory once (half the
+ *                    shared-memory traffic; orders with a compile-time kernel, any other order runs LR_PROJ_SINGLE).
+ *                    Measured on B200 it is 5-7 % slower than LR_PROJ_SINGLE at order 25 (166 registers per thread
+ *                    leave 11 warps per SM against 16), so it is not the default.
+ *   LR_PROJ_AUTO   : the faster of the two on B200 (LR_PROJ_SINGLE). */
+#define LR_PROJ_AUTO (-1)
+#define LR_PROJ_SINGLE 1
+#define LR_PROJ_PAIR 2
 
 /* How lr_tdi evaluates the Lagrange weights (same result to rounding).
  *   LR_TDI_PER_SAMPLE : every delayed term gets its own weight set at every sample.

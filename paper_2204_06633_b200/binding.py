@@ -20,6 +20,8 @@ LR_OPT_T0, LR_OPT_CHAIN, LR_OPT_CHANNELS, LR_OPT_TDI_GEN, LR_OPT_TDI_PATH = 1, 2
 LR_OPT_TDI_PLAN_CACHE = 6
 LR_OPT_CHUNK_SAMPLES = 7
 LR_OPT_FFT_LENGTH = 8
+LR_OPT_PROJ_PATH = 9
+LR_PROJ_AUTO, LR_PROJ_SINGLE, LR_PROJ_PAIR = -1, 1, 2
 LR_IP_CROSS, LR_IP_DIFF, LR_IP_BLOCKS = 0, 1, 1024
 LR_GB_NPAR = 6
 LR_GB_PAPER, LR_GB_CONFIG = 0, 1

@@ -83,6 +83,7 @@ struct lr_handle {
   bool const_ltt = false; // every light-time table is constant: lr_tdi's plan is one tile (NEXT-4)
   int tdi_path = -1;     // LR_OPT_TDI_PATH: -1 auto | 0 generic | 3 | 4
   int plan_cache = 1;    // LR_OPT_TDI_PLAN_CACHE
+  int proj_path = LR_PROJ_AUTO;   // LR_OPT_PROJ_PATH
   int sm_count = 0;
   int64_t chunk_samples = 0;   // LR_OPT_CHUNK_SAMPLES: 0 = automatic
   int64_t fft_length = 0;      // LR_OPT_FFT_LENGTH: 0 = n (no zero padding)
@@ -153,6 +154,7 @@ lr::Params make_params(const lr_handle* h, int64_t n) {
   P.m_front = (int)h->m_front(h->gen);
   P.m_back = (int)h->m_back();
   P.chain_sum = h->chain == LR_CHAIN_SUM ? 1 : 0;
+  P.proj_pair = h->proj_path == LR_PROJ_PAIR ? 1 : 0;   // LR_PROJ_AUTO: one sample per thread (the faster one)
   memcpy(P.bk, h->bk, sizeof(P.bk));
   return P;
 }
@@ -354,6 +356,9 @@ int lr_set_option(lr_handle* h, int key, double value) {
       if (value != LR_TDI_AUTO && value != LR_TDI_PER_SAMPLE && value != LR_TDI_FIR3 && value != LR_TDI_FIR4)
         return LR_EINVAL;
       h->tdi_path = (int)value; return LR_OK;
+    case LR_OPT_PROJ_PATH:
+      if (value != LR_PROJ_AUTO && value != LR_PROJ_SINGLE && value != LR_PROJ_PAIR) return LR_EINVAL;
+      h->proj_path = (int)value; return LR_OK;
     case LR_OPT_CHUNK_SAMPLES:
       if (value < 0 || value > 2147483647.0 || value != floor(value)) return LR_EINVAL;
       h->chunk_samples = (int64_t)value; return LR_OK;
@@ -375,6 +380,7 @@ int lr_get_option(const lr_handle* h, int key, double* value) {
     case LR_OPT_CHANNELS: *value = h->channels; return LR_OK;
     case LR_OPT_TDI_GEN: *value = h->gen; return LR_OK;
     case LR_OPT_TDI_PATH: *value = h->tdi_path; return LR_OK;
+    case LR_OPT_PROJ_PATH: *value = h->proj_path; return LR_OK;
     case LR_OPT_CHUNK_SAMPLES: *value = (double)h->chunk_samples; return LR_OK;
     case LR_OPT_FFT_LENGTH: *value = (double)h->fft_length; return LR_OK;
     case LR_OPT_TDI_PLAN_CACHE: *value = h->plan_cache; return LR_OK;

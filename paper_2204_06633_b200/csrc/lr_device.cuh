@@ -70,6 +70,7 @@ struct Params {
   int fir_tile0;         // FIR path: global tile whose geometry plan slot 0 is built from
   int fir_taps;          // FIR path: taps per series that can be non-zero (<= fir_wc; the padding is at the front)
   int chain_sum;         // 0: nested delays (default), 1: eq. 20 sums of the L at t
+  int proj_pair;         // 1: projection with two consecutive samples per thread (LR_PROJ_PAIR; same bits)
   double bk[kPMax + 1];  // bk[k] = 1 / prod_{m != k} (k - m), m = -P+1..P, for k = 1..P
 };
 
@@ -172,7 +173,112 @@ LR_HD void interp_sbp(const Params& prm, double eps, int a, Dif dif, double (&S)
   for (int s = 0; s < NS; ++s) S[s] = lo[s] - hi[s];
 }
 
+// The same for TWO consecutive samples A (anchor a) and B (anchor a + 1) whose targets eps_A, eps_B differ: the two
+// stencils overlap in 2P - 2 of their 2P - 1 first differences, so every difference is fetched ONCE (2P fetches
+// for the pair instead of 2 (2P - 1)) and used with both weight sets.  Iteration k fetches dif[q+1-k] and dif[q+k],
+// q = a - 1: sample A uses them for its low step k and its high step k+1, sample B for its low step k+1 and its
+// high step k (B's low step 1 reuses the upper fetch of iteration 1).  Every accumulator receives exactly the
+// operations of interp_sbp in the same order, so the results equal two interp_sbp calls bit for bit.
+// Compile-time P only.  win(c, out) fetches the NS first differences at index q + c, q = a - 1 (c is a compile-time
+// constant after unrolling: the caller can lay the window out so that c becomes an immediate offset).
+template <int PT, int NS, class Win>
+LR_HD void interp_sbp2(const Params& prm, double epsA, double epsB, Win win, double (&SA)[NS], double (&SB)[NS]) {
+  static_assert(PT > 0, "interp_sbp2 needs a compile-time pair count");
+  constexpr int P = PT;
+  double RA[P], RB[P];
+  const double zA = fma(epsA, epsA, -epsA), zB = fma(epsB, epsB, -epsB);
+  double preA = 1.0, preB = 1.0;
+#pragma unroll
+  for (int k = 1; k <= P; ++k) {
+    RA[k - 1] = preA * prm.bk[k];
+    preA *= zA - (double)(k * (k - 1));
+    RB[k - 1] = preB * prm.bk[k];
+    preB *= zB - (double)(k * (k - 1));
+  }
+  double sufA = 1.0, CA = 0.0, EA = 0.0, sufB = 1.0, CB = 0.0, EB = 0.0;
+  double loA[NS], hiA[NS], loB[NS], hiB[NS];
+#pragma unroll
+  for (int s = 0; s < NS; ++s) { loA[s] = 0.0; hiA[s] = 0.0; loB[s] = 0.0; hiB[s] = 0.0; }
+#pragma unroll
+  for (int k = P; k >= 1; --k) {
+    double dL[NS], dH[NS];
+    win(1 - k, dL);
+    win(k, dH);
+    // sample A: low step k; high step k+1 with the E of the previous iteration
+    const double RkA = RA[k - 1] * sufA;
+    sufA *= zA - (double)(k * (k - 1));
+    CA = fma(RkA, (double)k - epsA, CA);
+#pragma unroll
+    for (int s = 0; s < NS; ++s) loA[s] = fma(CA, dL[s], loA[s]);
+    if (k < P) {
+#pragma unroll
+      for (int s = 0; s < NS; ++s) hiA[s] = fma(EA, dH[s], hiA[s]);
+    }
+    if (k >= 2) EA = fma(RkA, epsA + (double)(k - 1), EA);
+    // sample B (anchor a + 1): low step k+1 with the C of the previous iteration; high step k
+    if (k < P) {
+#pragma unroll
+      for (int s = 0; s < NS; ++s) loB[s] = fma(CB, dL[s], loB[s]);
+    }
+    const double RkB = RB[k - 1] * sufB;
+    sufB *= zB - (double)(k * (k - 1));
+    CB = fma(RkB, (double)k - epsB, CB);
+    if (k >= 2) {
+      EB = fma(RkB, epsB + (double)(k - 1), EB);
+#pragma unroll
+      for (int s = 0; s < NS; ++s) hiB[s] = fma(EB, dH[s], hiB[s]);
+    } else {
+#pragma unroll
+      for (int s = 0; s < NS; ++s) loB[s] = fma(CB, dH[s], loB[s]);   // B's low step 1: dif[q + 1]
+    }
+  }
+#pragma unroll
+  for (int s = 0; s < NS; ++s) { SA[s] = loA[s] - hiA[s]; SB[s] = loB[s] - hiB[s]; }
+}
+
 // ---------------------------------------------------------------------------------------------- stage 1
+// Geometry of one time sample (eqs. 10-12 and the reception delays of eq. 16): everything that needs the positions
+// and the basis, so that only 15 doubles per sample stay live across the nine interpolations.
+struct ProjGeom {
+  double Dr[3];                          // reception delay k.x_i/c [samples]
+  double xip[3], xic[3], kn[3], rden[3]; // per arm (links 12, 23, 31 and their reverses): xi+, xix, k.n, 1/(2(1-k.n)(1+k.n))
+};
+
+template <class Coef>
+LR_HD void project_geometry(const Params& prm, const Coef& coef, double trel, const double* bs, ProjGeom& g) {
+  const double k0 = bs[0], k1 = bs[1], k2 = bs[2];
+  const double u0 = bs[3], u1 = bs[4], u2 = bs[5];
+  const double v0 = bs[6], v1 = bs[7], v2 = bs[8];
+  double x[3][3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) x[i][a] = spline_eval(prm, coef, i * 3 + a, trel);
+    g.Dr[i] = (k0 * x[i][0] + k1 * x[i][1] + k2 * x[i][2]) * prm.inv_cdt;   // reception delay k.x_i/c [samples]
+  }
+  // three arms: arm a joins receiver i = a and emitter j = (a+1)%3 (links 12, 23, 31); the reverse links
+  // 21, 32, 13 share xi+ and xix and flip the sign of k.n
+#pragma unroll
+  for (int arm = 0; arm < 3; ++arm) {
+    const int i = arm, j = (arm + 1) % 3;
+    const double d0 = x[i][0] - x[j][0], d1 = x[i][1] - x[j][1], d2 = x[i][2] - x[j][2];
+    const double inv = inv_sqrt(d0 * d0 + d1 * d1 + d2 * d2);
+    const double n0v = d0 * inv, n1v = d1 * inv, n2v = d2 * inv;  // emitter j -> receiver i
+    const double un = u0 * n0v + u1 * n1v + u2 * n2v;
+    const double vn = v0 * n0v + v1 * n1v + v2 * n2v;
+    g.kn[arm] = k0 * n0v + k1 * n1v + k2 * n2v;
+    // eq. 16 divides by 2 (1 - k.n) on one link of the arm and by 2 (1 + k.n) on the other: one reciprocal,
+    // 1 / (2 (1 - k.n)(1 + k.n)), computed here, serves both (an fp64 division is ~25 instructions and a branch;
+    // six of them at the end of the links' dependency chains, plus 1/sqrt as two operations, were 8 % of the
+    // kernel)
+    g.rden[arm] = 1.0 / (2.0 * ((1.0 - g.kn[arm]) * (1.0 + g.kn[arm])));
+    g.xip[arm] = un * un - vn * vn;   // eq. 12
+    g.xic[arm] = 2.0 * un * vn;
+  }
+}
+
+LR_HD int clamp_anchor(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
 // One time sample of eqs. 10-16 for all six links.  raw/dif: staged (h+, hx) pairs and their first
 // differences, W entries; nl = this sample's staged index; bs = k(3), u(3), v(3).  y6[slot] receives y_ij.
 template <int PT, class Store, class Coef = CoefGlobal>
@@ -253,6 +359,150 @@ LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W
     }
   }
 }
+
+// Two consecutive samples per thread (staged indices nl = A and nl + 1 = B).  Each of the nine interpolation times of
+// B lies ~1e-4 samples from A's shifted by one sample (|d/dt (k.x/c)| <= 1e-4, |dL/dt| <= 1e-7), so the stencils of a
+// pair share all but one first difference and interp_sbp2 fetches each from shared memory once.  Where the integer
+// parts of the two delays differ (the fraction wrapped between A and B: about one pair in 1e4) the pair takes two
+// single-sample interpolations (out of line: it is rare and would triple the code).  Results equal project_sample's
+// bit for bit.
+//
+// To keep the register count of the pair near that of a single sample, the thread first writes the geometry of both
+// samples (project_geometry's 15 numbers, the six emission delays and the six link factors (1 +- k.n) / (2 (1 -
+// k.n)(1 + k.n))) to a private column of shared memory, geo[kGeoFields][nthreads], and then walks the three RECEIVERS
+// in a rolled loop: reception at i, then the two links received at i.
+constexpr int kGeoDr = 0, kGeoDe = 3, kGeoXip = 9, kGeoXic = 12, kGeoF = 15, kGeoPerSample = 21;
+constexpr int kGeoFields = 2 * kGeoPerSample;
+
+template <class Coef>
+LR_HD void project_geometry_store(const Params& prm, const Coef& coef, double trel, const double* bs, double* geo,
+                                  int stride) {
+  ProjGeom g;
+  project_geometry(prm, coef, trel, bs, g);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    geo[(kGeoDr + i) * stride] = g.Dr[i];
+    geo[(kGeoXip + i) * stride] = g.xip[i];
+    geo[(kGeoXic + i) * stride] = g.xic[i];
+  }
+#pragma unroll
+  for (int arm = 0; arm < 3; ++arm) {
+    const int i = arm, j = (arm + 1) % 3;
+#pragma unroll
+    for (int dir = 0; dir < 2; ++dir) {
+      const int rx = dir == 0 ? i : j, tx = dir == 0 ? j : i;
+      const int slot = link_slot(rx, tx);
+      const double kappa = dir == 0 ? g.kn[arm] : -g.kn[arm];
+      // emission: t - L_rx,tx(t) - k.x_tx(t)/c
+      geo[(kGeoDe + slot) * stride] = fma(spline_eval(prm, coef, 9 + slot, trel), prm.inv_dt, g.Dr[tx]);
+      geo[(kGeoF + slot) * stride] = (1.0 + kappa) * g.rden[arm];   // eq. 16: 1 / (2 (1 - kappa))
+    }
+  }
+}
+
+#ifdef __CUDACC__
+// interp_sbp<PT, 2> on the staged (h+, hx) differences as an out-of-line call with rolled loops (the rare path of
+// project_pair; bk: the pair constants in shared memory, so that no kernel parameter has its address taken).  Same
+// operations in the same order as interp_sbp, hence the same bits.
+template <int PT>
+__device__ __noinline__ void interp_sbp_rolled(const double* bk, double eps, int a, const D2* dif_e, const D2* dif_o,
+                                               double* S) {
+  auto dif_at = [&](int m) { return (m & 1) ? dif_o[m >> 1] : dif_e[m >> 1]; };
+  double R[PT];
+  const double z = fma(eps, eps, -eps);
+  double pre = 1.0;
+#pragma unroll 1
+  for (int k = 1; k <= PT; ++k) {
+    R[k - 1] = pre * bk[k];
+    pre *= z - (double)(k * (k - 1));
+  }
+  double suf = 1.0, C = 0.0, E = 0.0, lo0 = 0.0, lo1 = 0.0, hi0 = 0.0, hi1 = 0.0;
+  const int q = a - 1;
+#pragma unroll 1
+  for (int k = PT; k >= 1; --k) {
+    const double Rk = R[k - 1] * suf;
+    suf *= z - (double)(k * (k - 1));
+    C = fma(Rk, (double)k - eps, C);
+    const D2 d = dif_at(q + 1 - k);
+    lo0 = fma(C, d.x, lo0);
+    lo1 = fma(C, d.y, lo1);
+    if (k >= 2) {
+      E = fma(Rk, eps + (double)(k - 1), E);
+      const D2 e = dif_at(q + k - 1);
+      hi0 = fma(E, e.x, hi0);
+      hi1 = fma(E, e.y, hi1);
+    }
+  }
+  S[0] = lo0 - hi0;
+  S[1] = lo1 - hi1;
+}
+
+// geo: this thread's column (element f of sample A at geo[f * stride], of sample B at geo[(kGeoPerSample + f) * stride]).
+// The first differences are staged DE-INTERLEAVED, dif_e[i] = dif[2 i], dif_o[i] = dif[2 i + 1]: the lanes of a warp
+// own every other sample, so with the plain layout their 16-byte reads of one tap would be 32 bytes apart (a two-way
+// bank conflict on every load: measured, 52.7 M conflicts in one year); de-interleaved, the lanes read consecutive
+// elements.  For a window anchored at q the tap q + c lies at (c even ? pe : po)[c >> 1] with two base pointers chosen
+// by the parity of q, so every tap is still an immediate offset.
+// bk_s: prm.bk in shared memory.  store(slot, yA, yB).
+template <int PT, class Store>
+__device__ __forceinline__ void project_pair(const Params& prm, const D2* raw, const D2* dif_e, const D2* dif_o, int W,
+                                             int nl, const double* geo, int stride, const double* bk_s, Store store) {
+  constexpr int a_min = PT;
+  const int a_max = W - PT;
+  auto interp2 = [&](double DA, double DB, int& aA, int& aB, double (&SA)[2], double (&SB)[2]) {
+    double eA, eB;
+    split_delay(DA, nl, aA, eA);
+    split_delay(DB, nl + 1, aB, eB);
+    aA = clamp_anchor(aA, a_min, a_max);
+    aB = clamp_anchor(aB, a_min, a_max);
+    if (aB == aA + 1) {
+      const int q = aA - 1, q2 = q >> 1;
+      const D2* pe = (q & 1) ? dif_o + q2 : dif_e + q2;        // taps q + c, c even
+      const D2* po = (q & 1) ? dif_e + q2 + 1 : dif_o + q2;    // taps q + c, c odd
+      auto win = [&](int c, double (&d)[2]) {
+        const D2 v = (c & 1) ? po[c >> 1] : pe[c >> 1];
+        d[0] = v.x; d[1] = v.y;
+      };
+      interp_sbp2<PT, 2>(prm, eA, eB, win, SA, SB);
+    } else {
+      interp_sbp_rolled<PT>(bk_s, eA, aA, dif_e, dif_o, SA);
+      interp_sbp_rolled<PT>(bk_s, eB, aB, dif_e, dif_o, SB);
+    }
+  };
+  const double* gA = geo;
+  const double* gB = geo + kGeoPerSample * stride;
+#pragma unroll 1
+  for (int i = 0; i < 3; ++i) {   // receiver
+    double SrA[2], SrB[2];
+    int arA, arB;
+    interp2(gA[(kGeoDr + i) * stride], gB[(kGeoDr + i) * stride], arA, arB, SrA, SrB);
+    const D2 rrA = raw[arA], rrB = raw[arB];
+#pragma unroll
+    for (int l = 0; l < 2; ++l) {
+      // the two links received at i: from (i+1)%3 (slot i, arm i) and from (i+2)%3 (the reverse link of arm (i+2)%3)
+      const int slot = l == 0 ? i : (i == 0 ? 3 : i == 1 ? 5 : 4);
+      const int arm = l == 0 ? i : (i == 0 ? 2 : i - 1);
+      int aeA, aeB;
+      double SeA[2], SeB[2];
+      interp2(gA[(kGeoDe + slot) * stride], gB[(kGeoDe + slot) * stride], aeA, aeB, SeA, SeB);
+      double yA, yB;
+      {
+        const D2 re = raw[aeA];
+        const double dhp = (re.x - rrA.x) - SeA[0] + SrA[0];
+        const double dhc = (re.y - rrA.y) - SeA[1] + SrA[1];
+        yA = (gA[(kGeoXip + arm) * stride] * dhp + gA[(kGeoXic + arm) * stride] * dhc) * gA[(kGeoF + slot) * stride];
+      }
+      {
+        const D2 re = raw[aeB];
+        const double dhp = (re.x - rrB.x) - SeB[0] + SrB[0];
+        const double dhc = (re.y - rrB.y) - SeB[1] + SrB[1];
+        yB = (gB[(kGeoXip + arm) * stride] * dhp + gB[(kGeoXic + arm) * stride] * dhc) * gB[(kGeoF + slot) * stride];
+      }
+      store(slot, yA, yB);
+    }
+  }
+}
+#endif
 
 // ---------------------------------------------------------------------------------------------- stage 2
 // X's two delay chains (eqs. 17-18): term k of chain A is + y_{A[k]} delayed by the

@@ -28,6 +28,15 @@ int launch_project_t(const Params& prm, const double* hp, const double* hc, cons
   cudaError_t e = prepare(project_kernel<PT>, smem);
   if (e != cudaSuccess) return (int)e;
   const int64_t grid = (int64_t)prm.ntiles * batch;
+  if constexpr (proj_pairs(PT)) {
+    if (prm.proj_pair) {
+      const size_t smem2 = proj_pair_smem((int)W);
+      if ((e = prepare(project_pair_kernel<PT>, smem2)) != cudaSuccess) return (int)e;
+      project_pair_kernel<PT><<<(unsigned)grid, kProjPairThreads, smem2, (cudaStream_t)stream>>>(prm, hp, hc, basis, y);
+      g_launches.fetch_add(1);
+      return (int)cudaGetLastError();
+    }
+  }
   project_kernel<PT><<<(unsigned)grid, kProjThreads, smem, (cudaStream_t)stream>>>(prm, hp, hc, basis, y);
   g_launches.fetch_add(1);
   return (int)cudaGetLastError();

@@ -16,11 +16,20 @@ namespace lr {
 // Launch shapes, tuned on B200 (profiles/r1_tuning.md): both kernels are bound by the FP64 pipe and want
 // 12-24 resident warps per SM; letting ptxas take 160-250 registers per thread (one CTA per SM) halves the
 // throughput.  The caps below keep the order-25 kernels spill-free.
-constexpr int kProjThreads = 128;
+constexpr int kProjThreads = 128;      // samples per projection tile (and threads of the one-sample-per-thread kernel)
+constexpr int kProjPairThreads = 64;   // threads of the two-samples-per-thread kernel (same 128-sample tile)
 constexpr int kTdiThreads = 256;
 #ifndef LR_PROJ_MINB
 #define LR_PROJ_MINB 4
 #endif
+// elements of each half of the de-interleaved difference window of the pair kernel
+__host__ __device__ constexpr int proj_pair_half(int W) { return (W >> 1) + 1; }
+// dynamic shared memory of project_pair_kernel: raw[W], dif_e[H], dif_o[H] (D2), geo[kGeoFields][threads]
+__host__ __device__ constexpr size_t proj_pair_smem(int W) {
+  return (size_t)(W + 2 * proj_pair_half(W)) * sizeof(D2) + (size_t)kGeoFields * kProjPairThreads * sizeof(double);
+}
+// orders whose projection runs two samples per thread (compile-time P; the run-time-P build keeps one)
+__host__ __device__ constexpr bool proj_pairs(int PT) { return PT >= 1; }
 __host__ __device__ constexpr int proj_min_blocks(int PT) { return PT == 0 ? 2 : PT <= 13 ? LR_PROJ_MINB : 3; }
 __host__ __device__ constexpr int tdi_min_blocks(int PT) { return PT == 0 ? 2 : PT <= 13 ? 3 : 2; }
 
@@ -87,6 +96,90 @@ project_kernel(const Params prm, const double* __restrict__ hp, const double* __
     project_sample<PT>(prm, raw, dif, W, n - g0, sample_trel(prm, ng), bs, store, CoefTile{sc, i_lo});
   else
     project_sample<PT>(prm, raw, dif, W, n - g0, sample_trel(prm, ng), bs, store, CoefGlobal{});
+}
+
+// Two consecutive samples per thread (project_pair): the same tile, staging and results as project_kernel with half
+// the threads; every first difference a pair of stencils shares is read from shared memory once.
+#ifndef LR_PROJ2_MINB
+#define LR_PROJ2_MINB 5
+#endif
+template <int PT>
+__global__ void __launch_bounds__(kProjPairThreads, LR_PROJ2_MINB)
+project_pair_kernel(const Params prm, const double* __restrict__ hp, const double* __restrict__ hc,
+                    const double* __restrict__ basis /* [batch][9] */, double* __restrict__ y) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int W = kProjThreads + prm.halo_lo + prm.halo_hi;
+  const int H = proj_pair_half(W);
+  D2* raw = reinterpret_cast<D2*>(smem_raw);
+  D2* dif_e = raw + W;      // first differences, de-interleaved: dif_e[i] = dif[2 i], dif_o[i] = dif[2 i + 1]
+  D2* dif_o = dif_e + H;
+  double* geo = reinterpret_cast<double*>(dif_o + H) + threadIdx.x;   // this thread's column of geo[kGeoFields][threads]
+
+  const int tile = blockIdx.x % prm.ntiles;
+  const int64_t b = blockIdx.x / prm.ntiles;
+  const int n0 = tile * kProjThreads;
+  const int g0 = n0 - prm.halo_lo;  // global sample index of staged index 0
+  const double* hpb = hp + b * prm.in_stride;
+  const double* hcb = hc + b * prm.in_stride;
+
+  __shared__ D4 sc[15 * 2];
+  __shared__ double bk_s[PT + 1];
+  if (threadIdx.x <= PT) bk_s[threadIdx.x] = prm.bk[threadIdx.x];
+  double u_unused;
+  const int n_last = n0 + kProjThreads - 1 < prm.n - 1 ? n0 + kProjThreads - 1 : prm.n - 1;
+  const int i_lo = spline_interval(prm, sample_trel(prm, prm.n_off + n0), u_unused);
+  const int i_hi = spline_interval(prm, sample_trel(prm, prm.n_off + n_last), u_unused);
+  const bool tile_coef = i_hi - i_lo <= 1;   // (block-uniform)
+  if (tile_coef && threadIdx.x < 30) {
+    const int ch = threadIdx.x >> 1, i = i_lo + (threadIdx.x & 1);
+    sc[threadIdx.x] = load4(prm.coef + (int64_t)ch * prm.nint + (i < prm.nint ? i : prm.nint - 1));
+  }
+  for (int m = threadIdx.x; m < W; m += kProjPairThreads) {
+    const int g = g0 + m;
+    D2 v{0.0, 0.0};
+    if (g >= prm.rd_lo && g < prm.rd_hi) { v.x = __ldg(hpb + g); v.y = __ldg(hcb + g); }
+    raw[m] = v;
+  }
+  __syncthreads();
+  for (int m = threadIdx.x; m < W - 1; m += kProjPairThreads) {
+    const D2 d{raw[m + 1].x - raw[m].x, raw[m + 1].y - raw[m].y};
+    ((m & 1) ? dif_o : dif_e)[m >> 1] = d;
+  }
+  __syncthreads();
+
+  const int nA = n0 + 2 * (int)threadIdx.x;
+  if (nA >= prm.n) return;
+  const bool hasB = nA + 1 < prm.n;
+  double* yb = y + b * 6 * prm.out_stride + nA;
+  const int ngA = prm.n_off + nA;   // global sample index
+  const int v_lo = prm.m_proj, v_hi = prm.n_glob - prm.m_proj;
+  const bool vA = ngA >= v_lo && ngA < v_hi, vB = hasB && ngA + 1 >= v_lo && ngA + 1 < v_hi;
+  const int64_t os = prm.out_stride;
+  if (!vA && !vB) {
+#pragma unroll
+    for (int s = 0; s < 6; ++s) {
+      yb[s * os] = 0.0;
+      if (hasB) yb[s * os + 1] = 0.0;
+    }
+    return;
+  }
+
+  double bs[9];
+#pragma unroll
+  for (int a = 0; a < 9; ++a) bs[a] = __ldg(basis + b * 9 + a);
+  auto store = [&](int slot, double a, double c) {
+    yb[slot * os] = vA ? a : 0.0;
+    if (hasB) yb[slot * os + 1] = vB ? c : 0.0;
+  };
+  const double tA = sample_trel(prm, ngA), tB = sample_trel(prm, ngA + 1);
+  if (tile_coef) {
+    project_geometry_store(prm, CoefTile{sc, i_lo}, tA, bs, geo, kProjPairThreads);
+    project_geometry_store(prm, CoefTile{sc, i_lo}, tB, bs, geo + kGeoPerSample * kProjPairThreads, kProjPairThreads);
+  } else {
+    project_geometry_store(prm, CoefGlobal{}, tA, bs, geo, kProjPairThreads);
+    project_geometry_store(prm, CoefGlobal{}, tB, bs, geo + kGeoPerSample * kProjPairThreads, kProjPairThreads);
+  }
+  project_pair<PT>(prm, raw, dif_e, dif_o, W, nA - g0, geo, kProjPairThreads, bk_s, store);
 }
 
 // ---------------------------------------------------------------------------------------------- stage 2

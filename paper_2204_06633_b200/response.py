@@ -89,6 +89,18 @@ class Response:
         B.lr_set_option(self._h, B.LR_OPT_TDI_PATH, {"auto": B.LR_TDI_AUTO, "per_sample": B.LR_TDI_PER_SAMPLE,
                                                      "fir3": B.LR_TDI_FIR3, "fir4": B.LR_TDI_FIR4}[path])
 
+    def set_proj_path(self, path):
+        """"auto" | "single" | "pair" (LR_OPT_PROJ_PATH)."""
+        B.lr_set_option(self._h, B.LR_OPT_PROJ_PATH, {"auto": B.LR_PROJ_AUTO, "single": B.LR_PROJ_SINGLE,
+                                                      "pair": B.LR_PROJ_PAIR}[path])
+
+    def create_plan(self, n, stream=None):
+        """A shareable read-only TDI plan for this handle's options and a series of n samples (lr_plan_create)."""
+        return B.lr_plan_create(self._h, n, stream)
+
+    def attach_plan(self, plan):
+        B.lr_plan_attach(self._h, plan)
+
     def set_plan_cache(self, on):
         B.lr_set_option(self._h, B.LR_OPT_TDI_PLAN_CACHE, 1 if on else 0)
 

@@ -320,6 +320,36 @@ def test_orders(lr, order):
     check_workload(lr, w, channels="XYZ", tdi_path="per_sample", proj=False)
 
 
+@pytest.mark.parametrize("order", [1, 5, 9, 13, 21, 25, 31, 41, 17])
+def test_project_pair_path_bitwise(lr, order):
+    """LR_PROJ_PAIR (two consecutive samples per thread, shared first differences, geometry parked in shared memory,
+    de-interleaved window) against LR_PROJ_SINGLE: the same bits, on ragged multi-template launches, on a time chunk
+    that starts at an odd global sample, and on orbits whose reception delay wraps through whole samples many
+    times (the out-of-line path of a pair whose integer shifts differ).  Order 17 has no compile-time kernel: the
+    option is accepted and runs the single path."""
+    import torch
+    w = inputs.config(3, batch=3, n=20011, t0=4.0e6)
+    w.order = order
+    hp, hc = _stack(w, range(3))
+    be, la, ps = ([getattr(s, k) for s in w.sources] for k in ("beta", "lam", "psi"))
+    hpd, hcd = to_dev(hp), to_dev(hc)
+    outs = {}
+    for path in ("single", "pair"):
+        R = lr.Response(w.table(), w.dt, order, 2, t0=w.t0)
+        R.set_proj_path(path)
+        y = R.project(hpd, hcd, be, la, ps)
+        lr.lr_set_option(R.handle, lr.LR_OPT_CHUNK_SAMPLES, 1792 * 2)    # chunks whose y window starts at a - halo
+        outs[path] = (y.cpu().numpy(), R.response(hpd, hcd, be, la, ps).cpu().numpy())
+    assert np.array_equal(outs["single"][0], outs["pair"][0])
+    assert np.array_equal(outs["single"][1], outs["pair"][1])
+    mp = lr.Response(w.table(), w.dt, order, 2, t0=w.t0).margins()[0]
+    assert np.count_nonzero(outs["pair"][0][:, :, mp:w.n - mp]) > 0.99 * 18 * (w.n - 2 * mp)
+    if order == 25:   # template 0 against the oracle, through the pair path
+        O = orc.Oracle(w.table(), w.dt, w.t0, order)
+        yo = O.project(hp[0], hc[0], be[0], la[0], ps[0], lo=mp, hi=mp + 3000)
+        assert_parity(outs["pair"][0][0][:, mp:mp + 3000], yo[:, mp:mp + 3000], "pair path", LINK_NAMES)
+
+
 # ---------------------------------------------------------------------------------------------- pins
 @pytest.mark.parametrize("knot_dt", [400.0, 1000.0, 1290.0])
 def test_dense_orbit_knots(lr, knot_dt):
