@@ -13,15 +13,12 @@
 
 namespace lr {
 
-// Launch shapes, tuned on B200 (profiles/r1_tuning.md): both kernels are bound by the FP64 pipe and want
+// Launch shapes, tuned on B200: both kernels are bound by the FP64 pipe and want
 // 12-24 resident warps per SM; letting ptxas take 160-250 registers per thread (one CTA per SM) halves the
 // throughput.  The caps below keep the order-25 kernels spill-free.
 constexpr int kProjThreads = 128;      // samples per projection tile (and threads of the one-sample-per-thread kernel)
 constexpr int kProjPairThreads = 64;   // threads of the two-samples-per-thread kernel (same 128-sample tile)
 constexpr int kTdiThreads = 256;
-#ifndef LR_PROJ_MINB
-#define LR_PROJ_MINB 4
-#endif
 // elements of each half of the de-interleaved difference window of the pair kernel
 __host__ __device__ constexpr int proj_pair_half(int W) { return (W >> 1) + 1; }
 // dynamic shared memory of project_pair_kernel: raw[W], dif_e[H], dif_o[H] (D2), geo[kGeoFields][threads]
@@ -30,7 +27,7 @@ __host__ __device__ constexpr size_t proj_pair_smem(int W) {
 }
 // orders whose projection runs two samples per thread (compile-time P; the run-time-P build keeps one)
 __host__ __device__ constexpr bool proj_pairs(int PT) { return PT >= 1; }
-__host__ __device__ constexpr int proj_min_blocks(int PT) { return PT == 0 ? 2 : PT <= 13 ? LR_PROJ_MINB : 3; }
+__host__ __device__ constexpr int proj_min_blocks(int PT) { return PT == 0 ? 2 : PT <= 13 ? 4 : 3; }
 __host__ __device__ constexpr int tdi_min_blocks(int PT) { return PT == 0 ? 2 : PT <= 13 ? 3 : 2; }
 
 // ---------------------------------------------------------------------------------------------- stage 1
@@ -100,11 +97,8 @@ project_kernel(const Params prm, const double* __restrict__ hp, const double* __
 
 // Two consecutive samples per thread (project_pair): the same tile, staging and results as project_kernel with half
 // the threads; every first difference a pair of stencils shares is read from shared memory once.
-#ifndef LR_PROJ2_MINB
-#define LR_PROJ2_MINB 5
-#endif
 template <int PT>
-__global__ void __launch_bounds__(kProjPairThreads, LR_PROJ2_MINB)
+__global__ void __launch_bounds__(kProjPairThreads, 5)   // 168 registers: 6 CTAs of 64 threads per SM
 project_pair_kernel(const Params prm, const double* __restrict__ hp, const double* __restrict__ hc,
                     const double* __restrict__ basis /* [batch][9] */, double* __restrict__ y) {
   extern __shared__ __align__(16) unsigned char smem_raw[];

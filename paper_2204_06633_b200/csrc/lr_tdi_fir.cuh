@@ -23,13 +23,9 @@
 
 namespace lr {
 
-#ifndef LR_FIR_MINB
-#define LR_FIR_MINB 7                    // resident apply CTAs per SM the register budget is set for
-#endif
-#ifndef LR_FIR_R
-#define LR_FIR_R 7
-#endif
-constexpr int kFirR = LR_FIR_R;          // consecutive samples per thread (odd: conflict-free 64-bit smem reads)
+constexpr int kFirMinBlocks = 7;  // resident apply CTAs per SM the register budget is set for (80 registers: 8 fit)
+constexpr int kFirR = 7;          // consecutive samples per thread (odd: conflict-free 64-bit smem reads; R = 5, 9,
+                                  // 11 and 14 were measured slower)
 constexpr int kFirKStride = 4;    // doubles per (series, m) coefficient record (NN <= 4)
 
 // series used by channel X, in "local" order 13, 31, 12, 21; Y and Z rotate the slots
@@ -355,7 +351,7 @@ __device__ __forceinline__ void fir_store(double* ob, int64_t N, int n, int chan
 }
 
 template <int NN>
-__global__ void __launch_bounds__(kFirThreads, NN > 3 ? 5 : LR_FIR_MINB)   // NN = 4: 28 accumulators
+__global__ void __launch_bounds__(kFirThreads, NN > 3 ? 5 : kFirMinBlocks)   // NN = 4: 28 accumulators
 tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ out, int channels,
                      const double* __restrict__ plan, const int* __restrict__ flags, int batch) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
