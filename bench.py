@@ -4,20 +4,27 @@
 Contract: `python bench.py --gpus N --steps K --warmup W` prints ONE JSON line.
   * a step = one pass of the whole hot path (six-link projection + TDI-2) over one batch of synthetic input;
   * N = 1 workload = BASELINE.json configs[1]: one Galactic binary, 1 year at dt = 10 s (3,153,600 samples),
-    Keplerian orbits, Lagrange order 25, nested second-generation TDI, X,Y,Z + A,E,T;  `--workload batch`
-    times configs[2] (MCMC batch, templates/s) in chunks instead;
+    Keplerian orbits, Lagrange order 25, nested second-generation TDI, X,Y,Z + A,E,T;
+  * the default run also carries a `batch` leg (one 64-template launch of configs[2], the MCMC batch: templates/s,
+    per-kernel roofline fractions, clocks, parameters -> log L) and an `orders` leg (orders 1, 9, 25, 41 on the
+    one-year shape: ms and fraction of the binding roof per kernel); `--workload batch` times all 1,024 templates;
   * N > 1: every rank runs the same-sized workload on its own seeded template(s) (the path shards over
     templates with no collective: "scaling": "weak"); time = max over ranks, value = all ranks' samples / time;
   * `value` has the inputs resident in HBM; `e2e` goes through lr_response_host with pinned HOST buffers;
   * `roofline`: the dominant kernel (the slower of lr_project / lr_tdi) against the FP64 issue rate measured
-    live by lr_measure_fp64_peak; `kernels` has both; `lr_response`, `likelihood`, `tdi_plan` are extra legs;
-  * `cpu_baseline` / `--impl reference`: the oracle (fp64 arithmetic, all host cores) on a bounded sample.
+    live by lr_measure_fp64_peak; `kernels` has both, lr_tdi also against the FMAs its FIR path EXECUTES;
+  * ncu-only counters (DRAM traffic, pipe busy) come from profiles/r2_ncu_counters.csv and are reported only while
+    the hash of csrc/ recorded there equals the sources this run was built from (null + reason otherwise);
+  * `cpu_baseline` / `--impl reference`: the oracle (fp64 arithmetic) on a bounded sample, all host cores and one.
 """
 from __future__ import annotations
 
 import argparse
+import csv
+import hashlib
 import json
 import os
+import subprocess
 import sys
 import threading
 import time
@@ -26,11 +33,42 @@ import numpy as np
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
 DEFAULT_CHUNK = 64   # templates per launch of the batched config (tests/test_gpu_fullsize.py checks this shape)
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernels from the one `ncu --set full`
-# capture summarised in profiles/r1_v5_launches.md (full capture of the final build); reported as roofline.traffic
-NCU_TRAFFIC = {("year", "lr_project"): 50714112 + 97300480, ("year", "lr_tdi"): 339880704 + 118690560}
+NCU_COUNTERS = os.path.join(ROOT, "profiles", "r2_ncu_counters.csv")
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
+
+
+def csrc_hash():
+    """sha256 over the sources liblr.so is built from (names and contents, sorted): the key of the ncu counters."""
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2204_06633_b200", "csrc")
+    for name in sorted(os.listdir(d)) + [os.path.join("..", "..", "include", "lr.h")]:
+        path = os.path.join(d, name)
+        if os.path.isfile(path) and name.endswith((".cu", ".cuh", ".hpp", ".h")):
+            h.update(os.path.basename(name).encode())
+            h.update(open(path, "rb").read())
+    return h.hexdigest()
+
+
+def ncu_counters(workload, kernel):
+    """Counters of one `ncu --set full` capture (profiles/r2_ncu_counters.csv; the .md beside it names the command),
+    valid only for the build they were captured on.  Returns (dict or None, reason)."""
+    try:
+        rows = list(csv.DictReader(open(NCU_COUNTERS)))
+    except OSError:
+        return None, "profiles/r2_ncu_counters.csv not found"
+    rows = [r for r in rows if r["workload"] == workload and r["api"] == kernel]
+    if not rows:
+        return None, f"no ncu capture of {kernel} on the {workload} workload"
+    now = csrc_hash()
+    r = rows[-1]
+    if r["csrc_sha256"] != now:
+        return None, f"csrc/ changed since the capture (captured {r['csrc_sha256'][:12]}, built from {now[:12]})"
+    num = lambda k: float(r[k]) if r.get(k) not in (None, "") else None
+    return {"kernel": r["kernel"], "time_us": num("time_us"), "dram_bytes": num("dram_bytes_read") + num("dram_bytes_write"),
+            "pipe_fp64_pct": num("pipe_fp64_pct"), "smem_wavefronts_pct": num("smem_wavefronts_pct"),
+            "issue_active_pct": num("issue_active_pct"), "registers": num("registers")}, None
+
 
 # algorithmic FP64 instruction slots per time sample (SURVEY.md §8(d), T = order + 1 taps; DFMA = 1)
 def ops_project(T):
@@ -164,6 +202,24 @@ def gb_waveform_device(srcs, n, dt, t0, device):
 
 
 # ------------------------------------------------------------------------------------------ CPU oracle
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def omp_threads():
+    """Threads the oracle's OpenMP loops use in this process (it has no setter: OMP_NUM_THREADS or all cores)."""
+    try:
+        return max(1, int(os.environ.get("OMP_NUM_THREADS", "")))
+    except ValueError:
+        return os.cpu_count() or 1
+
+
 def time_oracle(w, target_s=12.0):
     """The oracle as it stands (oracle/lr_oracle.cpp, fp64 arithmetic, OpenMP over samples) on a window of
     the workload's first template, sized for about target_s of host time.  Returns (samples/s, info)."""
@@ -174,7 +230,6 @@ def time_oracle(w, target_s=12.0):
     s = w.sources[0]
     mp, mf, mb = O.margins(w.tdi_gen)
     ch = {"XYZ": 0, "AET": 1, "XYZ_AET": 2}[w.channels]
-    cores = os.cpu_count() or 1
     mid = max(mf, w.n // 8)
 
     def run(m):
@@ -187,26 +242,48 @@ def time_oracle(w, target_s=12.0):
     t_probe, m_probe = run(2000)
     m = int(max(2000, min(w.n - mb - mid, m_probe * target_s / max(t_probe, 1e-6))))
     t, m = run(m)
-    return m / t, {"cores": cores, "kind": "oracle",
+    return m / t, {"cores": omp_threads(), "kind": "oracle", "cpu_model": cpu_model(),
                    "sample": f"{m} consecutive samples starting at n/8 of template 0 (projection + TDI-{w.tdi_gen}, "
                              f"fp64 build of the oracle, OpenMP over samples), {t:.1f} s wall"}
 
 
+def time_oracle_one_thread(args, target_s):
+    """The same measurement in a child process with OMP_NUM_THREADS=1 (PAPER.md:273 quotes "a single ... CPU
+    processor"): the oracle is not touched, the child is `bench.py --impl reference`."""
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    cmd = [sys.executable, os.path.abspath(__file__), "--impl", "reference", "--workload", args.workload, "--steps", "1",
+           "--warmup", "0", "--cpu-seconds", str(target_s)]
+    if args.order is not None:
+        cmd += ["--order", str(args.order)]
+    try:
+        r = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=60 + 20 * target_s)
+        line = [ln for ln in r.stdout.splitlines() if ln.startswith("{")][-1]
+        d = json.loads(line)["cpu_baseline"]
+        return {"value": d["value"], "unit": "samples/s", "cores": d["cores"], "sample": d["sample"]}
+    except Exception as exc:   # never let the optional figure break the contract line
+        return {"error": repr(exc)}
+
+
 def run_reference(args, rank, world):
-    """--impl reference: the oracle on the host cores, same metric/config; rank 0 only."""
+    """--impl reference: the oracle on the host cores, same metric/config; rank 0 only.  Every step is a MEASURED
+    bounded window of the workload (ms_per_step is the time of that window, `sample` says how long it was)."""
     if rank != 0:
         return
     w, _ = make_workload(args.workload, 0, args.order)
     vals, info = [], None
     per_step = min(args.cpu_seconds, max(1.0, min(20.0, 120.0 / max(1, args.steps + args.warmup))))
+    t_steps = []
     for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
         v, info = time_oracle(w, target_s=per_step)
         if i >= args.warmup:
             vals.append(v)
+            t_steps.append(time.perf_counter() - t0)
     v = float(np.mean(vals))
     line = {"impl": "reference", "metric": "response samples/s (6-link proj + TDI-2, fp64)", "value": v,
             "unit": "samples/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": 1e3 * w.n / v, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": 1e3 * float(np.mean(t_steps)), "ms_per_whole_workload_extrapolated": 1e3 * w.n / v,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": workload_config(w, 1, args),
             "cpu_baseline": dict(info, value=v, unit="samples/s"),
             "e2e": {"value": v, "unit": "samples/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
@@ -218,7 +295,163 @@ def workload_config(w, batch, args):
             "batch": batch, "n": w.n, "dt": w.dt, "lagrange_order": w.order,
             "tdi_gen": 1 if args.workload == "hybrid" else w.tdi_gen,
             "chain": "nested", "channels": w.channels, "orbits": w.orbit_kind, "tdi_path": args.tdi_path,
+            "tdi_plan": "cached (built once per handle, like the paper's orbit arrays, PAPER.md:263; the `tdi_plan` key "
+                        "has the step with the plan rebuilt in every call)",
             "l2": "flushed between steps (256 MiB memset outside the per-step event pairs)"}
+
+
+def hbm_peak():
+    """Measured HBM copy rate of this pool's B200 [GB/s] (driver-written MEASURED_PEAKS.json), else the fallback."""
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    except Exception:
+        return 6650.0, "fallback 6.65 TB/s (B200_PROFILING.md)"
+
+
+def kernel_stats(ms_proj, ms_tdi, units, order, gen, nout, tdi_info, peak, hbm_gbs):
+    """Per-kernel roofline figures.  units = template-samples one step processes.  frac_fp64: SURVEY §8(d)'s
+    ALGORITHMIC instruction slots per second / measured FP64 issue rate; lr_tdi also gets frac_executed: the FMAs its
+    FIR path really executes (3 channels x 4 series x taps x powers of tile time, from the handle) / the same rate;
+    frac_hbm: algorithmic bytes per second / measured HBM copy rate.  `bound`: the larger of the two fractions."""
+    T = order + 1
+    path, taps, powers = tdi_info
+    out = {}
+    for name, ms, ops, nbytes in (("lr_project", ms_proj, ops_project(T), BYTES_PROJECT),
+                                  ("lr_tdi", ms_tdi, ops_tdi(T, gen), bytes_tdi(nout))):
+        rate = units / (ms * 1e-3)
+        k = {"ms": ms, "alg_ops_per_sample": ops, "gops": ops * rate / 1e9, "frac_fp64": ops * rate / peak,
+             "alg_bytes_per_sample": nbytes, "alg_GBps": nbytes * rate / 1e9, "frac_hbm": nbytes * rate / 1e9 / hbm_gbs}
+        if name == "lr_tdi":
+            k["path"] = path
+            if path != "per_sample":
+                ex = 3 * 4 * taps * powers
+                k.update(executed_ops_per_sample=ex, fir_taps=taps, fir_powers=powers, frac_executed=ex * rate / peak,
+                         executed_note="FMAs of the per-tile FIR filters (3 channels x 4 series x taps x powers of tile "
+                                       "time); the algorithmic count charges a weight set per term and sample, so "
+                                       "frac_fp64 > 1 here means fewer instructions, not a fuller pipe")
+            else:
+                k.update(executed_ops_per_sample=ops, frac_executed=ops * rate / peak)
+        k["bound"] = "alu" if k.get("frac_executed", k["frac_fp64"]) >= k["frac_hbm"] else "hbm"
+        out[name] = k
+    return out
+
+
+def timed_steps(lr, R, Rt, hp, hc, ang, y, out, reps, flush, stream):
+    """reps x (lr_project, lr_tdi) on resident inputs; mean ms of each from CUDA events on the launch stream."""
+    import torch
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    tp, tt = [], []
+    for _ in range(reps):
+        if flush is not None:
+            flush.zero_()
+        e0, e1, e2 = ev(), ev(), ev()
+        e0.record(stream)
+        R.project(hp, hc, *ang, y_out=y)
+        e1.record(stream)
+        Rt.tdi(y, out=out)
+        e2.record(stream)
+        e2.synchronize()
+        tp.append(e0.elapsed_time(e1))
+        tt.append(e1.elapsed_time(e2))
+    return float(np.mean(tp)), float(np.mean(tt))
+
+
+def batch_leg(lr, dev, local_rank, peak, hbm_gbs, reps=6):
+    """BASELINE.json configs[2] (the MCMC batch) in the launch shape of `--workload batch`: ONE chunk of 64 of its
+    1,024 templates at the full 1,576,800 samples, A,E,T: lr_project + lr_tdi per launch (the whole config is 16
+    such launches), then parameters -> log L for the same 64 templates (lr_loglike_gb)."""
+    import torch
+    from harness import inputs
+    w = inputs.config(3)
+    nb, n = DEFAULT_CHUNK, w.n
+    src = w.sources[:nb]
+    R = lr.Response(w.table(), w.dt, w.order, w.tdi_gen, t0=w.t0, chain="nested", channels="AET")
+    hp, hc = inputs.gb_waveform_device(src, n, w.dt, w.t0, dev)
+    ang = ([s.beta for s in src], [s.lam for s in src], [s.psi for s in src])
+    y = torch.empty((nb, 6, n), dtype=torch.float64, device=dev)
+    out = torch.empty((nb, 3, n), dtype=torch.float64, device=dev)
+    stream = torch.cuda.current_stream()
+    timed_steps(lr, R, R, hp, hc, ang, y, out, 2, None, stream)          # warm-up (builds the plan)
+    l0 = lr.lr_launch_count()
+    with ClockSampler(local_rank) as clk:
+        ms_p, ms_t = timed_steps(lr, R, R, hp, hc, ang, y, out, reps, None, stream)
+        torch.cuda.synchronize()
+    launches = lr.lr_launch_count() - l0
+    ks = kernel_stats(ms_p, ms_t, float(nb) * n, w.order, w.tdi_gen, 3, R.tdi_info(), peak, hbm_gbs)
+    dom = "lr_tdi" if ms_t >= ms_p else "lr_project"
+    kd = ks[dom]
+    leg = {"workload": "BASELINE.json configs[2] (MCMC batch): one launch of 64 of the 1,024 templates, 1,576,800 samples "
+                       "each, Keplerian, order 25, nested TDI-2, A,E,T; inputs resident (8.8 GB per launch, far above L2)",
+           "templates_per_launch": nb, "reps": reps, "ms_per_launch": ms_p + ms_t,
+           "templates_per_s": nb / ((ms_p + ms_t) * 1e-3), "value": nb * n / ((ms_p + ms_t) * 1e-3), "unit": "samples/s",
+           "gpu_launches": launches, "kernels": ks,
+           "roofline": {"bound": "alu", "kernel": dom, "achieved": kd["gops"], "peak": peak / 1e9,
+                        "unit": "Gop/s (FP64 thread-instruction slots, DFMA = 1)", "frac": kd["frac_fp64"],
+                        "frac_executed": kd.get("frac_executed"), "traffic": None,
+                        "path_frac": (ks["lr_project"]["alg_ops_per_sample"] + ks["lr_tdi"]["alg_ops_per_sample"]) * nb * n
+                                     / ((ms_p + ms_t) * 1e-3) / peak},
+           "clocks": clk.summary()}
+    del y, hp, hc
+    # parameters -> log L for the 64 templates (15 doubles in, 1 out per template; wall clock incl. the read-back)
+    try:
+        gb = np.array([[s.A * (1.0 + np.cos(s.iota) ** 2), -2.0 * s.A * np.cos(s.iota), s.f0, s.fdot, 0.0, s.phi0]
+                       for s in src])
+        m = lr.lr_fft_good_length(n)
+        R.set_fft_length(m)
+        nf = m // 2 + 1
+        inv = torch.ones((3, nf), dtype=torch.float64, device=dev)
+        inv[:, 0] = 0.0
+        data_f = torch.fft.rfft(out[0], n=m, dim=-1).contiguous()
+        del out
+        tw = []
+        for it in range(5):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            ll = R.loglike_gb(gb, *ang, n, data_f, inv, -2.0 * w.dt / m).cpu()
+            if it >= 2:
+                tw.append((time.perf_counter() - t0) * 1e3)
+        leg["params_to_loglike"] = {"api": "lr_loglike_gb, 64 templates per call, transform zero padded to "
+                                           f"{m} samples (LR_OPT_FFT_LENGTH)", "ms_per_call_wall": float(np.median(tw)),
+                                    "loglike_per_s": nb / (float(np.median(tw)) * 1e-3),
+                                    "h2d_bytes_per_call": nb * 15 * 8, "d2h_bytes_per_call": nb * 8,
+                                    "log_l_of_the_data_template": float(ll[0])}
+    except Exception as exc:
+        leg["params_to_loglike"] = {"error": repr(exc)}
+    return leg
+
+
+def orders_leg(lr, dev, peak, hbm_gbs, orders=(1, 9, 25, 41), reps=5):
+    """SURVEY §8(f) NEXT-3 (orders below 10 "can improve the speed", order 1 -> 25 changes the run
+    time by "a factor of order unity"): the one-year shape at several Lagrange orders; per kernel the time and the
+    fraction of the roof that binds at that order (FP64 issue or HBM)."""
+    import torch
+    from harness import inputs
+    w = inputs.config(2)
+    s = w.sources[0]
+    hp_np, hc_np = w.waveform(0)
+    hp, hc = torch.from_numpy(hp_np).to(dev)[None], torch.from_numpy(hc_np).to(dev)[None]
+    ang = ([s.beta], [s.lam], [s.psi])
+    y = torch.empty((1, 6, w.n), dtype=torch.float64, device=dev)
+    out = torch.empty((1, 6, w.n), dtype=torch.float64, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    rows = []
+    for order in orders:
+        R = lr.Response(w.table(), w.dt, order, 2, t0=w.t0, chain="nested", channels="XYZ_AET")
+        timed_steps(lr, R, R, hp, hc, ang, y, out, 2, flush, stream)
+        ms_p, ms_t = timed_steps(lr, R, R, hp, hc, ang, y, out, reps, flush, stream)
+        ks = kernel_stats(ms_p, ms_t, float(w.n), order, 2, 6, R.tdi_info(), peak, hbm_gbs)
+        row = {"order": order, "ms_per_step": ms_p + ms_t, "value": w.n / ((ms_p + ms_t) * 1e-3)}
+        for name, k in ks.items():
+            row[name] = {"ms": k["ms"], "bound": k["bound"], "frac": max(k["frac_fp64"], k["frac_hbm"]) if name == "lr_project"
+                         else max(k["frac_executed"], k["frac_hbm"]), "frac_fp64": k["frac_fp64"], "frac_hbm": k["frac_hbm"],
+                         **({"frac_executed": k["frac_executed"]} if name == "lr_tdi" else {})}
+        rows.append(row)
+        R.close()
+    return {"workload": "BASELINE.json configs[1] shape (3,153,600 samples, X,Y,Z+A,E,T, plan cached) at other Lagrange orders",
+            "frac_note": "per kernel: fraction of the roof that binds at that order; lr_project: algorithmic FP64 slots or "
+                         "bytes; lr_tdi: executed FMAs of the FIR path or bytes",
+            "orders": rows}
 
 
 # --------------------------------------------------------------------------------------------- GPU arm
@@ -477,12 +710,16 @@ def run_gpu(args, rank, world, local_rank):
 
     if rank != 0:
         return
-    ops_t, ops_p = ops_tdi(T, tdi_gen), ops_project(T)
-    ach_tdi = ops_t * batch * n / (ms_tdi * 1e-3)
-    ach_proj = ops_p * batch * n / (ms_proj * 1e-3)
+    hbm_gbs, hbm_src = hbm_peak()
+    ks = kernel_stats(ms_proj, ms_tdi, float(batch) * n, w.order, tdi_gen, nout, Rt.tdi_info(), peak, hbm_gbs)
     dom = "lr_tdi" if ms_tdi >= ms_proj else "lr_project"
-    ach_dom = ach_tdi if dom == "lr_tdi" else ach_proj
-    traffic = NCU_TRAFFIC.get((args.workload, dom)) if (args.order is None or args.order == 25) else None
+    kd = ks[dom]
+    # ncu-only counters of the two kernels: from the tracked capture, valid only for the build it was taken on
+    ncu = {}
+    for api in ("lr_project", "lr_tdi"):
+        c, why = ncu_counters(args.workload, api) if (args.order is None and args.tdi_path == "auto") else (None, "non-default order or TDI path")
+        ncu[api] = c if c is not None else {"unavailable": why}
+    traffic = ncu[dom].get("dram_bytes")
     line = {
         "metric": "response samples/s (6-link proj + TDI-2, fp64)" if args.workload != "batch"
                   else "response samples/s (6-link proj + TDI-2 AET, fp64), batched",
@@ -496,31 +733,49 @@ def run_gpu(args, rank, world, local_rank):
                 "templates": eb, "h2d_bytes_per_step": 2 * eb * n * 8, "d2h_bytes_per_step": nout * eb * n * 8,
                 "api": "lr_response_host (pinned host buffers)"},
         "gpu_launches": launches,
-        "kernels": {"lr_project": {"ms": ms_proj, "alg_ops_per_sample": ops_p, "gops": ach_proj / 1e9,
-                                   "frac_fp64": ach_proj / peak, "alg_GBps": BYTES_PROJECT * batch * n / (ms_proj * 1e6)},
-                    "lr_tdi": {"ms": ms_tdi, "alg_ops_per_sample": ops_t, "gops": ach_tdi / 1e9,
-                               "frac_fp64": ach_tdi / peak, "alg_GBps": bytes_tdi(nout) * batch * n / (ms_tdi * 1e6)}},
+        "kernels": ks,
         "likelihood": lk,
         "params_to_loglike": pl,
         "lr_response": {"ms_per_step": ms_resp, "note": "one call, h -> out, y only in a scratch of two <= 1 GB slots"},
         "tdi_plan": {"cached_between_calls": True, "ms_tdi_with_plan_rebuilt_every_call": ms_tdi_cold,
                      "value_with_plan_rebuilt_every_call": units / (max_over_ranks(ms_proj + ms_tdi_cold) * 1e-3)
                      if world == 1 else None},
-        "roofline": {"bound": "alu", "kernel": dom + (" (tdi_fir_apply_kernel)" if dom == "lr_tdi" and args.tdi_path != "per_sample" else ""),
-                     "achieved": ach_dom / 1e9, "peak": peak / 1e9,
-                     "unit": "Gop/s (FP64 thread-instruction slots, DFMA = 1)", "frac": ach_dom / peak,
+        "roofline": {"bound": "alu", "kernel": dom + (" (tdi_fir_apply_kernel)" if dom == "lr_tdi" and ks["lr_tdi"]["path"] != "per_sample" else ""),
+                     "achieved": kd["gops"], "peak": peak / 1e9,
+                     "unit": "Gop/s (FP64 thread-instruction slots, DFMA = 1)", "frac": kd["frac_fp64"],
+                     "frac_executed": kd.get("frac_executed"),
                      "traffic": traffic,
+                     "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r2_ncu_counters.csv"
+                                       if traffic is not None else ncu[dom].get("unavailable"),
                      "peak_source": f"lr_measure_fp64_peak({args.peak_seconds} s DFMA kernel) on this device, this run",
                      "peak_nominal": torch.cuda.get_device_properties(dev).multi_processor_count * 64 *
                                      (clk.max_mhz or 1965) * 1e-3,   # SMs x 64 FP64 lanes x max SM clock [Gop/s]
-                     "pipe_busy_pct_ncu": {"lr_project": 71.1, "lr_tdi": 64.4, "source": "profiles/r1_v5_launches.md"},
-                     "shared_memory_pipe_busy_pct_ncu": {"lr_project": 85.6, "lr_tdi": 37.6},
-                     "path_frac": (ops_t + ops_p) * batch * n / ((ms_proj + ms_tdi) * 1e-3) / peak},
+                     "hbm_peak_GBps": hbm_gbs, "hbm_peak_source": hbm_src,
+                     "ncu": ncu, "csrc_sha256": csrc_hash(),
+                     "path_frac": (ks["lr_project"]["alg_ops_per_sample"] + ks["lr_tdi"]["alg_ops_per_sample"]) * batch * n
+                                  / ((ms_proj + ms_tdi) * 1e-3) / peak},
         "clocks": clk.summary(), "wall_s_timed_region": wall,
     }
+    # free the main workload's buffers before the extra legs
+    del y, out, flush, hp_h, hc_h, out_h
+    h_cache.clear()
+    torch.cuda.empty_cache()
+    if world == 1 and args.workload == "year" and args.order is None and args.tdi_path == "auto":
+        if not args.no_batch_leg:
+            try:
+                line["batch"] = batch_leg(lr, dev, local_rank, peak, hbm_gbs)
+            except Exception as exc:   # never let an extra leg break the contract line
+                line["batch"] = {"error": repr(exc)}
+            torch.cuda.empty_cache()
+        if not args.no_orders_leg:
+            try:
+                line["orders"] = orders_leg(lr, dev, peak, hbm_gbs)
+            except Exception as exc:
+                line["orders"] = {"error": repr(exc)}
     if world == 1 and not args.no_cpu_baseline:
         v, info = time_oracle(w, target_s=args.cpu_seconds)
-        line["cpu_baseline"] = dict(info, value=v, unit="samples/s")
+        line["cpu_baseline"] = dict(info, value=v, unit="samples/s",
+                                    one_thread=time_oracle_one_thread(args, args.cpu_seconds))
     print(json.dumps(line), flush=True)
 
 
@@ -600,8 +855,10 @@ def main():
     ap.add_argument("--chunk", type=int, default=DEFAULT_CHUNK, help="templates per launch (batch workload)")
     ap.add_argument("--e2e-templates", type=int, default=4)
     ap.add_argument("--peak-seconds", type=float, default=1.0)
-    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--cpu-seconds", type=float, default=10.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-batch-leg", action="store_true", help="skip the 64-template launch of configs[2]")
+    ap.add_argument("--no-orders-leg", action="store_true", help="skip the Lagrange-order sweep")
     ap.add_argument("--tdi-path", default="auto", choices=["auto", "per_sample", "fir3", "fir4"])
     ap.add_argument("--shard", default="templates", choices=["templates", "time"],
                     help="N > 1: 'templates' = every rank its own template(s) (weak scaling, default); 'time' = ONE "

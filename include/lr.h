@@ -65,6 +65,16 @@ typedef struct {
 #define LR_OPT_TDI_PLAN_CACHE 6 /* 1 (default): keep the FIR plan between lr_tdi calls; 0: rebuild every call */
 #define LR_OPT_PROJ_PATH 9 /* LR_PROJ_AUTO (default) | LR_PROJ_SINGLE | LR_PROJ_PAIR */
 
+/* Read-only keys of lr_get_option: what lr_tdi will do with the handle's current orbits and options.
+ *   LR_INFO_TDI_PATH   : the path LR_TDI_AUTO resolves to (LR_TDI_PER_SAMPLE | LR_TDI_FIR3 | LR_TDI_FIR4)
+ *   LR_INFO_FIR_TAPS   : taps per series of the merged FIR filters (0 on the per-sample path)
+ *   LR_INFO_FIR_POWERS : accumulators per output sample = powers of tile time (1 for constant light times, 3, 4; 0 on
+ *                        the per-sample path).  The FIR path executes 3 channels x 4 series x taps x powers FMAs per
+ *                        sample (bench.py's `executed_ops_per_sample`). */
+#define LR_INFO_TDI_PATH 101
+#define LR_INFO_FIR_TAPS 102
+#define LR_INFO_FIR_POWERS 103
+
 /* How lr_project maps time samples to threads (the results are the same bit for bit).
  *   LR_PROJ_SINGLE : one sample per thread.
  *   LR_PROJ_PAIR   : two consecutive samples per thread; the two Lagrange stencils of every interpolation time share

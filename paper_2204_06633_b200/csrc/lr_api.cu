@@ -127,6 +127,9 @@ struct lr_handle {
 
 namespace {
 
+struct TdiShape { int path, wc, taps, halo_lo, halo_hi; };
+TdiShape tdi_shape(const lr_handle* h);
+
 #define LR_CUDA(h, call)                      \
   do {                                        \
     cudaError_t e__ = (call);                 \
@@ -384,6 +387,13 @@ int lr_get_option(const lr_handle* h, int key, double* value) {
     case LR_OPT_CHUNK_SAMPLES: *value = (double)h->chunk_samples; return LR_OK;
     case LR_OPT_FFT_LENGTH: *value = (double)h->fft_length; return LR_OK;
     case LR_OPT_TDI_PLAN_CACHE: *value = h->plan_cache; return LR_OK;
+    case LR_INFO_TDI_PATH: *value = tdi_shape(h).path; return LR_OK;
+    case LR_INFO_FIR_TAPS: *value = tdi_shape(h).taps; return LR_OK;
+    case LR_INFO_FIR_POWERS: {
+      const TdiShape t = tdi_shape(h);
+      *value = t.path == LR_TDI_PER_SAMPLE ? 0 : h->const_ltt ? 1 : t.path == LR_TDI_FIR4 ? 4 : 3;
+      return LR_OK;
+    }
     default: return LR_EINVAL;
   }
 }
@@ -426,7 +436,6 @@ int project_window(lr_handle* h, const double* hp, const double* hc, const doubl
 }
 
 // which lr_tdi path this handle takes, and the staged halo of that path's kernels
-struct TdiShape { int path, wc, taps, halo_lo, halo_hi; };
 
 TdiShape tdi_shape(const lr_handle* h) {
   TdiShape t{h->tdi_path, 0, 0, 0, 0};

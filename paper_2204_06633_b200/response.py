@@ -108,6 +108,12 @@ class Response:
         B.lr_set_option(self._h, B.LR_OPT_TDI_GEN, gen)
         self.tdi_gen = gen
 
+    def tdi_info(self):
+        """(resolved lr_tdi path, FIR taps per series, accumulators per sample) of this handle (LR_INFO_*)."""
+        g = lambda k: int(B.lr_get_option(self._h, k))
+        path = {B.LR_TDI_PER_SAMPLE: "per_sample", B.LR_TDI_FIR3: "fir3", B.LR_TDI_FIR4: "fir4"}[g(B.LR_INFO_TDI_PATH)]
+        return path, g(B.LR_INFO_FIR_TAPS), g(B.LR_INFO_FIR_POWERS)
+
     def margins(self):
         return B.lr_get_margins(self._h)
 
