@@ -21,6 +21,8 @@ LR_OPT_TDI_PLAN_CACHE = 6
 LR_OPT_CHUNK_SAMPLES = 7
 LR_OPT_FFT_LENGTH = 8
 LR_OPT_PROJ_PATH = 9
+LR_OPT_Y_PRECISION = 10
+LR_Y_PLAIN, LR_Y_EXTENDED = 0, 1
 LR_INFO_TDI_PATH, LR_INFO_FIR_TAPS, LR_INFO_FIR_POWERS = 101, 102, 103
 LR_PROJ_AUTO, LR_PROJ_SINGLE, LR_PROJ_PAIR = -1, 1, 2
 LR_IP_CROSS, LR_IP_DIFF, LR_IP_BLOCKS = 0, 1, 1024

@@ -84,6 +84,7 @@ struct lr_handle {
   int tdi_path = -1;     // LR_OPT_TDI_PATH: -1 auto | 0 generic | 3 | 4
   int plan_cache = 1;    // LR_OPT_TDI_PLAN_CACHE
   int proj_path = LR_PROJ_AUTO;   // LR_OPT_PROJ_PATH
+  int y_precision = LR_Y_PLAIN;   // LR_OPT_Y_PRECISION
   int sm_count = 0;
   int64_t chunk_samples = 0;   // LR_OPT_CHUNK_SAMPLES: 0 = automatic
   int64_t fft_length = 0;      // LR_OPT_FFT_LENGTH: 0 = n (no zero padding)
@@ -157,6 +158,7 @@ lr::Params make_params(const lr_handle* h, int64_t n) {
   P.m_front = (int)h->m_front(h->gen);
   P.m_back = (int)h->m_back();
   P.chain_sum = h->chain == LR_CHAIN_SUM ? 1 : 0;
+  P.proj_ext = h->y_precision == LR_Y_EXTENDED ? 1 : 0;
   P.proj_pair = h->proj_path == LR_PROJ_PAIR ? 1 : 0;   // LR_PROJ_AUTO: one sample per thread (the faster one)
   memcpy(P.bk, h->bk, sizeof(P.bk));
   return P;
@@ -266,10 +268,21 @@ int lr_create(const lr_orbits* orb, double dt, int order, int tdi_gen, lr_handle
       if (orb->ltt[s * nk + k] != orb->ltt[s * nk]) { h->const_ltt = false; break; }
 
   std::vector<lr::D4> coef;
-  try { coef.resize((size_t)15 * (nk - 1)); } catch (...) { delete h; return LR_ENOMEM; }
+  try { coef.resize((size_t)lr::kSplineChannels * (nk - 1)); } catch (...) { delete h; return LR_ENOMEM; }
   try {
     for (int ch = 0; ch < 9; ++ch) lr::fit_channel(orb->x + (int64_t)ch * nk, nk, orb->knot_dt, coef.data() + (size_t)ch * (nk - 1));
     for (int s = 0; s < 6; ++s) lr::fit_channel(orb->ltt + (int64_t)s * nk, nk, orb->knot_dt, coef.data() + (size_t)(9 + s) * (nk - 1));
+    // channels 15..23: the three arm vectors x_i - x_j (arm a joins spacecraft a and (a+1)%3), splined from the exact
+    // differences of the table values.  The spline fit is linear in the table, so these ARE spline(x_i) - spline(x_j)
+    // -- but evaluated without the rounding of two ~1.5e11 m positions (LR_Y_EXTENDED)
+    std::vector<long double> dif((size_t)nk);
+    for (int arm = 0; arm < 3; ++arm)
+      for (int a = 0; a < 3; ++a) {
+        const double* xi = orb->x + ((int64_t)arm * 3 + a) * nk;
+        const double* xj = orb->x + ((int64_t)((arm + 1) % 3) * 3 + a) * nk;
+        for (int64_t k = 0; k < nk; ++k) dif[(size_t)k] = (long double)xi[k] - (long double)xj[k];
+        lr::fit_channel(dif.data(), nk, orb->knot_dt, coef.data() + (size_t)(15 + arm * 3 + a) * (nk - 1));
+      }
   } catch (...) { delete h; return LR_ENOMEM; }
 
   // largest light-time rate of the table: decides whether lr_tdi may treat the delays of a tile as a
@@ -359,6 +372,9 @@ int lr_set_option(lr_handle* h, int key, double value) {
       if (value != LR_TDI_AUTO && value != LR_TDI_PER_SAMPLE && value != LR_TDI_FIR3 && value != LR_TDI_FIR4)
         return LR_EINVAL;
       h->tdi_path = (int)value; return LR_OK;
+    case LR_OPT_Y_PRECISION:
+      if (value != LR_Y_PLAIN && value != LR_Y_EXTENDED) return LR_EINVAL;
+      h->y_precision = (int)value; return LR_OK;
     case LR_OPT_PROJ_PATH:
       if (value != LR_PROJ_AUTO && value != LR_PROJ_SINGLE && value != LR_PROJ_PAIR) return LR_EINVAL;
       h->proj_path = (int)value; return LR_OK;
@@ -384,6 +400,7 @@ int lr_get_option(const lr_handle* h, int key, double* value) {
     case LR_OPT_TDI_GEN: *value = h->gen; return LR_OK;
     case LR_OPT_TDI_PATH: *value = h->tdi_path; return LR_OK;
     case LR_OPT_PROJ_PATH: *value = h->proj_path; return LR_OK;
+    case LR_OPT_Y_PRECISION: *value = h->y_precision; return LR_OK;
     case LR_OPT_CHUNK_SAMPLES: *value = (double)h->chunk_samples; return LR_OK;
     case LR_OPT_FFT_LENGTH: *value = (double)h->fft_length; return LR_OK;
     case LR_OPT_TDI_PLAN_CACHE: *value = h->plan_cache; return LR_OK;
@@ -1127,7 +1144,7 @@ int64_t lr_fft_good_length(int64_t n) {
 }
 
 int lr_eval_orbit(lr_handle* h, int channel, const double* t, int64_t m, double* out, void* stream) {
-  if (!h || !t || !out || channel < 0 || channel > 14 || m < 1) return LR_EINVAL;
+  if (!h || !t || !out || channel < 0 || channel >= lr::kSplineChannels || m < 1) return LR_EINVAL;
   lr::Params P = make_params(h, 1);
   const int threads = 256;
   const int64_t blocks = (m + threads - 1) / threads;

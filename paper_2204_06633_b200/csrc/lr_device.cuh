@@ -29,6 +29,7 @@ namespace lr {
 
 constexpr int kPMax = 33;        // order <= 65
 constexpr double kC = 299792458.0;  // m/s
+constexpr int kSplineChannels = 24; // 9 positions, 6 light times, 9 arm-vector components (x_a - x_{a+1})
 
 struct alignas(16) D2 { double x, y; };
 struct alignas(32) D4 { double x, y, z, w; };
@@ -48,7 +49,7 @@ __host__ __device__ constexpr int rot_slot(int s, int r) {
 
 // Kernel parameters shared by both stages (passed by value).
 struct Params {
-  const D4* coef;      // DEVICE [15][nint] cubic coefficients (c0,c1,c2,c3) in u = (t - t_i)/h in [0,1)
+  const D4* coef;      // DEVICE [kSplineChannels][nint] cubic coefficients (c0,c1,c2,c3) in u = (t - t_i)/h in [0,1)
   int nint;            // spline intervals = n_knots - 1
   int p;               // P = (order+1)/2
   double trel0;        // t0 - t_start  [s]
@@ -70,6 +71,7 @@ struct Params {
   int fir_tile0;         // FIR path: global tile whose geometry plan slot 0 is built from
   int fir_taps;          // FIR path: taps per series that can be non-zero (<= fir_wc; the padding is at the front)
   int chain_sum;         // 0: nested delays (default), 1: eq. 20 sums of the L at t
+  int proj_ext;          // 1: LR_Y_EXTENDED (emission delays relative to the reception split, arm-vector splines)
   int proj_pair;         // 1: projection with two consecutive samples per thread (LR_PROJ_PAIR; same bits)
   double bk[kPMax + 1];  // bk[k] = 1 / prod_{m != k} (k - m), m = -P+1..P, for k = 1..P
 };
@@ -109,7 +111,7 @@ struct CoefGlobal {
   LR_HD D4 get(const Params& P, int ch, int i) const { return load4(P.coef + (int64_t)ch * P.nint + i); }
 };
 struct CoefTile {
-  const D4* sc;   // [15][2]
+  const D4* sc;   // [channels staged][2]
   int i0;
   LR_HD D4 get(const Params&, int ch, int i) const { return sc[ch * 2 + (i - i0)]; }
 };
@@ -281,29 +283,57 @@ LR_HD int clamp_anchor(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? h
 
 // One time sample of eqs. 10-16 for all six links.  raw/dif: staged (h+, hx) pairs and their first
 // differences, W entries; nl = this sample's staged index; bs = k(3), u(3), v(3).  y6[slot] receives y_ij.
-template <int PT, class Store, class Coef = CoefGlobal>
+//
+// EXT (LR_Y_EXTENDED): the same sample with the delays formed so that y is good to a few fp64 roundings instead of ~2e-14.
+// What limits the plain form is not the interpolation but the DELAYS: k.x_i/c is ~500 s (50-100 samples), so the
+// fp64 value of a delay carries 7e-15 samples of rounding, and Delta h = h(t_e) - h(t_r) with t_e - t_r ~ 1 sample sees
+// it as a relative error of 1e-14 (which TDI then amplifies by up to 1e6 in the T channel).  Here
+//   * the arm vectors x_i - x_j come from their own splines (channels 15..23, fitted to the exact differences of the
+//     table values: the same function, without the rounding of two 1.5e11 m positions); only spacecraft 1 is located
+//     by its position spline, k.x_2/c and k.x_3/c follow from the arm vectors (18 spline evaluations per sample), and
+//   * an emission time is placed RELATIVE to its reception time: with D_r = I_r - eps_r split exactly,
+//     D_e - D_r = L_ij/dt -+ k.(x_i - x_j)/(c dt) =: dD is a small number known to ~1e-16 samples, and
+//     u = dD - eps_r, I_e = I_r + ceil(u), eps_e = ceil(u) - u.  The rounding of D_r itself then moves BOTH times
+//     together, which changes Delta h by w dt * 7e-15 only.
+template <int PT, bool EXT, class Store, class Coef = CoefGlobal>
 LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W, int nl, double trel,
                           const double* bs, Store store, const Coef& coef = Coef{}) {
   // geometry first (everything that needs the positions and the basis), so that only 12 doubles stay live
   // across the nine interpolations: Dr[3] and, per arm, xi+, xix, k.n
   double Dr[3], xip[3], xic[3], kn[3], rden[3];
+  double kd[EXT ? 3 : 1];   // EXT: k.(x_i - x_j)/c [samples] per arm
   {
     const double k0 = bs[0], k1 = bs[1], k2 = bs[2];
     const double u0 = bs[3], u1 = bs[4], u2 = bs[5];
     const double v0 = bs[6], v1 = bs[7], v2 = bs[8];
     double x[3][3];
+    if constexpr (EXT) {   // reception delay of spacecraft 1 from its position; the other two follow from the arms
 #pragma unroll
-    for (int i = 0; i < 3; ++i) {
+      for (int a = 0; a < 3; ++a) x[0][a] = spline_eval(prm, coef, a, trel);
+      Dr[0] = (k0 * x[0][0] + k1 * x[0][1] + k2 * x[0][2]) * prm.inv_cdt;
+    } else {
 #pragma unroll
-      for (int a = 0; a < 3; ++a) x[i][a] = spline_eval(prm, coef, i * 3 + a, trel);
-      Dr[i] = (k0 * x[i][0] + k1 * x[i][1] + k2 * x[i][2]) * prm.inv_cdt;   // reception delay k.x_i/c [samples]
+      for (int i = 0; i < 3; ++i) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) x[i][a] = spline_eval(prm, coef, i * 3 + a, trel);
+        Dr[i] = (k0 * x[i][0] + k1 * x[i][1] + k2 * x[i][2]) * prm.inv_cdt;   // reception delay k.x_i/c [samples]
+      }
     }
     // three arms: arm a joins receiver i = a and emitter j = (a+1)%3 (links 12, 23, 31); the reverse links
     // 21, 32, 13 share xi+ and xix and flip the sign of k.n
 #pragma unroll
     for (int arm = 0; arm < 3; ++arm) {
       const int i = arm, j = (arm + 1) % 3;
-      const double d0 = x[i][0] - x[j][0], d1 = x[i][1] - x[j][1], d2 = x[i][2] - x[j][2];
+      double d0, d1, d2;
+      if constexpr (EXT) {
+        d0 = spline_eval(prm, coef, 15 + arm * 3, trel);
+        d1 = spline_eval(prm, coef, 16 + arm * 3, trel);
+        d2 = spline_eval(prm, coef, 17 + arm * 3, trel);
+        kd[arm] = (k0 * d0 + k1 * d1 + k2 * d2) * prm.inv_cdt;
+        if (arm < 2) Dr[arm + 1] = Dr[arm] - kd[arm];   // k.x_j/c = k.x_i/c - k.(x_i - x_j)/c
+      } else {
+        d0 = x[i][0] - x[j][0]; d1 = x[i][1] - x[j][1]; d2 = x[i][2] - x[j][2];
+      }
       const double inv = inv_sqrt(d0 * d0 + d1 * d1 + d2 * d2);
       const double n0v = d0 * inv, n1v = d1 * inv, n2v = d2 * inv;  // emitter j -> receiver i
       const double un = u0 * n0v + u1 * n1v + u2 * n2v;
@@ -333,8 +363,9 @@ LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W
   for (int i = 0; i < 3; ++i) {
     double eps;
     split_delay(Dr[i], nl, ar[i], eps);
-    ar[i] = clampi(ar[i], a_min, a_max);
+    ar[i] = clampi(ar[i], a_min, a_max);   // (only ever moves the anchor of a sample inside the margins: zeroed)
     interp_sbp<PT, 2>(prm, eps, ar[i], fetch, Sr[i]);
+    if constexpr (EXT) Dr[i] = eps;        // from here on Dr[i] holds the FRACTION of the reception split
   }
 
 #pragma unroll
@@ -345,11 +376,13 @@ LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W
       const int rx = dir == 0 ? i : j, tx = dir == 0 ? j : i;
       const int slot = link_slot(rx, tx);
       const double kappa = dir == 0 ? kn[arm] : -kn[arm];
-      // emission: t - L_rx,tx(t) - k.x_tx(t)/c
-      const double De = fma(spline_eval(prm, coef, 9 + slot, trel), prm.inv_dt, Dr[tx]);
+      // emission: t - L_rx,tx(t) - k.x_tx(t)/c.  EXT: relative to the reception split, D_e - D_r = L/dt +
+      // k.(x_tx - x_rx)/(c dt) with x_tx - x_rx = -(x_i - x_j) for link ij and +(x_i - x_j) for link ji
+      const double De = EXT ? fma(spline_eval(prm, coef, 9 + slot, trel), prm.inv_dt, dir == 0 ? -kd[EXT ? arm : 0] : kd[EXT ? arm : 0]) - Dr[rx]
+                            : fma(spline_eval(prm, coef, 9 + slot, trel), prm.inv_dt, Dr[tx]);
       int ae;
       double eps, Se[2];
-      split_delay(De, nl, ae, eps);
+      split_delay(De, EXT ? ar[rx] - 1 : nl, ae, eps);
       ae = clampi(ae, a_min, a_max);
       interp_sbp<PT, 2>(prm, eps, ae, fetch, Se);
       const D2 re = raw[ae], rr = raw[ar[rx]];

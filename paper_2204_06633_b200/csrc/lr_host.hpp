@@ -13,7 +13,8 @@ namespace lr {
 //   s_0 + 2 s_1 = (-5 y_0 + 4 y_1 + y_2) / (2h),   2 s_{n-2} + s_{n-1} = (5 y_{n-1} - 4 y_{n-2} - y_{n-3}) / (2h)
 // (the end rows are the interior row combined with continuity of the third derivative at knots 1 and n-2).
 // Writes the per-interval coefficients of c0 + c1 u + c2 u^2 + c3 u^3, u = (t - t_i)/h.
-inline void fit_channel(const double* y, int64_t n, double h_, lr::D4* out) {
+template <class In>
+inline void fit_channel(const In* y, int64_t n, double h_, lr::D4* out) {
   typedef long double R;
   const R h = (R)h_;
   std::vector<R> dg(n), up(n), rhs(n), s(n);
@@ -36,7 +37,7 @@ inline void fit_channel(const double* y, int64_t n, double h_, lr::D4* out) {
   for (int64_t i = n - 2; i >= 0; --i) s[i] = (rhs[i] - up[i] * s[i + 1]) / dg[i];
   for (int64_t i = 0; i + 1 < n; ++i) {
     const R dy = (R)y[i + 1] - (R)y[i];
-    out[i].x = y[i];
+    out[i].x = (double)y[i];
     out[i].y = (double)(h * s[i]);
     out[i].z = (double)((R)3 * dy - h * ((R)2 * s[i] + s[i + 1]));
     out[i].w = (double)(-(R)2 * dy + h * (s[i] + s[i + 1]));

@@ -29,7 +29,7 @@ int launch_project_t(const Params& prm, const double* hp, const double* hc, cons
   if (e != cudaSuccess) return (int)e;
   const int64_t grid = (int64_t)prm.ntiles * batch;
   if constexpr (proj_pairs(PT)) {
-    if (prm.proj_pair) {
+    if (prm.proj_pair && !prm.proj_ext) {
       const size_t smem2 = proj_pair_smem((int)W);
       if ((e = prepare(project_pair_kernel<PT>, smem2)) != cudaSuccess) return (int)e;
       project_pair_kernel<PT><<<(unsigned)grid, kProjPairThreads, smem2, (cudaStream_t)stream>>>(prm, hp, hc, basis, y);
@@ -37,7 +37,12 @@ int launch_project_t(const Params& prm, const double* hp, const double* hc, cons
       return (int)cudaGetLastError();
     }
   }
-  project_kernel<PT><<<(unsigned)grid, kProjThreads, smem, (cudaStream_t)stream>>>(prm, hp, hc, basis, y);
+  if (prm.proj_ext) {
+    if ((e = prepare(project_kernel<PT, true>, smem)) != cudaSuccess) return (int)e;
+    project_kernel<PT, true><<<(unsigned)grid, kProjThreads, smem, (cudaStream_t)stream>>>(prm, hp, hc, basis, y);
+  } else {
+    project_kernel<PT><<<(unsigned)grid, kProjThreads, smem, (cudaStream_t)stream>>>(prm, hp, hc, basis, y);
+  }
   g_launches.fetch_add(1);
   return (int)cudaGetLastError();
 }

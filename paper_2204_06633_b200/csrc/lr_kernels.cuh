@@ -33,7 +33,8 @@ __host__ __device__ constexpr int tdi_min_blocks(int PT) { return PT == 0 ? 2 : 
 // ---------------------------------------------------------------------------------------------- stage 1
 // grid.x = ntiles * batch; tile = blockIdx.x % ntiles, template = blockIdx.x / ntiles.
 // dynamic smem: D2 raw[W], D2 dif[W] with W = kProjThreads + halo_lo + halo_hi  (x = h+, y = hx)
-template <int PT>
+// EXT: LR_Y_EXTENDED (24 spline channels, emission delays relative to the reception split: project_sample<PT, true>)
+template <int PT, bool EXT = false>
 __global__ void __launch_bounds__(kProjThreads, proj_min_blocks(PT))
 project_kernel(const Params prm, const double* __restrict__ hp, const double* __restrict__ hc,
                const double* __restrict__ basis /* [batch][9] */, double* __restrict__ y) {
@@ -51,14 +52,15 @@ project_kernel(const Params prm, const double* __restrict__ hp, const double* __
 
   // the samples of a tile fall in one or two spline intervals (knots are hours apart): their coefficients
   // go to shared memory, so that no evaluation in project_sample waits on a global load
-  __shared__ D4 sc[15 * 2];
+  constexpr int NCH = EXT ? kSplineChannels : 15;   // spline channels this kernel evaluates
+  __shared__ D4 sc[NCH * 2];
   double u_unused;
   const int n_last = n0 + kProjThreads - 1 < prm.n - 1 ? n0 + kProjThreads - 1 : prm.n - 1;
   const int i_lo = spline_interval(prm, sample_trel(prm, prm.n_off + n0), u_unused);
   const int i_hi = spline_interval(prm, sample_trel(prm, prm.n_off + n_last), u_unused);
   // (measured: orders <= 25 gain 2 %, orders 31 and 41 lose 3-4 % -- their shared-memory pipe is the fuller one)
   const bool tile_coef = PT > 0 && PT <= 13 && i_hi - i_lo <= 1;   // (block-uniform)
-  if (tile_coef && threadIdx.x < 30) {
+  if (tile_coef && threadIdx.x < 2 * NCH && !(EXT && threadIdx.x >= 6 && threadIdx.x < 18)) {   // (EXT: x_2, x_3 unused)
     const int ch = threadIdx.x >> 1, i = i_lo + (threadIdx.x & 1);
     sc[threadIdx.x] = load4(prm.coef + (int64_t)ch * prm.nint + (i < prm.nint ? i : prm.nint - 1));
   }
@@ -90,9 +92,9 @@ project_kernel(const Params prm, const double* __restrict__ hp, const double* __
   const int64_t os = prm.out_stride;
   auto store = [&](int slot, double v) { yb[slot * os] = v; };
   if (tile_coef)
-    project_sample<PT>(prm, raw, dif, W, n - g0, sample_trel(prm, ng), bs, store, CoefTile{sc, i_lo});
+    project_sample<PT, EXT>(prm, raw, dif, W, n - g0, sample_trel(prm, ng), bs, store, CoefTile{sc, i_lo});
   else
-    project_sample<PT>(prm, raw, dif, W, n - g0, sample_trel(prm, ng), bs, store, CoefGlobal{});
+    project_sample<PT, EXT>(prm, raw, dif, W, n - g0, sample_trel(prm, ng), bs, store, CoefGlobal{});
 }
 
 // Two consecutive samples per thread (project_pair): the same tile, staging and results as project_kernel with half

@@ -94,6 +94,10 @@ class Response:
         B.lr_set_option(self._h, B.LR_OPT_PROJ_PATH, {"auto": B.LR_PROJ_AUTO, "single": B.LR_PROJ_SINGLE,
                                                       "pair": B.LR_PROJ_PAIR}[path])
 
+    def set_y_precision(self, mode):
+        """"plain" | "extended" (LR_OPT_Y_PRECISION)."""
+        B.lr_set_option(self._h, B.LR_OPT_Y_PRECISION, {"plain": B.LR_Y_PLAIN, "extended": B.LR_Y_EXTENDED}[mode])
+
     def create_plan(self, n, stream=None):
         """A shareable read-only TDI plan for this handle's options and a series of n samples (lr_plan_create)."""
         return B.lr_plan_create(self._h, n, stream)

@@ -350,6 +350,84 @@ def test_project_pair_path_bitwise(lr, order):
         assert_parity(outs["pair"][0][0][:, mp:mp + 3000], yo[:, mp:mp + 3000], "pair path", LINK_NAMES)
 
 
+# ------------------------------------------------------------------------- LR_Y_EXTENDED (NEXT-1)
+@pytest.mark.parametrize("f0", [1e-4, 1e-3, 1e-2])
+def test_extended_y_end_to_end(lr, f0):
+    """LR_OPT_Y_PRECISION = LR_Y_EXTENDED (the accuracy half of the fused row; PAPER.md:181
+    eq. 16 and 193-197 eqs. 17-18 for the cancellations involved).  The end-to-end error of the path (GPU h -> out
+    against the ALL-long-double oracle pipeline) is set by y: TDI amplifies errors of y by up to 1e6 in T at 0.1 mHz.
+    With the emission delays placed relative to the reception split and the arm vectors splined directly, y agrees
+    with the oracle to a few 1e-16 (plain: 2.4e-14) and end-to-end T is <= 1e-9 at 0.1 mHz and <= 1e-10 from 1 mHz
+    (plain: 2.2e-8 and 2.2e-10); measured round 2: 7.8e-10, 8.1e-12, 1.8e-13 beside an fp64-y floor of 6.3e-11,
+    6.8e-13, 3.6e-15.  The plain path is untouched (same kernel instantiation as before)."""
+    w = inputs.config(2, n=20011, f0=f0, t0=3.0e7)
+    tab = w.table()
+    s = w.sources[0]
+    hp, hc = w.waveform(0)
+    O = orc.Oracle(tab, w.dt, w.t0, w.order)
+    yo = O.project(hp, hc, s.beta, s.lam, s.psi)
+    o_ld = O.tdi(yo, 2, nested=True, channels=orc.CH_XYZ_AET)          # long-double y into long-double TDI
+    errs = {}
+    for mode in ("plain", "extended"):
+        R = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="XYZ_AET")
+        R.set_y_precision(mode)
+        mp, mf, mb = R.margins()
+        y = R.project(to_dev(hp)[None], to_dev(hc)[None], [s.beta], [s.lam], [s.psi])
+        yh = y.cpu().numpy()[0]
+        assert not yh[:, :mp].any() and not yh[:, w.n - mp:].any()
+        ey = assert_parity(yh[:, mp:w.n - mp], yo[:, mp:w.n - mp], f"project ({mode})", LINK_NAMES)
+        out = R.tdi(y).cpu().numpy()[0]
+        from parity_util import channel_errors
+        e2e = [channel_errors(out[c, mf:w.n - mb], o_ld[c, mf:w.n - mb]) for c in range(6)]
+        errs[mode] = (max(r for r, _ in ey), e2e)
+        if mode == "extended":
+            one = R.response(to_dev(hp)[None], to_dev(hc)[None], [s.beta], [s.lam], [s.psi]).cpu().numpy()[0]
+            assert np.array_equal(one, out)                               # the one-call path takes the option too
+    y_plain, y_ext = errs["plain"][0], errs["extended"][0]
+    assert y_ext <= 5e-15 and y_ext < 0.3 * y_plain, (y_plain, y_ext)
+    t_rel = errs["extended"][1][5][0]
+    assert t_rel <= (1e-9 if f0 < 5e-4 else 1e-10), t_rel
+    assert t_rel < 0.2 * errs["plain"][1][5][0]
+    for c in range(5):                                                    # X, Y, Z, A, E end to end
+        assert errs["extended"][1][c][0] <= 1e-11
+
+
+@pytest.mark.parametrize("cfg,kw", [(1, {}), (3, {"batch": 3, "n": 9001}), (4, {"n": 12345, "t0": 5.0e7}),
+                                    (5, {"n": 20001})])
+def test_extended_y_parity_other_configs(lr, cfg, kw):
+    """LR_Y_EXTENDED per call on the other configs' orbits and orders (equal-arm, Keplerian batch, perturbed orbits at
+    order 41, chirp): lr_project within 1e-14 of the oracle per link, and the chunked one-call path bit-identical."""
+    import torch
+    w = inputs.config(cfg, **kw)
+    tab = w.table()
+    idx = range(len(w.sources))
+    hp, hc = _stack(w, idx)
+    be, la, ps = ([getattr(s, k) for s in w.sources] for k in ("beta", "lam", "psi"))
+    R = lr.Response(tab, w.dt, w.order, w.tdi_gen, t0=w.t0, channels=w.channels)
+    R.set_y_precision("extended")
+    O = orc.Oracle(tab, w.dt, w.t0, w.order)
+    mp, mf, mb = R.margins()
+    y = R.project(to_dev(hp), to_dev(hc), be, la, ps)
+    yh = y.cpu().numpy()
+    for k in idx:
+        yo = O.project(hp[k], hc[k], be[k], la[k], ps[k])
+        assert_parity(yh[k][:, mp:w.n - mp], yo[:, mp:w.n - mp], f"config {cfg} extended b={k}", LINK_NAMES,
+                      rel_tol=1e-14, abs_tol=1e-13)
+    ref = R.tdi(y).cpu().numpy()
+    lr.lr_set_option(R.handle, lr.LR_OPT_CHUNK_SAMPLES, 1792)
+    assert np.array_equal(R.response(to_dev(hp), to_dev(hc), be, la, ps).cpu().numpy(), ref)
+    oo = O.tdi(yh[0], w.tdi_gen, nested=True, channels=ORC_CH[w.channels])
+    assert_parity(ref[0][:, mf:w.n - mb], oo[:, mf:w.n - mb], f"config {cfg} tdi of extended y", CH_NAMES[w.channels])
+    # the arm-vector splines are the differences of the position splines (the fit is linear in the table)
+    t = to_dev(np.linspace(w.t0 + 10 * w.dt, w.t0 + (w.n - 10) * w.dt, 257))
+    ev = lambda ch: lr.lr_eval_orbit(R.handle, ch, t, torch.empty_like(t)).cpu().numpy()
+    for arm in range(3):
+        for a in range(3):
+            d = ev(15 + arm * 3 + a)
+            assert np.abs(d - (ev(arm * 3 + a) - ev(((arm + 1) % 3) * 3 + a))).max() <= 1e-4     # metres (ulp of 1 au: 3e-5)
+            assert np.abs(d).max() < 3.2e9
+
+
 # ---------------------------------------------------------------------------------------------- pins
 @pytest.mark.parametrize("knot_dt", [400.0, 1000.0, 1290.0])
 def test_dense_orbit_knots(lr, knot_dt):
