@@ -64,15 +64,15 @@ project_kernel(const Params prm, const double* __restrict__ hp, const double* __
     const int ch = threadIdx.x >> 1, i = i_lo + (threadIdx.x & 1);
     sc[threadIdx.x] = load4(prm.coef + (int64_t)ch * prm.nint + (i < prm.nint ? i : prm.nint - 1));
   }
+  // one pass, one barrier: every element's successor is loaded too (it hits L1) and the first difference is formed
+  // in registers
   for (int m = threadIdx.x; m < W; m += kProjThreads) {
     const int g = g0 + m;
-    D2 v{0.0, 0.0};
+    D2 v{0.0, 0.0}, v1{0.0, 0.0};
     if (g >= prm.rd_lo && g < prm.rd_hi) { v.x = __ldg(hpb + g); v.y = __ldg(hcb + g); }
+    if (g + 1 >= prm.rd_lo && g + 1 < prm.rd_hi && m + 1 < W) { v1.x = __ldg(hpb + g + 1); v1.y = __ldg(hcb + g + 1); }
     raw[m] = v;
-  }
-  __syncthreads();
-  for (int m = threadIdx.x; m < W - 1; m += kProjThreads) {
-    dif[m] = D2{raw[m + 1].x - raw[m].x, raw[m + 1].y - raw[m].y};
+    if (m + 1 < W) dif[m] = D2{v1.x - v.x, v1.y - v.y};
   }
   __syncthreads();
 
