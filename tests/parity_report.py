@@ -26,10 +26,13 @@ def fmt(errs):
     return " ".join(f"{r:.1e}/{m:.1e}" for r, m in errs)
 
 
-def report(name, w, lr, chain="nested", tab=None):
+def report(name, w, lr, chain="nested", tab=None, y_precision="plain"):
     tab = tab or w.table()
     n, gen, ch = w.n, w.tdi_gen, "XYZ_AET"
     R = lr.Response(tab, w.dt, w.order, gen, t0=w.t0, chain=chain, channels=ch)
+    R.set_y_precision(y_precision)
+    if y_precision != "plain":
+        name += f", LR_Y_{y_precision.upper()}"
     O = orc.Oracle(tab, w.dt, w.t0, w.order)
     mp, mf, mb = R.margins()
     s = w.sources[0]
@@ -73,9 +76,13 @@ def main():
     for f0 in (None, 1e-4, 1e-3, 1e-2):
         for chain in ("nested", "sum"):
             worst = max(worst, report("config 2 year (shortened)", inputs.config(2, n=20011, f0=f0, t0=3.0e7), lr, chain))
+        worst = max(worst, report("config 2 year (shortened)", inputs.config(2, n=20011, f0=f0, t0=3.0e7), lr,
+                                  y_precision="extended"))
     worst = max(worst, report("config 3 batch, template 0 (shortened)", inputs.config(3, batch=1, n=20011), lr))
     for f0 in (None, 1e-4):
-        worst = max(worst, report("config 4 numerical-style orbits (shortened)", inputs.config(4, n=12345, t0=5.0e7, f0=f0), lr))
+        for yp in ("plain", "extended"):
+            worst = max(worst, report("config 4 numerical-style orbits (shortened)",
+                                      inputs.config(4, n=12345, t0=5.0e7, f0=f0), lr, y_precision=yp))
     full = inputs.config(5)
     n = 30001
     w5 = inputs.config(5, n=n, t0=full.t0 + (full.n - n) * full.dt)
