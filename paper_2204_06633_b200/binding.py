@@ -152,11 +152,14 @@ def lr_create(table, dt, lagrange_order, tdi_gen):
 
 
 def lr_destroy(h):
+    _N_OUT.pop(h.value if hasattr(h, "value") else int(h), None)
     lib().lr_destroy(h)
 
 
 def lr_set_option(h, key, value):
     _check(lib().lr_set_option(h, int(key), float(value)), "lr_set_option", h)
+    if int(key) == LR_OPT_CHANNELS:
+        _N_OUT.pop(h.value if hasattr(h, "value") else int(h), None)
 
 
 def lr_get_option(h, key):
@@ -165,9 +168,16 @@ def lr_get_option(h, key):
     return v.value
 
 
+_N_OUT = {}   # handle address -> rows per template, kept in step by lr_set_option / lr_destroy (saves a call per launch)
+
+
 def _n_out(h):
     """Rows per template lr_tdi writes with this handle's LR_OPT_CHANNELS (the C ABI takes no size for `out`)."""
-    return 6 if int(lr_get_option(h, LR_OPT_CHANNELS)) == LR_XYZ_AET else 3
+    key = h.value if hasattr(h, "value") else int(h)
+    n = _N_OUT.get(key)
+    if n is None:
+        n = _N_OUT[key] = 6 if int(lr_get_option(h, LR_OPT_CHANNELS)) == LR_XYZ_AET else 3
+    return n
 
 
 def _angles(beta, lam, psi):
