@@ -64,6 +64,10 @@ struct FirTile {
 };
 
 // A: chain delays at the nodes.  x0 = sample index of the tile's first sample, B = tile length.
+// (The nodes of the first and last partly valid tiles can lie inside the margins, i.e. up to one tile outside the
+// span lr_tdi checked against the knot table; spline_interval clamps the interval index there, which extrapolates the
+// end cubic by at most 224 samples.  Only the polynomial fit over the tile sees those nodes: the valid samples of the
+// tile lie inside the table, and the fit of a smooth cubic is exact wherever its nodes are.)
 template <int GEN, int NN>
 LR_HD void fir_chain_nodes(const Params& prm, FirTile<GEN, NN>& T, int n0, int B, int tid, int nthreads) {
   constexpr int NK = FirTile<GEN, NN>::NK;
