@@ -345,6 +345,7 @@ def workload_config(w, batch, args):
             "batch": batch, "n": w.n, "dt": w.dt, "lagrange_order": w.order,
             "tdi_gen": 1 if args.workload == "hybrid" else w.tdi_gen,
             "chain": "nested", "channels": w.channels, "orbits": w.orbit_kind, "tdi_path": args.tdi_path,
+            "y_precision": args.y_precision,
             "tdi_plan": "cached (built once per handle, like the paper's orbit arrays, PAPER.md:263; the `tdi_plan` key "
                         "has the step with the plan rebuilt in every call)",
             "l2": "flushed between steps (256 MiB memset outside the per-step event pairs)"}
@@ -519,6 +520,7 @@ def run_gpu(args, rank, world, local_rank):
     nout = 6 if w.channels == "XYZ_AET" else 3
     R = lr.Response(w.table(), w.dt, w.order, w.tdi_gen, t0=w.t0, chain="nested", channels=w.channels,
                     tdi_path=args.tdi_path)
+    R.set_y_precision(args.y_precision)
     Rt, tdi_gen = R, w.tdi_gen
     if args.workload == "hybrid":
         from harness import inputs as _inp
@@ -733,7 +735,7 @@ def run_gpu(args, rank, world, local_rank):
     templates = sum_over_ranks(float(batch))
 
     # end to end through the C ABI with pinned HOST buffers (H2D + project + TDI + D2H inside the timed region)
-    eb = min(batch, args.e2e_templates)
+    eb = min(batch, chunk if args.workload == "batch" else args.e2e_templates)   # batch: one whole launch chunk
     hp_h = torch.empty((eb, n), dtype=torch.float64).pin_memory()
     hc_h = torch.empty((eb, n), dtype=torch.float64).pin_memory()
     out_h = torch.empty((eb, nout, n), dtype=torch.float64).pin_memory()
@@ -907,6 +909,8 @@ def main():
     ap.add_argument("--peak-seconds", type=float, default=1.0)
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--y-precision", default="extended", choices=["extended", "plain"],
+                    help="LR_OPT_Y_PRECISION of lr_project (the library's default is extended)")
     ap.add_argument("--no-batch-leg", action="store_true", help="skip the 64-template launch of configs[2]")
     ap.add_argument("--no-orders-leg", action="store_true", help="skip the Lagrange-order sweep")
     ap.add_argument("--tdi-path", default="auto", choices=["auto", "per_sample", "fir3", "fir4"])

@@ -64,16 +64,17 @@ typedef struct {
 #define LR_OPT_FFT_LENGTH 8 /* transform length of lr_loglike_gb (>= n, zero padded); 0 (default) = n */
 #define LR_OPT_TDI_PLAN_CACHE 6 /* 1 (default): keep the FIR plan between lr_tdi calls; 0: rebuild every call */
 #define LR_OPT_PROJ_PATH 9 /* LR_PROJ_AUTO (default) | LR_PROJ_SINGLE | LR_PROJ_PAIR */
-#define LR_OPT_Y_PRECISION 10 /* LR_Y_PLAIN (default) | LR_Y_EXTENDED */
+#define LR_OPT_Y_PRECISION 10 /* LR_Y_EXTENDED (default) | LR_Y_PLAIN */
 
 /* How lr_project forms the delayed times (the end-to-end accuracy of the path).
+ * The same eq. 16 either way; the difference is where fp64 rounding enters.
  *   LR_Y_PLAIN    : every delay is an fp64 number of samples (t - k.x_i/c is ~50-100 samples away: 7e-15 samples of
- *                   rounding), y agrees with the long-double oracle to ~2e-14.
+ *                   rounding), y agrees with the long-double oracle to ~2e-14 (the round-1 kernel, bit for bit).
  *   LR_Y_EXTENDED : the emission time of a link is placed relative to the split (integer, fraction) of its reception
  *                   time, from L_ij/dt and k.(x_i - x_j)/(c dt) with the arm vectors x_i - x_j splined from the exact
- *                   differences of the table; y agrees with the oracle to a few 1e-16, and the end-to-end T channel
- *                   (which amplifies errors of y by up to 1e6 at 0.1 mHz) improves by the same factor.  Costs a few
- *                   per cent of lr_project; runs the one-sample-per-thread kernel. */
+ *                   differences of the table; y agrees with the oracle to ~1e-15, and the end-to-end T channel
+ *                   (which amplifies errors of y by up to 1e6 at 0.1 mHz) improves by the same factor.  Costs 2 % of
+ *                   lr_project and is the default; runs the one-sample-per-thread kernel. */
 #define LR_Y_PLAIN 0
 #define LR_Y_EXTENDED 1
 

@@ -84,7 +84,7 @@ struct lr_handle {
   int tdi_path = -1;     // LR_OPT_TDI_PATH: -1 auto | 0 generic | 3 | 4
   int plan_cache = 1;    // LR_OPT_TDI_PLAN_CACHE
   int proj_path = LR_PROJ_AUTO;   // LR_OPT_PROJ_PATH
-  int y_precision = LR_Y_PLAIN;   // LR_OPT_Y_PRECISION
+  int y_precision = LR_Y_EXTENDED;   // LR_OPT_Y_PRECISION
   int sm_count = 0;
   int64_t chunk_samples = 0;   // LR_OPT_CHUNK_SAMPLES: 0 = automatic
   int64_t fft_length = 0;      // LR_OPT_FFT_LENGTH: 0 = n (no zero padding)

@@ -356,38 +356,36 @@ LR_HD void project_sample(const Params& prm, const D2* raw, const D2* dif, int W
   const int a_min = PT > 0 ? PT : prm.p, a_max = W - (PT > 0 ? PT : prm.p);
   auto clampi = [](int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); };
 
-  // reception: h at t - k.x_i/c for the three receivers (each shared by the two links it receives)
-  double Sr[3][2];
-  int ar[3];
+  // receiver by receiver: h at the reception time t - k.x_i/c (shared by the two links received at i), then the two
+  // emission times of those links; only one receiver's reception sums are live at a time
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    double eps;
-    split_delay(Dr[i], nl, ar[i], eps);
-    ar[i] = clampi(ar[i], a_min, a_max);   // (only ever moves the anchor of a sample inside the margins: zeroed)
-    interp_sbp<PT, 2>(prm, eps, ar[i], fetch, Sr[i]);
-    if constexpr (EXT) Dr[i] = eps;        // from here on Dr[i] holds the FRACTION of the reception split
-  }
-
+    double Sr[2], er;
+    int ar;
+    split_delay(Dr[i], nl, ar, er);
+    ar = clampi(ar, a_min, a_max);   // (only ever moves the anchor of a sample inside the margins: zeroed)
+    interp_sbp<PT, 2>(prm, er, ar, fetch, Sr);
+    const D2 rr = raw[ar];
 #pragma unroll
-  for (int arm = 0; arm < 3; ++arm) {
-    const int i = arm, j = (arm + 1) % 3;
-#pragma unroll
-    for (int dir = 0; dir < 2; ++dir) {
-      const int rx = dir == 0 ? i : j, tx = dir == 0 ? j : i;
-      const int slot = link_slot(rx, tx);
-      const double kappa = dir == 0 ? kn[arm] : -kn[arm];
+    for (int l = 0; l < 2; ++l) {
+      // the links received at i: from j = (i+1)%3 (slot i: arm i, direction ij) and from (i+2)%3 (the reverse link of
+      // arm (i+2)%3)
+      const int arm = l == 0 ? i : (i + 2) % 3;
+      const int tx = l == 0 ? (i + 1) % 3 : (i + 2) % 3;
+      const int slot = link_slot(i, tx);
+      const double kappa = l == 0 ? kn[arm] : -kn[arm];
       // emission: t - L_rx,tx(t) - k.x_tx(t)/c.  EXT: relative to the reception split, D_e - D_r = L/dt +
-      // k.(x_tx - x_rx)/(c dt) with x_tx - x_rx = -(x_i - x_j) for link ij and +(x_i - x_j) for link ji
-      const double De = EXT ? fma(spline_eval(prm, coef, 9 + slot, trel), prm.inv_dt, dir == 0 ? -kd[EXT ? arm : 0] : kd[EXT ? arm : 0]) - Dr[rx]
+      // k.(x_tx - x_rx)/(c dt) with x_tx - x_rx = -(x_a - x_b) for the link ab of arm ab and +(x_a - x_b) for link ba
+      const double De = EXT ? fma(spline_eval(prm, coef, 9 + slot, trel), prm.inv_dt, l == 0 ? -kd[EXT ? arm : 0] : kd[EXT ? arm : 0]) - er
                             : fma(spline_eval(prm, coef, 9 + slot, trel), prm.inv_dt, Dr[tx]);
       int ae;
       double eps, Se[2];
-      split_delay(De, EXT ? ar[rx] - 1 : nl, ae, eps);
+      split_delay(De, EXT ? ar - 1 : nl, ae, eps);
       ae = clampi(ae, a_min, a_max);
       interp_sbp<PT, 2>(prm, eps, ae, fetch, Se);
-      const D2 re = raw[ae], rr = raw[ar[rx]];
-      const double dhp = (re.x - rr.x) - Se[0] + Sr[rx][0];
-      const double dhc = (re.y - rr.y) - Se[1] + Sr[rx][1];
+      const D2 re = raw[ae];
+      const double dhp = (re.x - rr.x) - Se[0] + Sr[0];
+      const double dhc = (re.y - rr.y) - Se[1] + Sr[1];
       store(slot, (xip[arm] * dhp + xic[arm] * dhc) * ((1.0 + kappa) * rden[arm]));  // eq. 16: / (2 (1 - kappa))
     }
   }

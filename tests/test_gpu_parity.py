@@ -336,13 +336,19 @@ def test_project_pair_path_bitwise(lr, order):
     outs = {}
     for path in ("single", "pair"):
         R = lr.Response(w.table(), w.dt, order, 2, t0=w.t0)
+        R.set_y_precision("plain")      # the pair kernel implements the plain delay form
         R.set_proj_path(path)
         y = R.project(hpd, hcd, be, la, ps)
         lr.lr_set_option(R.handle, lr.LR_OPT_CHUNK_SAMPLES, 1792 * 2)    # chunks whose y window starts at a - halo
         outs[path] = (y.cpu().numpy(), R.response(hpd, hcd, be, la, ps).cpu().numpy())
     assert np.array_equal(outs["single"][0], outs["pair"][0])
     assert np.array_equal(outs["single"][1], outs["pair"][1])
-    mp = lr.Response(w.table(), w.dt, order, 2, t0=w.t0).margins()[0]
+    Rx = lr.Response(w.table(), w.dt, order, 2, t0=w.t0)
+    Rx.set_proj_path("pair")            # with the default LR_Y_EXTENDED the option is accepted and runs the single kernel
+    assert lr.lr_get_option(Rx.handle, lr.LR_OPT_Y_PRECISION) == lr.LR_Y_EXTENDED
+    yx = Rx.project(hpd, hcd, be, la, ps).cpu().numpy()
+    assert np.abs(yx - outs["single"][0]).max() <= 1e-12 * np.abs(yx).max()
+    mp = Rx.margins()[0]
     assert np.count_nonzero(outs["pair"][0][:, :, mp:w.n - mp]) > 0.99 * 18 * (w.n - 2 * mp)
     if order == 25:   # template 0 against the oracle, through the pair path
         O = orc.Oracle(w.table(), w.dt, w.t0, order)
