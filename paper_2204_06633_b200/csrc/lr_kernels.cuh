@@ -27,7 +27,8 @@ __host__ __device__ constexpr size_t proj_pair_smem(int W) {
 }
 // orders whose projection runs two samples per thread (compile-time P; the run-time-P build keeps one)
 __host__ __device__ constexpr bool proj_pairs(int PT) { return PT >= 1; }
-__host__ __device__ constexpr int proj_min_blocks(int PT) { return PT == 0 ? 2 : PT <= 13 ? 4 : 3; }
+// (orders 31 and 41 spill 40-110 B at the 128 registers of 4 CTAs per SM and are still 2-4 % faster than at 3 CTAs)
+__host__ __device__ constexpr int proj_min_blocks(int PT) { return PT == 0 ? 2 : 4; }
 __host__ __device__ constexpr int tdi_min_blocks(int PT) { return PT == 0 ? 2 : PT <= 13 ? 3 : 2; }
 
 // ---------------------------------------------------------------------------------------------- stage 1
@@ -58,8 +59,9 @@ project_kernel(const Params prm, const double* __restrict__ hp, const double* __
   const int n_last = n0 + kProjThreads - 1 < prm.n - 1 ? n0 + kProjThreads - 1 : prm.n - 1;
   const int i_lo = spline_interval(prm, sample_trel(prm, prm.n_off + n0), u_unused);
   const int i_hi = spline_interval(prm, sample_trel(prm, prm.n_off + n_last), u_unused);
-  // (measured: orders <= 25 gain 2 %, orders 31 and 41 lose 3-4 % -- their shared-memory pipe is the fuller one)
-  const bool tile_coef = PT > 0 && PT <= 13 && i_hi - i_lo <= 1;   // (block-uniform)
+  // (measured, plain form: orders <= 25 gain 2 %, orders 31 and 41 lose 1-2 % -- their shared-memory pipe is the fuller
+  // one; the extended form, with 18 evaluations per sample, gains 8-10 % at those orders too)
+  const bool tile_coef = PT > 0 && (PT <= 13 || EXT) && i_hi - i_lo <= 1;   // (block-uniform)
   if (tile_coef && threadIdx.x < 2 * NCH && !(EXT && threadIdx.x >= 6 && threadIdx.x < 18)) {   // (EXT: x_2, x_3 unused)
     const int ch = threadIdx.x >> 1, i = i_lo + (threadIdx.x & 1);
     sc[threadIdx.x] = load4(prm.coef + (int64_t)ch * prm.nint + (i < prm.nint ? i : prm.nint - 1));
