@@ -438,7 +438,10 @@ def batch_leg(lr, dev, local_rank, peak, hbm_gbs, reps=6):
            "gpu_launches": launches, "kernels": ks,
            "roofline": {"bound": "alu", "kernel": dom, "achieved": kd["gops"], "peak": peak / 1e9,
                         "unit": "Gop/s (FP64 thread-instruction slots, DFMA = 1)", "frac": kd["frac_fp64"],
-                        "frac_executed": kd.get("frac_executed"), "traffic": None,
+                        "frac_executed": kd.get("frac_executed"),
+                        "traffic": (ncu_counters("batch", dom)[0] or {}).get("dram_bytes"),
+                        "traffic_source": "profiles/r2_ncu_counters.csv (workload batch)" if ncu_counters("batch", dom)[0]
+                                          else ncu_counters("batch", dom)[1],
                         "path_frac": (ks["lr_project"]["alg_ops_per_sample"] + ks["lr_tdi"]["alg_ops_per_sample"]) * nb * n
                                      / ((ms_p + ms_t) * 1e-3) / peak},
            "clocks": clk.summary()}

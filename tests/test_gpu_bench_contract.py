@@ -42,6 +42,26 @@ def test_bench_line_contract():
     assert {"sm_mhz", "sm_max_mhz", "reasons"} <= set(d["clocks"])
 
 
+def test_bench_default_line_carries_batch_orders_and_one_thread():
+    """The default (one-year) run is the driver's line: besides the contract keys it must carry the batch leg of
+    BASELINE.json configs[2] (templates/s, per-kernel fractions), the executed-work fraction of lr_tdi, the order
+    sweep and the one-thread oracle figure with the CPU model ("next" item 2)."""
+    d = _run("--gpus", "1", "--steps", "3", "--warmup", "3", "--peak-seconds", "0.1", "--cpu-seconds", "1")
+    assert d["config"]["workload"].startswith("BASELINE.json configs[1]") and "cached" in d["config"]["tdi_plan"]
+    k = d["kernels"]["lr_tdi"]
+    assert k["path"] == "fir3" and k["executed_ops_per_sample"] == 3 * 4 * k["fir_taps"] * k["fir_powers"] == 1116
+    assert 0.3 < k["frac_executed"] < 1.0 and k["frac_fp64"] > 1.0
+    b = d["batch"]
+    assert b["templates_per_launch"] == 64 and b["templates_per_s"] > 500 and b["roofline"]["frac"] >= 0.5
+    assert b["params_to_loglike"]["loglike_per_s"] > 500
+    assert [r["order"] for r in d["orders"]["orders"]] == [1, 9, 25, 41]
+    assert all(0 < r[c]["frac"] < 1.2 for r in d["orders"]["orders"] for c in ("lr_project", "lr_tdi"))
+    cb = d["cpu_baseline"]
+    assert cb["cpu_model"] and cb["one_thread"]["cores"] == 1 and 0 < cb["one_thread"]["value"] < cb["value"]
+    rf = d["roofline"]
+    assert len(rf["csrc_sha256"]) == 64 and ("unavailable" in rf["ncu"]["lr_project"] or rf["traffic"] > 0)
+
+
 def test_bench_reference_arm():
     d = _run("--impl", "reference", "--steps", "1", "--warmup", "0", "--workload", "tiny", "--cpu-seconds", "0.5")
     assert d["impl"] == "reference" and d["value"] > 0
