@@ -781,8 +781,8 @@ def run_gpu(args, rank, world, local_rank):
         "value": value, "unit": "samples/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": dict(workload_config(w, batch, args), chunk_templates=chunk,
-                       parallelism=f"{world} rank(s), templates sharded, no collective"),
+        "config": workload_config(w, batch, args),     # (the same object in the --impl reference arm)
+        "launch": {"chunk_templates": chunk, "parallelism": f"{world} rank(s), templates sharded, no collective"},
         "templates_per_s": templates / (ms_step * 1e-3),
         "e2e": {"value": e2e_units / (e2e_ms * 1e-3), "unit": "samples/s", "ms_per_step": e2e_ms,
                 "templates": eb, "h2d_bytes_per_step": 2 * eb * n * 8, "d2h_bytes_per_step": nout * eb * n * 8,
