@@ -19,6 +19,10 @@
  *   - outputs are fully written; samples inside the fixed margins (lr_get_margins) are exactly 0.0.
  *   - lr_project / lr_tdi enqueue work on `cuda_stream` (a cudaStream_t, NULL = legacy default stream)
  *     and return without synchronising.  lr_response_host is synchronous.
+ *   - lr_project (batch <= 16) and lr_tdi may be captured into a CUDA graph (cudaStreamBeginCapture on `cuda_stream`):
+ *     they then wait on nothing outside the capture.  Call each once outside a capture first (so that the TDI plan
+ *     exists and the staging slots are idle), keep the handle's options unchanged, and replay the graph on one stream
+ *     at a time.  Every other computing call returns LR_EINVAL on a capturing stream.
  *   - all entry points return 0 on success or a negative LR_E* code; they never abort, throw or print.
  *     Inputs are not scanned for NaN (NaN propagates).
  *   - a handle keeps per-call staging state (and lr_tdi's plan): use one handle from one host thread and one

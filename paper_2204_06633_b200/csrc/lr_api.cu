@@ -140,6 +140,28 @@ TdiShape tdi_shape(const lr_handle* h);
     }                                         \
   } while (0)
 
+// Is the caller recording `st` into a CUDA graph?  lr_project and lr_tdi can be captured (a launch-bound loop of
+// small calls replays as one graph launch): they then wait on no event recorded outside the capture and record none
+// that the handle would wait on later.
+bool capturing(cudaStream_t st) {
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  return cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs == cudaStreamCaptureStatusActive;
+}
+// Event queries and allocations are among the calls a thread may not make while a global-mode capture is active:
+// this guard switches the calling thread to the relaxed mode for its lifetime.
+struct RelaxedCapture {
+  cudaStreamCaptureMode mode = cudaStreamCaptureModeRelaxed;
+  RelaxedCapture() { (void)cudaThreadExchangeStreamCaptureMode(&mode); }
+  ~RelaxedCapture() { (void)cudaThreadExchangeStreamCaptureMode(&mode); }
+};
+// an event recorded outside the capture must have completed already: a capture cannot wait for it
+bool event_done(cudaEvent_t ev) {
+  RelaxedCapture relaxed;
+  const bool done = cudaEventQuery(ev) == cudaSuccess;
+  if (!done) (void)cudaGetLastError();
+  return done;
+}
+
 lr::Params make_params(const lr_handle* h, int64_t n) {
   lr::Params P;
   memset(&P, 0, sizeof(P));
@@ -186,6 +208,12 @@ int stage_basis(lr_handle* h, const double* beta, const double* lam, const doubl
   Stage& S = h->stage[h->next_slot];
   h->next_slot = (h->next_slot + 1) % kSlots;
   if (!S.done) LR_CUDA(h, cudaEventCreateWithFlags(&S.done, cudaEventDisableTiming));
+  if (capturing(st)) {
+    // graph capture: only the parameter-buffer path (the constants become part of the kernel node), and only on a
+    // slot whose earlier users have finished
+    if (batch > lr::kSmallStage || (S.pending && !event_done(S.done))) return LR_EINVAL;
+    S.pending = false;
+  }
   if (S.pending) {
     // the slot's earlier users must be done with it: only a rewrite of the pinned host side needs the HOST to wait;
     // the small path (constants in the kernel's parameter buffer) orders the device side on the stream instead
@@ -194,6 +222,7 @@ int stage_basis(lr_handle* h, const double* beta, const double* lam, const doubl
     S.pending = false;
   }
   if (S.cap < batch) {
+    RelaxedCapture relaxed;   // (a first use of this slot inside a capture)
     if (S.host) cudaFreeHost(S.host);
     if (S.dev) cudaFree(S.dev);
     S.host = nullptr; S.dev = nullptr; S.cap = 0;
@@ -580,12 +609,17 @@ int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, do
       pl = h->plan;
       const bool fresh = h->plan_cache || (h->in_call && h->built_in_call);
       if (!(fresh && plan_matches(pl, h, w.n_glob, path))) {
+        if (capturing(st)) return LR_EINVAL;   // build the plan with one call outside the capture first
         const int rc = build_plan(h, pl, ts, w.n_glob, st, false);
         if (rc != LR_OK) return rc;
         h->built_in_call = true;
       }
     }
-    LR_CUDA(h, cudaStreamWaitEvent(st, pl->ready, 0));   // the plan may have been built on another stream
+    if (capturing(st)) {
+      if (!event_done(pl->ready)) return LR_EINVAL;      // (a capture cannot wait for work outside it)
+    } else {
+      LR_CUDA(h, cudaStreamWaitEvent(st, pl->ready, 0));   // the plan may have been built on another stream
+    }
     pa.coef = pl->coef; pa.flags = pl->flags; pa.list = pl->flags + P.ntiles;
     pa.plan_tiles = P.ntiles;
     if (h->sm_count == 0) {
@@ -605,10 +639,7 @@ int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, do
       LR_CUDA(h, cudaEventCreateWithFlags(&h->fix_join, cudaEventDisableTiming));
     }
     pa.side = h->fix_side; pa.fork = h->fix_fork; pa.join = h->fix_join;
-    if (pl->list_state.load() == 1) {
-      if (cudaEventQuery(pl->list_ev) == cudaSuccess) pl->list_state = 2;
-      else (void)cudaGetLastError();   // cudaErrorNotReady is not an error of this call
-    }
+    if (pl->list_state.load() == 1 && event_done(pl->list_ev)) pl->list_state = 2;
     if (pl->list_state.load() == 2) {
       const int cnt = pl->list_host[0];
       bool any = cnt > 0 && uniform;   // (one-tile plan: a flagged plan tile concerns every window)
@@ -622,7 +653,7 @@ int tdi_window(lr_handle* h, const double* y, int64_t batch, const Window& w, do
       if (pa.skip_fixup) *join_later = nullptr;   // nothing to wait for
       else { pa.join_extra = *join_later; pa.wait_join = false; }
     }
-    if (!pa.skip_fixup) h->last_join = h->fix_join;
+    if (!pa.skip_fixup && !capturing(st)) h->last_join = h->fix_join;
     apply_window(P, w);
     P.ntiles = (int)((w.n + lr::kFirTile - 1) / lr::kFirTile);
   } else {
@@ -664,8 +695,10 @@ int lr_project(lr_handle* h, const double* hp, const double* hc, const double* b
   const Window w{n, 0, n, 0, n, n, n};
   rc = project_window(h, hp, hc, S->dev, batch, w, y, stream);
   if (rc != LR_OK) return rc;
-  LR_CUDA(h, cudaEventRecord(S->done, st));
-  S->pending = true;
+  if (!capturing(st)) {   // (a captured event could not be waited for by a later call)
+    LR_CUDA(h, cudaEventRecord(S->done, st));
+    S->pending = true;
+  }
   return LR_OK;
 }
 
@@ -743,6 +776,7 @@ int lr_response_span(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const
                      int64_t n, int64_t first, int64_t count, double* out, void* stream) {
   lr_handle* h = hp_;
   if (!h || !ht_ || !h_plus || !h_cross || !beta || !lam || !psi || !out) return LR_EINVAL;
+  if (capturing((cudaStream_t)stream)) return LR_EINVAL;   // only lr_project and lr_tdi can be captured into a graph
   int rc = check_project(h, batch, n);
   if (rc == LR_OK) rc = check_tdi(ht_, batch, n);
   if (rc != LR_OK) return rc;
@@ -802,6 +836,7 @@ int lr_response_host(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const
                      const double* lam, const double* psi, int64_t batch, int64_t n, double* out, void* stream) {
   lr_handle* h = hp_;
   if (!h || !ht_ || !h_plus || !h_cross || !beta || !lam || !psi || !out) return LR_EINVAL;
+  if (capturing((cudaStream_t)stream)) return LR_EINVAL;   // only lr_project and lr_tdi can be captured into a graph
   int rc = check_project(h, batch, n);
   if (rc == LR_OK) rc = check_tdi(ht_, batch, n);
   if (rc != LR_OK) return rc;
@@ -905,6 +940,7 @@ int lr_response_host(lr_handle* hp_, lr_handle* ht_, const double* h_plus, const
 int lr_gb_waveform(lr_handle* h, const double* gb, int64_t batch, int64_t n, double* h_plus, double* h_cross,
                    void* stream) {
   if (!h || !gb || !h_plus || !h_cross || !size_ok(batch, n)) return LR_EINVAL;
+  if (capturing((cudaStream_t)stream)) return LR_EINVAL;
   for (int64_t i = 0; i < batch * 6; ++i)
     if (!std::isfinite(gb[i])) return LR_EINVAL;
   cudaStream_t st = (cudaStream_t)stream;
@@ -931,6 +967,7 @@ int response_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const double* 
                 const double* psi, int64_t batch, int64_t n, double* out, int64_t o_stride, void* stream) {
   lr_handle* h = hp_;
   if (!h || !ht_ || !gb || !beta || !lam || !psi || !out) return LR_EINVAL;
+  if (capturing((cudaStream_t)stream)) return LR_EINVAL;   // only lr_project and lr_tdi can be captured into a graph
   int rc = check_project(h, batch, n);
   if (rc == LR_OK) rc = check_tdi(ht_, batch, n);
   if (rc != LR_OK) return rc;
@@ -1090,6 +1127,7 @@ int lr_loglike_gb(lr_handle* hp_, lr_handle* ht_, const double* gb, const double
 int lr_plan_create(lr_handle* h, int64_t n, void* stream, lr_plan** out) {
   if (!h || !out) return LR_EINVAL;
   *out = nullptr;
+  if (capturing((cudaStream_t)stream)) return LR_EINVAL;
   const int rc = check_tdi(h, 1, n);
   if (rc != LR_OK) return rc;
   const TdiShape ts = tdi_shape(h);

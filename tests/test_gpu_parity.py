@@ -789,6 +789,50 @@ def test_shared_plan_two_streams_bitwise(lr):
         lr.lr_plan_create(Rp.handle, w.n)
 
 
+def test_project_and_tdi_replay_from_a_cuda_graph(lr):
+    """lr_project (parameter-buffer staging, batch <= 16) and lr_tdi can be captured into a CUDA graph once the plan
+    exists: the tiny config (launch-latency bound: three launches) replays bit-identically, new inputs written into
+    the captured buffers give the results of direct calls, and the calls that cannot be captured say so (LR_EINVAL)
+    without breaking the capture."""
+    import torch
+    w = inputs.config(1)
+    s = w.sources[0]
+    hp, hc = w.waveform(0)
+    hpd, hcd = to_dev(hp)[None].clone(), to_dev(hc)[None].clone()
+    R = lr.Response(w.table(), w.dt, w.order, 1, t0=w.t0)
+    y = torch.empty((1, 6, w.n), dtype=torch.float64, device="cuda")
+    out = torch.empty((1, 3, w.n), dtype=torch.float64, device="cuda")
+    for _ in range(2):                                     # outside a capture first: builds the plan
+        R.project(hpd, hcd, [s.beta], [s.lam], [s.psi], y_out=y)
+        R.tdi(y, out=out)
+    torch.cuda.synchronize()
+    ref = out.clone()
+    st = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    refused = None
+    with torch.cuda.graph(g, stream=st):
+        R.project(hpd, hcd, [s.beta], [s.lam], [s.psi], y_out=y, stream=st)
+        R.tdi(y, out=out, stream=st)
+        try:
+            R.response(hpd, hcd, [s.beta], [s.lam], [s.psi], out=out, stream=st)
+        except lr.LrError as e:
+            refused = e.code
+    assert refused == lr.LR_EINVAL
+    out.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref)
+    hpd.mul_(0.5)                                          # new input in the captured buffers
+    hcd.mul_(0.5)
+    g.replay()
+    torch.cuda.synchronize()
+    got = out.clone()
+    want = R.tdi(R.project(hpd, hcd, [s.beta], [s.lam], [s.psi]))
+    torch.cuda.synchronize()
+    assert torch.equal(got, want)
+    assert np.array_equal(R.tdi(R.project(hpd * 2, hcd * 2, [s.beta], [s.lam], [s.psi])).cpu().numpy(), ref.cpu().numpy())
+
+
 def test_binding_checks_out_against_the_channel_option(lr):
     """The C ABI takes no size for `out`: the binding checks it against the handle's LR_OPT_CHANNELS (lr_get_option),
     so a [B,3,N] buffer is never handed to a handle that writes six rows; angle arrays must match the batch."""
