@@ -57,6 +57,7 @@ typedef struct {
 #define LR_ERANGE (-2)  /* the sample span (with the backward reach of the delays) leaves the knot table */
 #define LR_ECUDA (-3)   /* a CUDA call failed; lr_last_cuda_error gives the CUDA code */
 #define LR_ENOMEM (-4)  /* host allocation failed */
+#define LR_ELIMIT (-5)  /* a size exceeds the fixed capacity of a no-allocation entry point (lr_inner_product_static) */
 
 /* option keys for lr_set_option */
 #define LR_OPT_T0 1       /* time of sample 0 [s]; default orbits->t_start */
@@ -285,6 +286,23 @@ int lr_response_gb(lr_handle* h_proj, lr_handle* h_tdi, const double* gb, const 
 int lr_inner_product(const double* fa, const double* fb, const double* inv_psd, double scale, int mode,
                      int64_t batch, int64_t batch_b, int nch, int64_t nf, double* work, double* out,
                      void* cuda_stream);
+
+/* lr_inner_product for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): the same kernels and the same results bit for bit, with the scratch of the reduction (the
+ * per-block partial sums) in a device array that is part of the library image instead of a caller-supplied `work`
+ * buffer.  The call allocates nothing: no cudaMalloc, cudaFree or allocating library routine; its first call on a
+ * device resolves the array's address (cudaGetSymbolAddress, with that device current) and caches it.
+ *   - limit: batch <= LR_IP_STATIC_MAX_BATCH (64); a larger batch returns LR_ELIMIT and launches nothing (split
+ *     the batch, or use lr_inner_product).  The array is LR_IP_STATIC_MAX_BATCH * LR_IP_BLOCKS doubles = 512 KB of
+ *     device memory on every GPU that loads the library, held until the process exits.
+ *   - ALL calls on a device share the one array: two calls whose kernels can overlap on the GPU (different streams
+ *     without an ordering between them, or two host threads) race on it and give wrong results.  Calls on one
+ *     stream, or otherwise ordered, are safe.  Nothing in it needs clearing between calls: stage 1 overwrites every
+ *     element stage 2 reads.
+ * Arguments as lr_inner_product without `work`.  Errors: LR_EINVAL, LR_ELIMIT, LR_ECUDA. */
+#define LR_IP_STATIC_MAX_BATCH 64
+int lr_inner_product_static(const double* fa, const double* fb, const double* inv_psd, double scale, int mode,
+                            int64_t batch, int64_t batch_b, int nch, int64_t nf, double* out, void* cuda_stream);
 
 /* One likelihood evaluation per template, parameters in, one scalar out ("only the scalar
  * returns"; eqs. 2-3, 5-9, 10-22): lr_response_gb into scratch, the library's real-to-complex FFT (cuFFT, fp64)

@@ -15,7 +15,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("LR_LIBRARY", os.path.join(_HERE, "liblr.so"))  # override: A/B builds
 
-LR_OK, LR_EINVAL, LR_ERANGE, LR_ECUDA, LR_ENOMEM = 0, -1, -2, -3, -4
+LR_OK, LR_EINVAL, LR_ERANGE, LR_ECUDA, LR_ENOMEM, LR_ELIMIT = 0, -1, -2, -3, -4, -5
+LR_IP_STATIC_MAX_BATCH = 64
 LR_OPT_T0, LR_OPT_CHAIN, LR_OPT_CHANNELS, LR_OPT_TDI_GEN, LR_OPT_TDI_PATH = 1, 2, 3, 4, 5
 LR_OPT_TDI_PLAN_CACHE = 6
 LR_OPT_CHUNK_SAMPLES = 7
@@ -35,7 +36,7 @@ LR_MAX_ORDER = 65
 
 # every symbol include/lr.h declares
 SYMBOLS = ("lr_create", "lr_destroy", "lr_set_option", "lr_get_option", "lr_get_margins", "lr_project", "lr_tdi",
-           "lr_inner_product", "lr_gb_parameters", "lr_fft_good_length", "lr_gb_waveform", "lr_response_gb", "lr_loglike_gb", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count", "lr_plan_create", "lr_plan_attach", "lr_plan_release", "lr_plan_bytes",
+           "lr_inner_product", "lr_inner_product_static", "lr_gb_parameters", "lr_fft_good_length", "lr_gb_waveform", "lr_response_gb", "lr_loglike_gb", "lr_response", "lr_response_span", "lr_get_span_halo", "lr_response_host", "lr_eval_orbit", "lr_measure_fp64_peak", "lr_launch_count", "lr_plan_create", "lr_plan_attach", "lr_plan_release", "lr_plan_bytes",
            "lr_last_cuda_error", "lr_strerror")
 
 
@@ -87,6 +88,7 @@ def lib():
     L.lr_get_span_halo.argtypes = [vp, vp, pi64, pi64, pi64]
     L.lr_response_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i64, vp, vp]
     L.lr_inner_product.argtypes = [vp, vp, vp, dbl, ci, i64, i64, ci, i64, vp, vp, vp]
+    L.lr_inner_product_static.argtypes = [vp, vp, vp, dbl, ci, i64, i64, ci, i64, vp, vp]
     L.lr_gb_waveform.argtypes = [vp, vp, i64, i64, vp, vp, vp]
     L.lr_gb_parameters.argtypes = [dbl, dbl, dbl, dbl, dbl, ci, vp]
     L.lr_fft_good_length.argtypes = [i64]
@@ -365,6 +367,23 @@ def lr_inner_product(fa, fb, inv_psd, scale, mode=LR_IP_CROSS, out=None, stream=
     _check(lib().lr_inner_product(fa.data_ptr(), fb.data_ptr(), _dev_ptr(inv_psd, "inv_psd", nch * nf), float(scale),
                                   int(mode), B, fb.shape[0], nch, nf, work.data_ptr(), _dev_ptr(out, "out", B),
                                   _stream(stream)), "lr_inner_product")
+    return out
+
+
+def lr_inner_product_static(fa, fb, inv_psd, scale, out, mode=LR_IP_CROSS, stream=None):
+    """lr_inner_product_static: as lr_inner_product, with the scratch inside the library (no allocation anywhere:
+    `out` CUDA float64 [B] is the caller's).  B <= LR_IP_STATIC_MAX_BATCH, else LrError(LR_ELIMIT)."""
+    import torch
+    for name, t in (("fa", fa), ("fb", fb)):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.complex128 and t.is_contiguous()
+                and t.dim() == 3):
+            raise TypeError(f"{name} must be a contiguous complex128 CUDA tensor [batch, nch, nf]")
+    B, nch, nf = fa.shape
+    if fb.shape[1:] != fa.shape[1:] or fb.shape[0] not in (1, B):
+        raise ValueError("fb must be [batch or 1, nch, nf]")
+    _check(lib().lr_inner_product_static(fa.data_ptr(), fb.data_ptr(), _dev_ptr(inv_psd, "inv_psd", nch * nf),
+                                         float(scale), int(mode), B, fb.shape[0], nch, nf, _dev_ptr(out, "out", B),
+                                         _stream(stream)), "lr_inner_product_static")
     return out
 
 

@@ -1204,6 +1204,7 @@ const char* lr_strerror(int code) {
     case LR_ERANGE: return "sample span (with the delays' backward reach) is not covered by the orbit table";
     case LR_ECUDA: return "CUDA error (see lr_last_cuda_error)";
     case LR_ENOMEM: return "host allocation failed";
+    case LR_ELIMIT: return "size exceeds the fixed capacity of this no-allocation entry point (see include/lr.h)";
     default: return "unknown error code";
   }
 }

@@ -92,3 +92,58 @@ extern "C" int lr_inner_product(const double* fa, const double* fb, const double
   lr::g_launches.fetch_add(2);
   return cudaGetLastError() == cudaSuccess ? LR_OK : LR_ECUDA;
 }
+
+// ------------------------------------------------------------------------------- no-allocation entry point
+// lr_inner_product_static: the same two-stage reduction with its scratch (the per-block partial sums of stage 1) in a
+// file-scope device array instead of a caller-supplied buffer, for callers that cannot allocate: code under CUDA
+// graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Every GPU that loads liblr holds the array
+// (LR_IP_STATIC_MAX_BATCH x LR_IP_BLOCKS doubles = 512 KB) until the process exits.
+namespace lr {
+static __device__ __align__(256) double g_ip_static_work[(size_t)LR_IP_STATIC_MAX_BATCH * LR_IP_BLOCKS];
+
+// In host code `g_ip_static_work` is a host-side stand-in for the symbol, not a device address; the address comes
+// from cudaGetSymbolAddress, once per device, with that device current.
+constexpr int kMaxDevices = 64;
+static std::atomic<double*> g_ip_static_ptr[kMaxDevices];
+
+static int ip_static_scratch(double** ptr) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return LR_ECUDA;
+  double* p = g_ip_static_ptr[dev].load(std::memory_order_acquire);
+  if (!p) {   // set-up of this device (racing threads resolve the same address)
+    void* q = nullptr;
+    if (cudaGetSymbolAddress(&q, g_ip_static_work) != cudaSuccess || !q) {
+      (void)cudaGetLastError();
+      return LR_ECUDA;
+    }
+    p = static_cast<double*>(q);
+    g_ip_static_ptr[dev].store(p, std::memory_order_release);
+  }
+  *ptr = p;
+  return LR_OK;
+}
+}  // namespace lr
+
+extern "C" int lr_inner_product_static(const double* fa, const double* fb, const double* inv_psd, double scale,
+                                       int mode, int64_t batch, int64_t batch_b, int nch, int64_t nf, double* out,
+                                       void* stream) {
+  if (!fa || !fb || !inv_psd || !out) return LR_EINVAL;
+  if (batch < 1 || (batch_b != 1 && batch_b != batch) || nch < 1 || nf < 1) return LR_EINVAL;
+  if (mode != LR_IP_CROSS && mode != LR_IP_DIFF) return LR_EINVAL;
+  if (batch > LR_IP_STATIC_MAX_BATCH) return LR_ELIMIT;   // the scratch array holds LR_IP_STATIC_MAX_BATCH templates
+  double* work = nullptr;
+  const int rc = lr::ip_static_scratch(&work);
+  if (rc != LR_OK) return rc;
+  const int64_t M = (int64_t)nch * nf;
+  cudaStream_t st = (cudaStream_t)stream;
+  // Nothing in the scratch has to start at zero: stage 1 writes every one of the batch x LR_IP_BLOCKS partial sums
+  // stage 2 reads (a block with an empty slice writes 0), so whatever the previous call left behind is overwritten
+  // before it is read.
+  dim3 grid(LR_IP_BLOCKS, (unsigned)batch);
+  lr::ip_partial_kernel<<<grid, lr::kIpThreads, 0, st>>>(reinterpret_cast<const double2*>(fa),
+                                                         reinterpret_cast<const double2*>(fb), inv_psd, M, batch_b,
+                                                         mode, work);
+  lr::ip_final_kernel<<<(unsigned)batch, lr::kIpThreads, 0, st>>>(work, LR_IP_BLOCKS, scale, out);
+  lr::g_launches.fetch_add(2);
+  return cudaGetLastError() == cudaSuccess ? LR_OK : LR_ECUDA;
+}
