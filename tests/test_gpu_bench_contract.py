@@ -90,3 +90,26 @@ def test_fp64_operand_probe_orders_the_modes(tmp_path):
     nominal = sms * 64 * 2.2e9
     assert all(0 < x < nominal for x in r), r
     assert r[2] < 0.9 * r[1] and r[1] <= 1.05 * r[0] and r[3] <= 1.02 * r[1], r
+
+
+def test_shuffle_exchange_is_not_faster_than_lds(tmp_path):
+    """tests/probes/shuffle_vs_lds_probe.cu: handing every lane a 16-byte stencil element through warp shuffles
+    (4 SHFL.32) delivers no more elements per second than one LDS.128 per lane from shared memory: the measurement
+    behind DESIGN.md §6's paragraph on warp shuffles (north_star names them for the stencil reductions; the hot
+    kernels read their windows with LDS.128 instead)."""
+    import ctypes
+    import shutil
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    so = str(tmp_path / "shuffle_vs_lds_probe.so")
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-shared", "-Xcompiler", "-fPIC",
+                    os.path.join(ROOT, "tests", "probes", "shuffle_vs_lds_probe.cu"), "-o", so], check=True)
+    L = ctypes.CDLL(so)
+    L.probe_exchange.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
+    r = []
+    for m in range(2):
+        v = ctypes.c_double()
+        assert L.probe_exchange(m, ctypes.byref(v)) == 0
+        r.append(v.value)
+    print(f"LDS.128: {r[0]:.3e} elements/s, 4 x SHFL.32: {r[1]:.3e} elements/s")
+    assert r[0] > 0 and r[1] > 0
+    assert r[1] <= 1.05 * r[0], r
