@@ -831,6 +831,36 @@ def test_project_and_tdi_replay_from_a_cuda_graph(lr):
     torch.cuda.synchronize()
     assert torch.equal(got, want)
     assert np.array_equal(R.tdi(R.project(hpd * 2, hcd * 2, [s.beta], [s.lam], [s.psi])).cpu().numpy(), ref.cpu().numpy())
+    # a series with flagged tiles: the capture then holds the fork to the handle's side stream, the fix-up kernel and
+    # the join back (light times that cross a whole number of samples in the middle of the series)
+    dt, n, t0, order = 10.0, 40000, 3.0e7, 9
+    base = inputs.orbit_table("kepler", t0, t0 + n * dt)
+    tk = base.t_start + base.knot_dt * np.arange(base.n_knots)
+    ltt = np.tile(10.0 + 2e-9 * (tk - (t0 + 0.5 * n * dt)), (6, 1)) * (1 + 1e-7 * np.arange(6))[:, None]
+    tab = inputs.OrbitTable(base.t_start, base.knot_dt, base.x, np.ascontiguousarray(ltt))
+    w2 = inputs.config(2, n=n, t0=t0)
+    hp2, hc2 = w2.waveform(0)
+    s2 = w2.sources[0]
+    hp2d, hc2d = to_dev(hp2)[None], to_dev(hc2)[None]
+    R2 = lr.Response(tab, dt, order, 2, t0=t0, tdi_path="fir3")
+    y2 = torch.empty((1, 6, n), dtype=torch.float64, device="cuda")
+    o2 = torch.empty((1, 3, n), dtype=torch.float64, device="cuda")
+    for _ in range(2):
+        R2.project(hp2d, hc2d, [s2.beta], [s2.lam], [s2.psi], y_out=y2)
+        R2.tdi(y2, out=o2)
+    torch.cuda.synchronize()
+    ref2 = o2.clone()
+    g2 = torch.cuda.CUDAGraph()
+    l0 = lr.lr_launch_count()
+    with torch.cuda.graph(g2, stream=st):
+        R2.project(hp2d, hc2d, [s2.beta], [s2.lam], [s2.psi], y_out=y2, stream=st)
+        R2.tdi(y2, out=o2, stream=st)
+    assert lr.lr_launch_count() - l0 == 4                  # source basis, projection, fix-up, apply
+    for _ in range(3):
+        o2.zero_()
+        g2.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(o2, ref2)
 
 
 def test_binding_checks_out_against_the_channel_option(lr):
