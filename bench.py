@@ -574,10 +574,12 @@ def run_gpu(args, rank, world, local_rank):
                 tt += e1.elapsed_time(e2)
         return tp, tt
 
+    # (the roofline denominator is measured BEFORE the warm-up: the first step after its second-long DFMA kernel runs
+    # 20 % slow, which would weigh on a run with few timed steps)
+    peak = lr.lr_measure_fp64_peak(args.peak_seconds)   # FP64 thread-instructions / s, this device, now
     for _ in range(args.warmup):
         step(False)
     torch.cuda.synchronize()
-    peak = lr.lr_measure_fp64_peak(args.peak_seconds)   # FP64 thread-instructions / s, this device, now
     barrier()
     torch.cuda.synchronize()
     launches0 = lr.lr_launch_count()
@@ -869,9 +871,9 @@ def run_gpu_time_sharded(args, rank, world, local_rank):
         e1.synchronize()
         return e0.elapsed_time(e1)
 
+    peak = lr.lr_measure_fp64_peak(args.peak_seconds)
     for _ in range(args.warmup):
         step()
-    peak = lr.lr_measure_fp64_peak(args.peak_seconds)
     barrier()
     torch.cuda.synchronize()
     launches0 = lr.lr_launch_count()
