@@ -422,9 +422,10 @@ def batch_leg(lr, dev, local_rank, peak, hbm_gbs, reps=6):
     y = torch.empty((nb, 6, n), dtype=torch.float64, device=dev)
     out = torch.empty((nb, 3, n), dtype=torch.float64, device=dev)
     stream = torch.cuda.current_stream()
+    clk = ClockSampler(local_rank)
     timed_steps(lr, R, R, hp, hc, ang, y, out, 2, None, stream)          # warm-up (builds the plan)
     l0 = lr.lr_launch_count()
-    with ClockSampler(local_rank) as clk:
+    with clk:
         ms_p, ms_t = timed_steps(lr, R, R, hp, hc, ang, y, out, reps, None, stream)
         torch.cuda.synchronize()
     launches = lr.lr_launch_count() - l0
@@ -577,15 +578,16 @@ def run_gpu(args, rank, world, local_rank):
     # (the roofline denominator is measured BEFORE the warm-up: the first step after its second-long DFMA kernel runs
     # 20 % slow, which would weigh on a run with few timed steps)
     peak = lr.lr_measure_fp64_peak(args.peak_seconds)   # FP64 thread-instructions / s, this device, now
+    clk = ClockSampler(local_rank)     # (NVML is initialised here, not between the warm-up and the timed steps: 0.1 s
+                                       # of idle GPU makes the next step 30 % slow)
     for _ in range(args.warmup):
         step(False)
     torch.cuda.synchronize()
     barrier()
-    torch.cuda.synchronize()
     launches0 = lr.lr_launch_count()
     tps, tts = [], []
     wall0 = time.perf_counter()
-    with ClockSampler(local_rank) as clk:
+    with clk:
         for _ in range(args.steps):
             a, b = step(True)
             tps.append(a)
@@ -872,12 +874,13 @@ def run_gpu_time_sharded(args, rank, world, local_rank):
         return e0.elapsed_time(e1)
 
     peak = lr.lr_measure_fp64_peak(args.peak_seconds)
+    clk = ClockSampler(local_rank)
     for _ in range(args.warmup):
         step()
     barrier()
     torch.cuda.synchronize()
     launches0 = lr.lr_launch_count()
-    with ClockSampler(local_rank) as clk:
+    with clk:
         ms = [step() for _ in range(args.steps)]
         torch.cuda.synchronize()
     barrier()
