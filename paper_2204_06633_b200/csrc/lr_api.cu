@@ -498,7 +498,10 @@ TdiShape tdi_shape(const lr_handle* h) {
     t.halo_lo = back > (int)(mf - h->m_proj()) ? back : (int)(mf - h->m_proj());
     t.halo_hi = h->p + lr::kFirR;
     // very long stencils: keep the per-sample kernel
-    if (lr::fir_apply_smem_bytes(lr::kFirTile + t.halo_lo + t.halo_hi, t.wc) > 200 * 1024) t.path = LR_TDI_PER_SAMPLE;
+    const int Wst = lr::kFirTile + t.halo_lo + t.halo_hi;
+    if ((t.path == LR_TDI_FIR4 && !h->const_ltt ? lr::fir_mma_smem_bytes(Wst, t.wc) : lr::fir_apply_smem_bytes(Wst, t.wc)) >
+        200 * 1024)
+      t.path = LR_TDI_PER_SAMPLE;
   }
   if (t.path == LR_TDI_PER_SAMPLE) {
     t.wc = 0;

@@ -114,6 +114,11 @@ static int launch_tdi_fir(const Params& prm, int channels, const double* y, doub
     if ((e = prepare(tdi_fir_apply_kernel<1>, smem)) != cudaSuccess) return (int)e;
     tdi_fir_apply_kernel<1><<<(unsigned)grid, kFirThreads, smem, st>>>(prm, y, out, channels, plan.coef, plan.flags,
                                                                      (int)batch);
+  } else if constexpr (NN == 4) {   // cubic plans: the tensor-path kernel (a full 8 x 8 x 4 FP64 MMA tile)
+    const size_t smem_m = fir_mma_smem_bytes(W, prm.fir_wc);
+    if ((e = prepare(tdi_fir_apply_mma_kernel<4>, smem_m)) != cudaSuccess) return (int)e;
+    tdi_fir_apply_mma_kernel<4><<<(unsigned)grid, kFirMmaThreads, smem_m, st>>>(prm, y, out, channels, plan.coef,
+                                                                              plan.flags, (int)batch);
   } else {
     if ((e = prepare(tdi_fir_apply_kernel<NN>, smem)) != cudaSuccess) return (int)e;
     tdi_fir_apply_kernel<NN><<<(unsigned)grid, kFirThreads, smem, st>>>(prm, y, out, channels, plan.coef, plan.flags,

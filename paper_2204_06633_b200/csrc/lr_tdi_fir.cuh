@@ -355,7 +355,7 @@ __device__ __forceinline__ void fir_store(double* ob, int64_t N, int n, int chan
 }
 
 template <int NN>
-__global__ void __launch_bounds__(kFirThreads, NN > 3 ? 5 : kFirMinBlocks)   // NN = 4: 28 accumulators
+__global__ void __launch_bounds__(kFirThreads, kFirMinBlocks)
 tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ out, int channels,
                      const double* __restrict__ plan, const int* __restrict__ flags, int batch) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -437,6 +437,200 @@ tdi_fir_apply_kernel(const Params prm, const double* __restrict__ y, double* __r
     fir_store(ob, N, n, channels, valid ? res[i] : 0.0, valid ? res[B + i] : 0.0, valid ? res[2 * B + i] : 0.0);
   }
 }
+
+// ------------------------------------------------------------------------- apply kernel, cubic plans (NN = 4)
+// The same filter through the FP64 tensor path (mma.sync.m8n8k4.f64).  A DFMA of the loop above reads two fresh
+// 64-bit register operands and cannot issue every second cycle (43 per SM and clock at NN = 4); an MMA reads four
+// operand registers per eight FMAs per thread and runs at the pipe's rate.  With four powers of tile time the tensor
+// tile is full: every y series feeds exactly two of the three channels, so for series s
+//   D[8 samples][8 columns] += A[8 samples][4 taps] * B[4 taps][8 columns],
+//   A[i][k] = dif_s[n0 + i + m0 + k],  B[k][(half, p)] = K_p[channel of that half][s][m0 + k],
+// columns = (left channel: p = 0..3 | right channel: p = 0..3).  Three accumulator tiles per 8 samples:
+//   XY (series 12, 21: X | Y),  ZY (series 23, 32: Z | Y),  XZ (series 31, 13: X | Z),
+// and X = XY.left + XZ.left, Y = XY.right + ZY.right, Z = ZY.left + XZ.right; the powers of tile time are applied to
+// the sums at the end (as in fir_apply).  (With three powers the tile would be 6/8 full: no faster than the DFMA loop;
+// the quadratic plans keep it.)
+// One CTA = one plan tile of 224 samples = 4 warps x 7 row tiles of 8 samples.  A is a Hankel block (it depends on
+// i + k only), so the A fragment of row tile j at tap step q is the fragment of row tile j+1 at step q-2: two sliding
+// windows of 7 fragments (even and odd steps), one new LDS.64 per step.  dynamic smem: dif[6][W] | K[12][Wc][4] |
+// raw[6][W + 1] (the y window as it arrives by cp.async); the staged sums res[3][4][224] overlay dif and K once the
+// MMAs are done.
+constexpr int kFirMmaThreads = 128;
+LR_HD size_t fir_mma_smem_bytes(int W, int Wc) {
+  const size_t a = fir_apply_smem_bytes(W, Wc) + (size_t)6 * ((W + 2) & ~1) * sizeof(double);   // dif | K | raw
+  const size_t b = (size_t)12 * kFirTile * sizeof(double);
+  return a > b ? a : b;
+}
+
+#ifdef __CUDACC__
+__device__ __forceinline__ void dmma_8x8x4(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+template <int NN>
+__global__ void __launch_bounds__(kFirMmaThreads, 3)
+tdi_fir_apply_mma_kernel(const Params prm, const double* __restrict__ y, double* __restrict__ out, int channels,
+                         const double* __restrict__ plan, const int* __restrict__ flags, int batch) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int B = kFirTile, RT = 7;                        // row tiles (of 8 samples) per warp
+  static_assert(NN == 4 && NN == kFirKStride, "the MMA tile holds two channels x four powers");
+  static_assert(kFirMmaThreads / 32 * RT * 8 == kFirTile, "4 warps x 7 row tiles x 8 samples");
+  const int W = B + prm.halo_lo + prm.halo_hi;
+  const int Wc = prm.fir_wc;
+  const int Wr = (W + 2) & ~1;                               // staged y samples per series (W differences need W + 1)
+  double* dif = reinterpret_cast<double*>(smem_raw);
+  double* K = dif + 6 * W;
+  double* raw = K + fir_plan_doubles_per_tile(Wc);           // [6][Wr]
+  double* res = dif;                                         // [3 channels][4 powers][B], after the MMAs
+
+  const int tid = threadIdx.x;
+  const int tile = blockIdx.x / batch;                       // local tile: local samples [n0, n0 + B)
+  const int64_t b = blockIdx.x - (int64_t)tile * batch;
+  const int n0 = tile * B;
+  const int g0 = n0 - prm.halo_lo;
+  const int tile_g = tile + prm.n_off / B;                   // global tile (prm.n_off is a multiple of B)
+  const int n0g = prm.n_off + n0;
+  const int64_t N = prm.out_stride;
+  const int nout = channels == 2 ? 6 : 3;
+  double* ob = out + b * nout * N;
+
+  const int v_lo = prm.m_front, v_hi = prm.n_glob - prm.m_back;   // valid global samples [v_lo, v_hi)
+  if (n0g + B <= v_lo || n0g >= v_hi) {                      // tile entirely inside a margin
+    for (int i = tid; i < B; i += kFirMmaThreads)
+      if (n0 + i < prm.n)
+        for (int c = 0; c < nout; ++c) ob[(int64_t)c * N + n0 + i] = 0.0;
+    return;
+  }
+  if (flags[tile_g] != 0) return;                            // exact per-sample tile: the fix-up kernel's
+
+  {   // the tile's plan: global -> shared without passing through registers, in flight under the loads of y
+    const double2* src = reinterpret_cast<const double2*>(plan + (size_t)tile_g * fir_plan_doubles_per_tile(Wc));
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(K);
+    const int cnt = (int)(fir_plan_doubles_per_tile(Wc) / 2);
+    for (int m = tid; m < cnt; m += kFirMmaThreads)
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * m), "l"(src + m) : "memory");
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  }
+  {   // the y window of the six series: asynchronous 8-byte copies (the rows of y need not be 16-byte aligned), all in
+      // flight at once; with 12 warps per SM a staging phase of six dependent global loads would not be hidden
+    const double* yb = y + b * 6 * prm.in_stride + g0;
+    if (g0 >= prm.rd_lo && g0 + W < prm.rd_hi) {             // (block-uniform) the whole window is readable
+      const unsigned dst = (unsigned)__cvta_generic_to_shared(raw);
+#pragma unroll
+      for (int sr = 0; sr < 6; ++sr) {
+        const double* ys = yb + sr * prm.in_stride;
+        for (int w = tid; w <= W; w += kFirMmaThreads)
+          asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 8u * (unsigned)(sr * Wr + w)), "l"(ys + w)
+                       : "memory");
+      }
+    } else {
+      for (int sr = 0; sr < 6; ++sr) {
+        const double* ys = yb + sr * prm.in_stride;
+        for (int w = tid; w <= W; w += kFirMmaThreads) {
+          const int g = g0 + w;
+          raw[sr * Wr + w] = (g >= prm.rd_lo && g < prm.rd_hi) ? __ldg(ys + w) : 0.0;
+        }
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  __syncthreads();
+  for (int m = tid; m < 6 * W; m += kFirMmaThreads) {        // exact first differences, as the one-shot kernel forms them
+    const int sr = m / W, w = m - sr * W;
+    dif[m] = raw[sr * Wr + w + 1] - raw[sr * Wr + w];
+  }
+  __syncthreads();
+
+  const int warp = tid >> 5, lane = tid & 31;
+  const int row = lane >> 2, kq = lane & 3;                  // A: [row][kq]; B: [kq][column = row]; D: [row][2 kq, 2 kq + 1]
+  const int half = row >> 2, pw = row & 3;                   // B column -> (left | right channel, power)
+  const int back = Wc - (prm.p - 1);
+  const int Q = (Wc + 3) >> 2;                               // tap steps of 4 (coefficients beyond Wc count as 0)
+  const int abase = prm.halo_lo + warp * (RT * 8) - back + row + kq;   // A fragment u: dif[abase + 4 u]
+  // accumulator tiles: (series slots, (channel, local series) of the left and of the right half), see above and
+  // fir_base_slot: X = {13, 31, 12, 21}, Y = {21, 12, 23, 32}, Z = {32, 23, 31, 13} in local order
+  double acc[3][RT][2];
+#pragma unroll
+  for (int t = 0; t < 3; ++t)
+#pragma unroll
+    for (int j = 0; j < RT; ++j) { acc[t][j][0] = 0.0; acc[t][j][1] = 0.0; }
+#pragma unroll
+  for (int t = 0; t < 3; ++t) {
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      // XY: slot 0 = (X,2)|(Y,1), slot 5 = (X,3)|(Y,0);  ZY: slot 1 = (Z,1)|(Y,2), slot 4 = (Z,0)|(Y,3);
+      // XZ: slot 2 = (X,1)|(Z,2), slot 3 = (X,0)|(Z,3)
+      const int slot = t == 0 ? (e == 0 ? 0 : 5) : t == 1 ? (e == 0 ? 1 : 4) : (e == 0 ? 2 : 3);
+      const int csl = t == 0 ? (e == 0 ? 0 * 4 + 2 : 0 * 4 + 3) : t == 1 ? (e == 0 ? 2 * 4 + 1 : 2 * 4 + 0)
+                                                                       : (e == 0 ? 0 * 4 + 1 : 0 * 4 + 0);
+      const int csr = t == 0 ? (e == 0 ? 1 * 4 + 1 : 1 * 4 + 0) : t == 1 ? (e == 0 ? 1 * 4 + 2 : 1 * 4 + 3)
+                                                                       : (e == 0 ? 2 * 4 + 2 : 2 * 4 + 3);
+      const double* a = dif + slot * W + abase;
+      const double* kb = K + ((size_t)(half ? csr : csl) * Wc + kq) * kFirKStride + pw;   // + 4 q taps
+      // A fragments of the even / odd steps as circular windows: at step q = q0 + s (q0 a multiple of 2 RT) row tile j
+      // needs fragment u = q + 2 j, kept at position (j + s / 2) % RT; after the step the position of row tile 0
+      // takes fragment u = q + 2 RT.  All positions are compile-time constants (no register moves).
+      double we[RT], wo[RT];
+#pragma unroll
+      for (int j = 0; j < RT; ++j) { we[j] = a[4 * (2 * j)]; wo[j] = a[4 * (2 * j + 1)]; }
+#pragma unroll 1
+      for (int q0 = 0; q0 < Q; q0 += 2 * RT) {
+#pragma unroll
+        for (int sp = 0; sp < 2 * RT; ++sp) {
+          const int q = q0 + sp;
+          if (q < Q) {                                         // (warp-uniform)
+            const double bf = 4 * q + kq < Wc ? kb[(size_t)4 * q * kFirKStride] : 0.0;
+            if (sp % 2 == 0) {
+#pragma unroll
+              for (int j = 0; j < RT; ++j) dmma_8x8x4(acc[t][j][0], acc[t][j][1], we[(j + sp / 2) % RT], bf);
+              we[(sp / 2) % RT] = a[4 * (q + 2 * RT)];
+            } else {
+#pragma unroll
+              for (int j = 0; j < RT; ++j) dmma_8x8x4(acc[t][j][0], acc[t][j][1], wo[(j + sp / 2) % RT], bf);
+              wo[(sp / 2) % RT] = a[4 * (q + 2 * RT)];
+            }
+          }
+        }
+      }
+    }
+  }
+  __syncthreads();                                           // every warp is done with dif and K: res may overlay them
+  // lanes with kq < 2 hold left halves (powers 2 kq, 2 kq + 1), the others right halves (powers 2 (kq - 2), ...):
+  //   kq < 2 : X = XY + XZ complete, Z (ZY.left) partial;  kq >= 2 : Y = XY + ZY complete, Z (XZ.right) partial
+#pragma unroll
+  for (int j = 0; j < RT; ++j) {
+    const int i = warp * (RT * 8) + j * 8 + row;
+    const int p0 = 2 * (kq & 1);
+    const bool left = kq < 2;
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      const double mine = left ? acc[0][j][c] + acc[2][j][c] : acc[0][j][c] + acc[1][j][c];   // X | Y
+      const double zpart = left ? acc[1][j][c] : acc[2][j][c];
+      const double z = zpart + __shfl_xor_sync(0xffffffffu, zpart, 2);
+      res[((left ? 0 : 1) * 4 + p0 + c) * B + i] = mine;
+      if (left) res[(2 * 4 + p0 + c) * B + i] = z;
+    }
+  }
+  __syncthreads();
+  const double hf = 0.5 * (double)(B - 1), inv_hf = 1.0 / hf;
+  const bool full = n0 + B <= prm.n && n0g >= v_lo && n0g + B <= v_hi;   // (block-uniform) a full tile of valid samples
+  for (int i = tid; i < B; i += kFirMmaThreads) {
+    const int n = n0 + i;
+    if (!full && n >= prm.n) break;
+    const double tau = ((double)i - hf) * inv_hf;
+    double v[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const double* r = res + (size_t)c * 4 * B + i;
+      v[c] = fma(fma(fma(r[3 * B], tau, r[2 * B]), tau, r[B]), tau, r[0]);
+    }
+    const bool valid = full || (n0g + i >= v_lo && n0g + i < v_hi);
+    fir_store(ob, N, n, channels, valid ? v[0] : 0.0, valid ? v[1] : 0.0, valid ? v[2] : 0.0);
+  }
+}
+#endif
 
 // ---------------------------------------------------------------------------------------- fix-up kernel
 // The tiles the plan flagged (a delay crosses a whole number of samples inside them) with the exact
