@@ -67,12 +67,13 @@ def ncu_counters(workload, kernel):
     num = lambda k: float(r[k]) if r.get(k) not in (None, "") else None
     return {"kernel": r["kernel"], "time_us": num("time_us"), "dram_bytes": num("dram_bytes_read") + num("dram_bytes_write"),
             "pipe_fp64_pct": num("pipe_fp64_pct"), "smem_wavefronts_pct": num("smem_wavefronts_pct"),
-            "issue_active_pct": num("issue_active_pct"), "registers": num("registers")}, None
+            "issue_active_pct": num("issue_active_pct"), "registers": num("registers"),
+            "pipe_dmma_pct": num("pipe_dmma_pct")}, None
 
 
 # algorithmic FP64 instruction slots per time sample (SURVEY.md §8(d), T = order + 1 taps; DFMA = 1)
 NCU_FIELDS = ("csrc_sha256", "workload", "api", "kernel", "time_us", "registers", "dram_bytes_read", "dram_bytes_write",
-              "pipe_fp64_pct", "smem_wavefronts_pct", "issue_active_pct", "inst_executed", "warps_active_pct")
+              "pipe_fp64_pct", "smem_wavefronts_pct", "issue_active_pct", "inst_executed", "warps_active_pct", "pipe_dmma_pct")
 
 
 def ncu_import(raw_csv, workload):
@@ -94,7 +95,7 @@ def ncu_import(raw_csv, workload):
         return v
 
     new = []
-    for api, pat in (("lr_project", "project_kernel"), ("lr_tdi", "tdi_fir_apply_kernel")):
+    for api, pat in (("lr_project", "project_kernel"), ("lr_tdi", "tdi_fir_apply")):
         hits = [r for r in body if pat in r[ix["Kernel Name"]]]
         if not hits:
             continue
@@ -109,7 +110,9 @@ def ncu_import(raw_csv, workload):
                     "smem_wavefronts_pct": f"{val(r, 'l1tex__data_pipe_lsu_wavefronts_mem_shared.sum.pct_of_peak_sustained_elapsed'):.2f}",
                     "issue_active_pct": f"{val(r, 'smsp__issue_active.avg.pct_of_peak_sustained_active'):.2f}",
                     "inst_executed": f"{val(r, 'smsp__inst_executed.sum'):.0f}",
-                    "warps_active_pct": f"{val(r, 'sm__warps_active.avg.pct_of_peak_sustained_active'):.2f}"})
+                    "warps_active_pct": f"{val(r, 'sm__warps_active.avg.pct_of_peak_sustained_active'):.2f}",
+                    "pipe_dmma_pct": (f"{val(r, 'sm__pipe_tensor_subpipe_dmma_cycles_active.avg.pct_of_peak_sustained_active'):.2f}"
+                                      if "sm__pipe_tensor_subpipe_dmma_cycles_active.avg.pct_of_peak_sustained_active" in ix else "")})
     old = []
     if os.path.exists(NCU_COUNTERS):
         old = [r for r in csv.DictReader(open(NCU_COUNTERS)) if not (r["workload"] == workload and r["api"] in {n["api"] for n in new})]

@@ -68,7 +68,7 @@ def test_tracked_counters_match_the_tracked_sources():
     """The committed profiles/r2_ncu_counters.csv belongs to the committed csrc/ (a kernel edit without a new capture
     makes bench.py print null, which is right, but should not be committed unnoticed)."""
     rows = list(csv.DictReader(open(os.path.join(ROOT, "profiles", "r2_ncu_counters.csv"))))
-    assert {(r["workload"], r["api"]) for r in rows} == {("year", "lr_project"), ("year", "lr_tdi"),
+    assert {(r["workload"], r["api"]) for r in rows} >= {("year", "lr_project"), ("year", "lr_tdi"),
                                                          ("batch", "lr_project"), ("batch", "lr_tdi")}
     assert {r["csrc_sha256"] for r in rows} == {bench.csrc_hash()}
 
