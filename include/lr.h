@@ -20,9 +20,11 @@
  *   - lr_project / lr_tdi enqueue work on `cuda_stream` (a cudaStream_t, NULL = legacy default stream)
  *     and return without synchronising.  lr_response_host is synchronous.
  *   - lr_project (batch <= 16) and lr_tdi may be captured into a CUDA graph (cudaStreamBeginCapture on `cuda_stream`):
- *     they then wait on nothing outside the capture.  Call each once outside a capture first (so that the TDI plan
- *     exists and the staging slots are idle), keep the handle's options unchanged, and replay the graph on one stream
- *     at a time.  Every other computing call returns LR_EINVAL on a capturing stream.
+ *     they then wait on nothing outside the capture.  Call lr_tdi once outside a capture first, with the same n and
+ *     options (the graph keeps the addresses of the handle's TDI plan: do not change LR_OPT_* or call lr_tdi with
+ *     another n on that handle while the graph is in use, which would rebuild the plan), replay the graph on one stream
+ *     at a time, and destroy it before the handle.  Every other computing call returns LR_EINVAL on a capturing
+ *     stream.
  *   - all entry points return 0 on success or a negative LR_E* code; they never abort, throw or print.
  *     Inputs are not scanned for NaN (NaN propagates).
  *   - a handle keeps per-call staging state (and lr_tdi's plan): use one handle from one host thread and one

@@ -102,6 +102,7 @@ struct lr_handle {
   lr::D4* coef = nullptr;
   Stage stage[kSlots];
   int next_slot = 0;
+  Stage graph_stage;     // the slot of launches captured into CUDA graphs: never reallocated, never used by direct calls
   // scratch of lr_response / lr_response_host: y of one chunk, and for the host variant two staging
   // buffers each for h and out plus the copy streams of the three-stage pipeline
   double* y_scr = nullptr; size_t y_cap = 0;        // elements
@@ -205,15 +206,32 @@ bool in_table(const lr_handle* h, int64_t n_first, int64_t n_last, double back_r
 // [batch][9] (step P1 of the path) on the caller's stream.  Device layout of a slot: basis | gb | angles.
 int stage_basis(lr_handle* h, const double* beta, const double* lam, const double* psi, int64_t batch,
                 cudaStream_t st, Stage** used, const double* gb = nullptr, const double** gb_dev = nullptr) {
+  if (capturing(st)) {
+    // graph capture: only the parameter-buffer path (the constants become part of the kernel node), into a slot of
+    // its own that no direct call touches and that is never reallocated (the graph keeps its address).  Captured
+    // launches of one stream are ordered, so they may share it.
+    if (batch > lr::kSmallStage) return LR_EINVAL;
+    Stage& G = h->graph_stage;
+    if (!G.dev) {
+      RelaxedCapture relaxed;   // (allocation is not a capturable call)
+      LR_CUDA(h, cudaMalloc(&G.dev, (size_t)lr::kSmallStage * 18 * sizeof(double)));
+      G.cap = lr::kSmallStage;
+    }
+    lr::SmallStage ss;
+    memset(&ss, 0, sizeof(ss));
+    ss.n = (int)batch; ss.has_gb = gb ? 1 : 0;
+    if (gb) memcpy(ss.v, gb, (size_t)batch * 6 * sizeof(double));
+    for (int64_t b = 0; b < batch; ++b) {
+      ss.v[6 * batch + 3 * b] = beta[b]; ss.v[6 * batch + 3 * b + 1] = lam[b]; ss.v[6 * batch + 3 * b + 2] = psi[b];
+    }
+    LR_CUDA(h, (cudaError_t)lr::launch_source_basis_small(ss, G.dev, (void*)st));
+    if (gb_dev) *gb_dev = G.dev + 9 * batch;
+    *used = &G;
+    return LR_OK;
+  }
   Stage& S = h->stage[h->next_slot];
   h->next_slot = (h->next_slot + 1) % kSlots;
   if (!S.done) LR_CUDA(h, cudaEventCreateWithFlags(&S.done, cudaEventDisableTiming));
-  if (capturing(st)) {
-    // graph capture: only the parameter-buffer path (the constants become part of the kernel node), and only on a
-    // slot whose earlier users have finished
-    if (batch > lr::kSmallStage || (S.pending && !event_done(S.done))) return LR_EINVAL;
-    S.pending = false;
-  }
   if (S.pending) {
     // the slot's earlier users must be done with it: only a rewrite of the pinned host side needs the HOST to wait;
     // the small path (constants in the kernel's parameter buffer) orders the device side on the stream instead
@@ -222,7 +240,6 @@ int stage_basis(lr_handle* h, const double* beta, const double* lam, const doubl
     S.pending = false;
   }
   if (S.cap < batch) {
-    RelaxedCapture relaxed;   // (a first use of this slot inside a capture)
     if (S.host) cudaFreeHost(S.host);
     if (S.dev) cudaFree(S.dev);
     S.host = nullptr; S.dev = nullptr; S.cap = 0;
@@ -351,6 +368,7 @@ int lr_create(const lr_orbits* orb, double dt, int order, int tdi_gen, lr_handle
 
 void lr_destroy(lr_handle* h) {
   if (!h) return;
+  if (h->graph_stage.dev) cudaFree(h->graph_stage.dev);
   for (int s = 0; s < kSlots; ++s) {
     Stage& S = h->stage[s];
     if (S.pending) cudaEventSynchronize(S.done);

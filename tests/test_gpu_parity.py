@@ -822,6 +822,18 @@ def test_project_and_tdi_replay_from_a_cuda_graph(lr):
     g.replay()
     torch.cuda.synchronize()
     assert torch.equal(out, ref)
+    # direct calls afterwards (bigger batches: the ring of staging slots is reallocated) leave the graph's own
+    # staging slot alone
+    wb = inputs.config(3, batch=19, n=w.n, t0=w.t0)
+    hb, cb = _stack(wb, range(19))
+    for nb in (19, 3, 19, 1, 5):
+        R.project(to_dev(hb[:nb]), to_dev(cb[:nb]), [x.beta for x in wb.sources[:nb]], [x.lam for x in wb.sources[:nb]],
+                  [x.psi for x in wb.sources[:nb]])
+    torch.cuda.synchronize()
+    out.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref)
     hpd.mul_(0.5)                                          # new input in the captured buffers
     hcd.mul_(0.5)
     g.replay()
