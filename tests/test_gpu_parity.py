@@ -947,6 +947,56 @@ def test_gpu_inner_product_parity(lr):
         lr.lr_inner_product(fh_d, fh_d, inv_d, 1.0, mode=7)
 
 
+def test_handles_release_their_device_memory(lr):
+    """lr_destroy gives back everything a handle took: spline coefficients, staging slots, the TDI plan (its own and
+    a shared one once the last reference goes), the y / h / spectrum scratch of the one-call paths and the cuFFT
+    plan.  Forty create / use / destroy cycles leave the free device memory where it was."""
+    import gc
+    import torch
+    w = inputs.config(3, batch=3, n=20011)
+    tab = w.table()
+    hp, hc = _stack(w, range(3))
+    hpd, hcd = to_dev(hp), to_dev(hc)
+    be, la, ps = ([getattr(s, k) for s in w.sources] for k in ("beta", "lam", "psi"))
+    gb = np.array([[s.A * (1.0 + np.cos(s.iota) ** 2), -2.0 * s.A * np.cos(s.iota), s.f0, s.fdot, 0.0, s.phi0]
+                   for s in w.sources])
+    nf = w.n // 2 + 1
+    inv = torch.ones((3, nf), dtype=torch.float64, device="cuda")
+    out = torch.empty((3, 3, w.n), dtype=torch.float64, device="cuda")
+    y = torch.empty((3, 6, w.n), dtype=torch.float64, device="cuda")
+    host_out = np.empty((3, 3, w.n))
+
+    def cycle():
+        R = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="AET")
+        R.project(hpd, hcd, be, la, ps, y_out=y)
+        R.tdi(y, out=out)
+        R.response(hpd, hcd, be, la, ps, out=out)
+        R.response_host(hp, hc, be, la, ps, host_out)
+        data_f = torch.fft.rfft(out[0], dim=-1).contiguous()
+        R.loglike_gb(gb, be, la, ps, w.n, data_f, inv, -2.0 * w.dt / w.n)
+        plan = R.create_plan(w.n)
+        R2 = lr.Response(tab, w.dt, w.order, 2, t0=w.t0, channels="AET")
+        R2.attach_plan(plan)
+        lr.lr_plan_release(plan)
+        R2.tdi(y, out=out)
+        torch.cuda.synchronize()
+        del data_f
+        R.close()
+        R2.close()
+
+    for _ in range(3):          # the library's and torch's one-time allocations (cuFFT module, caching allocator)
+        cycle()
+    gc.collect()
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    for _ in range(40):
+        cycle()
+    gc.collect()
+    torch.cuda.synchronize()
+    free1 = torch.cuda.mem_get_info()[0]
+    assert free0 - free1 <= 4 << 20, f"{(free0 - free1) / 2**20:.1f} MiB of device memory not returned after 40 cycles"
+
+
 # ---------------------------------------------------------------------------------------- edge cases
 def test_edge_cases_and_errors(lr):
     import torch
