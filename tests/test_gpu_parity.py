@@ -875,6 +875,51 @@ def test_project_and_tdi_replay_from_a_cuda_graph(lr):
         assert torch.equal(o2, ref2)
 
 
+def test_shared_plan_from_two_host_threads(lr):
+    """include/lr.h: handles that share a plan may be used from different host threads and streams at the same time
+    (each handle from one thread).  Two threads, each with its own handle, stream, y and out, 50 lr_tdi calls each on
+    one attached plan (ctypes releases the GIL during the calls): every result equals the single-threaded one."""
+    import threading
+    import torch
+    w = inputs.config(2, n=60011, f0=3e-3, t0=3.0e7)
+    tab = w.table()
+    s = w.sources[0]
+    hp, hc = w.waveform(0)
+    R0 = lr.Response(tab, w.dt, w.order, 2, t0=w.t0)
+    y = R0.project(to_dev(hp)[None], to_dev(hc)[None], [s.beta], [s.lam], [s.psi])
+    ys = [y, (y * 0.25).contiguous()]
+    refs = [R0.tdi(v).clone() for v in ys]
+    plan = R0.create_plan(w.n)
+    torch.cuda.synchronize()
+    errors = []
+
+    def worker(k):
+        try:
+            torch.cuda.set_device(0)
+            R = lr.Response(tab, w.dt, w.order, 2, t0=w.t0)
+            R.attach_plan(plan)
+            st = torch.cuda.Stream()
+            out = torch.empty_like(refs[k])
+            for _ in range(50):
+                out.zero_()
+                R.tdi(ys[k], out=out, stream=st)
+                st.synchronize()
+                if not torch.equal(out, refs[k]):
+                    errors.append((k, "mismatch"))
+                    return
+            R.close()
+        except Exception as e:   # pragma: no cover
+            errors.append((k, repr(e)))
+
+    threads = [threading.Thread(target=worker, args=(k,)) for k in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    lr.lr_plan_release(plan)
+    assert not errors, errors
+
+
 def test_binding_checks_out_against_the_channel_option(lr):
     """The C ABI takes no size for `out`: the binding checks it against the handle's LR_OPT_CHANNELS (lr_get_option),
     so a [B,3,N] buffer is never handed to a handle that writes six rows; angle arrays must match the batch."""
